@@ -1,0 +1,349 @@
+/*
+ * oracle/lp_oracle.c -- CPU ORACLE for the Lagrangian-Particle (LP) hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ * It shares no code, header, table or helper with the CUDA path under
+ * paper_2602_23434_b200/ and neither imports the other.
+ *
+ * Plain, slow, scalar fp64 C.  Compile with  gcc -O2 -ffp-contract=off  so that no
+ * a*b+c is fused: every + - * / sqrt floor below is one correctly rounded IEEE-754
+ * operation, evaluated in the order written.  (The CUDA path reproduces the
+ * key / gather / push arithmetic operation by operation so that indices and
+ * positions can be compared bit for bit; reading R14.)
+ *
+ * What it computes, with the passage of /root/reference/PAPER.md each part follows
+ * ("R<n>" = a reading listed in DESIGN.md section 3, taken where the paper is silent):
+ *
+ *   orc_bin_table        N_b log-spaced energy bins          PAPER.md:122, 282-284 (Eq. 13)      R1,R3
+ *   orc_cell_key         containing cell of x_LP             PAPER.md:81-85 (sampling)           R15
+ *   orc_sort_perm        order by (cell key, id)             not in the paper (north_star)       --
+ *   orc_gather           trilinear sampling of v,B,rho       PAPER.md:85 ("sample fluid ...")    R2
+ *   orc_push_stage0/1    two-stage predictor-corrector       PAPER.md:83 (Eq. 1), 218-227        R16
+ *   orc_coefficients     gamma_g, dtau, c_r, a               PAPER.md:85, 96-99 (Eq. 4), 105-107 R4-R9
+ *   orc_cfl_nsub         CFL-limited substep count           north_star                          R12
+ *   orc_spectral_row     donor-cell upwind update of chi     PAPER.md:107 (Eq. 6)                R1,R10,R11
+ *   orc_spectral_update  the three above for every particle  PAPER.md:218-231 (Particles_Spectra)
+ *   orc_step             one whole step with frozen fields   PAPER.md:216-233 (Table 1)
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force cell search and O(N^2)
+ * selection sort; constant / linear / cell-centre fields for the gather; uniform
+ * flow, the closed form Eq. 10 and homologous flow for the pusher;
+ * the analytic synchrotron-cooled power law, the adiabatic rho^{1/3} law, a
+ * scale-invariance product formula, the loss steady state, number conservation,
+ * positivity and hand-worked N_b = 2, 3 cases for the spectral update.
+ * No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct {
+    int32_t nx, ny, nz;        /* cells per axis; cell-centred data, index (k*ny + j)*nx + i   */
+    double  xlo[3], xhi[3];    /* domain                                                         */
+    int32_t periodic[3];       /* 1: periodic axis, 0: zero-gradient (clamped) axis              */
+    int32_t nbins;             /* N_b                                                            */
+    double  e_min, e_max;      /* outer bin edges                                                */
+    double  kappa, u_rad;      /* c_r = kappa * (|B|^2/2 + u_rad)          (Eq. 4, R4-R6)        */
+    double  cfl_e;             /* C_E, energy-space CFL number             (R12)                 */
+    int32_t max_substeps;      /* cap on n_sub                             (R12)                 */
+} orc_params;
+
+/* ---------------------------------------------------------------- bins (R1, R3) */
+
+/* N_b+1 log-spaced edges spanning exactly [e_min, e_max]; widths; geometric centres.
+ * PAPER.md:122 defers the discretisation to [19]; Eq. 13 indexes
+ * "N_b energy bins between e_min and e_max". */
+void orc_bin_table(int32_t nbins, double e_min, double e_max,
+                   double *E /*[nbins+1]*/, double *dE /*[nbins]*/, double *Ec /*[nbins]*/)
+{
+    for (int k = 0; k <= nbins; ++k)
+        E[k] = e_min * pow(e_max / e_min, (double)k / (double)nbins);
+    for (int i = 0; i < nbins; ++i) {
+        dE[i] = E[i + 1] - E[i];
+        Ec[i] = sqrt(E[i] * E[i + 1]);
+    }
+}
+
+/* ---------------------------------------------------------------- cell key (R15) */
+
+static int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+/* Containing cell per axis c = floor((x - xlo) * inv_dx), inv_dx = n / (xhi - xlo),
+ * clamped to [0, n-1]; a face belongs to the upper cell.  key = (ck*ny + cj)*nx + ci. */
+void orc_cell_key(const orc_params *g, int64_t np,
+                  const double *x, const double *y, const double *z, uint32_t *key)
+{
+    const double idx = (double)g->nx / (g->xhi[0] - g->xlo[0]);
+    const double idy = (double)g->ny / (g->xhi[1] - g->xlo[1]);
+    const double idz = (double)g->nz / (g->xhi[2] - g->xlo[2]);
+    for (int64_t p = 0; p < np; ++p) {
+        int ci = clampi((int)floor((x[p] - g->xlo[0]) * idx), 0, g->nx - 1);
+        int cj = clampi((int)floor((y[p] - g->xlo[1]) * idy), 0, g->ny - 1);
+        int ck = clampi((int)floor((z[p] - g->xlo[2]) * idz), 0, g->nz - 1);
+        key[p] = (uint32_t)((ck * g->ny + cj) * g->nx + ci);
+    }
+}
+
+/* ---------------------------------------------------------------- sort */
+
+typedef struct { uint32_t key; uint64_t id; int64_t src; } orc_sort_rec;
+
+static int orc_cmp(const void *a, const void *b)
+{
+    const orc_sort_rec *p = (const orc_sort_rec *)a, *q = (const orc_sort_rec *)b;
+    if (p->key != q->key) return p->key < q->key ? -1 : 1;
+    if (p->id != q->id)   return p->id < q->id ? -1 : 1;
+    return 0;
+}
+
+/* perm[n] = index (in the current order) of the particle that comes n-th when ordered
+ * ascending by (key, id).  ids are unique, so the order is total and perm is unique. */
+void orc_sort_perm(int64_t np, const uint32_t *key, const uint64_t *id, int64_t *perm)
+{
+    orc_sort_rec *r = (orc_sort_rec *)malloc((size_t)np * sizeof *r);
+    for (int64_t p = 0; p < np; ++p) { r[p].key = key[p]; r[p].id = id[p]; r[p].src = p; }
+    qsort(r, (size_t)np, sizeof *r, orc_cmp);
+    for (int64_t p = 0; p < np; ++p) perm[p] = r[p].src;
+    free(r);
+}
+
+/* ---------------------------------------------------------------- gather (R2) */
+
+static int wrap_index(int i, int n, int periodic)
+{
+    if (periodic) { int m = i % n; return m < 0 ? m + n : m; }
+    return clampi(i, 0, n - 1);
+}
+
+/* Trilinear interpolation of nq cell-centred fields at one position.
+ * Per axis: s = (x - xlo)*inv_dx - 1/2, i0 = floor(s), f = s - i0; neighbours i0, i0+1
+ * mapped by floor-mod (periodic) or clamped (zero gradient, as the outflow BC of
+ * PAPER.md:276).  Corners are summed z outer, y, x inner; weight = (wz*wy)*wx. */
+static void gather_point(const orc_params *g, int nq, const double *const *q,
+                         double px, double py, double pz, double *out)
+{
+    const double idx = (double)g->nx / (g->xhi[0] - g->xlo[0]);
+    const double idy = (double)g->ny / (g->xhi[1] - g->xlo[1]);
+    const double idz = (double)g->nz / (g->xhi[2] - g->xlo[2]);
+    double sx = (px - g->xlo[0]) * idx - 0.5, sy = (py - g->xlo[1]) * idy - 0.5,
+           sz = (pz - g->xlo[2]) * idz - 0.5;
+    double fx0 = floor(sx), fy0 = floor(sy), fz0 = floor(sz);
+    double fx = sx - fx0, fy = sy - fy0, fz = sz - fz0;
+    int i0 = (int)fx0, j0 = (int)fy0, k0 = (int)fz0;
+    int ii[2] = { wrap_index(i0, g->nx, g->periodic[0]), wrap_index(i0 + 1, g->nx, g->periodic[0]) };
+    int jj[2] = { wrap_index(j0, g->ny, g->periodic[1]), wrap_index(j0 + 1, g->ny, g->periodic[1]) };
+    int kk[2] = { wrap_index(k0, g->nz, g->periodic[2]), wrap_index(k0 + 1, g->nz, g->periodic[2]) };
+    double wx[2] = { 1.0 - fx, fx }, wy[2] = { 1.0 - fy, fy }, wz[2] = { 1.0 - fz, fz };
+    for (int m = 0; m < nq; ++m) out[m] = 0.0;
+    for (int cz = 0; cz < 2; ++cz)
+        for (int cy = 0; cy < 2; ++cy)
+            for (int cx = 0; cx < 2; ++cx) {
+                double w = (wz[cz] * wy[cy]) * wx[cx];
+                int64_t c = ((int64_t)kk[cz] * g->ny + jj[cy]) * g->nx + ii[cx];
+                for (int m = 0; m < nq; ++m) out[m] = out[m] + w * q[m][c];
+            }
+}
+
+/* out[m*np + p] = field m at particle p, m = 0..6 in the order vx,vy,vz,bx,by,bz,rho. */
+void orc_gather(const orc_params *g, const double *const *fields7, int64_t np,
+                const double *x, const double *y, const double *z, double *out7)
+{
+    for (int64_t p = 0; p < np; ++p) {
+        double o[7];
+        gather_point(g, 7, fields7, x[p], y[p], z[p], o);
+        for (int m = 0; m < 7; ++m) out7[(int64_t)m * np + p] = o[m];
+    }
+}
+
+/* ---------------------------------------------------------------- push (Eq. 1, R16) */
+
+/* Stage 0 (Particles_RK#1): k1 = v(x^n), rho_old = rho(x^n),
+ * x* = x^n + dt*k1.  x* is not wrapped (the gather wraps indices). */
+void orc_push_stage0(const orc_params *g, const double *const *fields7, int64_t np,
+                     const double *x, const double *y, const double *z, double dt,
+                     double *k1 /*[3][np]*/, double *rho_old /*[np]*/, double *xs /*[3][np]*/,
+                     int32_t nthreads)
+{
+    const double *q[4] = { fields7[0], fields7[1], fields7[2], fields7[6] };
+    (void)nthreads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads > 0 ? nthreads : 1)
+#endif
+    for (int64_t p = 0; p < np; ++p) {
+        double o[4];
+        gather_point(g, 4, q, x[p], y[p], z[p], o);
+        k1[p] = o[0]; k1[np + p] = o[1]; k1[2 * np + p] = o[2];
+        rho_old[p] = o[3];
+        xs[p]          = x[p] + dt * o[0];
+        xs[np + p]     = y[p] + dt * o[1];
+        xs[2 * np + p] = z[p] + dt * o[2];
+    }
+}
+
+/* Periodic wrap into [lo, hi): x -= L*floor((x-lo)/L); a result >= hi becomes lo. */
+static double wrap_pos(double x, double lo, double hi)
+{
+    double L = hi - lo;
+    x = x - L * floor((x - lo) / L);
+    if (x >= hi) x = lo;
+    return x;
+}
+
+/* Stage 1 (Particles_RK#2 + Particles_Boundary): k2 = v(x*) from
+ * the fields passed now (the caller may have advanced them);
+ * x^{n+1} = x^n + (dt/2)*(k1 + k2)  (Heun).  Periodic axes are wrapped; on a
+ * non-periodic axis the position is kept and bit (1 << axis) of status is set when
+ * it lies outside [lo, hi). */
+void orc_push_stage1(const orc_params *g, const double *const *fields7, int64_t np,
+                     double *x, double *y, double *z, const double *xs, const double *k1,
+                     double dt, int32_t *status /*[np] or NULL*/, int32_t nthreads)
+{
+    const double *q[3] = { fields7[0], fields7[1], fields7[2] };
+    double *pos[3] = { x, y, z };
+    const double hdt = 0.5 * dt;
+    (void)nthreads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads > 0 ? nthreads : 1)
+#endif
+    for (int64_t p = 0; p < np; ++p) {
+        double k2[3];
+        int32_t st = 0;
+        gather_point(g, 3, q, xs[p], xs[np + p], xs[2 * np + p], k2);
+        for (int d = 0; d < 3; ++d) {
+            double xn = pos[d][p] + hdt * (k1[(int64_t)d * np + p] + k2[d]);
+            if (g->periodic[d]) xn = wrap_pos(xn, g->xlo[d], g->xhi[d]);
+            else if (xn < g->xlo[d] || xn >= g->xhi[d]) st |= (1 << d);
+            pos[d][p] = xn;
+        }
+        if (status) status[p] = st;
+    }
+}
+
+/* ---------------------------------------------------------------- coefficients (R4-R9) */
+
+/* From v, B, rho_new gathered at x^{n+1} and rho_old gathered at x^n:
+ *   gamma_g = 1/sqrt(1 - |v|^2)  (c = 1),  dtau = dt/gamma_g
+ *   c_r     = kappa*(|B|^2/2 + u_rad)                                  PAPER.md:96-99 (Eq. 4)
+ *   a       = -log(rho_new/rho_old)/(3 dtau)  = (1/3) div_mu u^mu      PAPER.md:105 (continuity), R7
+ * so that d(eps)/d(tau) = -eps*(a + c_r*eps) is the bracket of Eq. 6. */
+void orc_coefficients(const orc_params *g, double dt, const double v[3], const double B[3],
+                      double rho_new, double rho_old, double *a, double *cr, double *dtau)
+{
+    double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+    double b2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+    double gam = 1.0 / sqrt(1.0 - v2);
+    *dtau = dt / gam;
+    *cr = g->kappa * (0.5 * b2 + g->u_rad);
+    *a = -log(rho_new / rho_old) / (3.0 * *dtau);
+}
+
+/* ---------------------------------------------------------------- CFL (R12) */
+
+/* Edge velocities w_k = -E_k*(a + c_r*E_k); outflow rate of bin i is
+ * (max(w_{i+1},0) - min(w_i,0))/dE_i; lambda = max over bins;
+ * n_sub = max(1, ceil(dtau*lambda/C_E)), capped at max_substeps (return value's
+ * sign is flipped when the cap was applied so that the caller can count it). */
+int32_t orc_cfl_nsub(int32_t nbins, const double *E, const double *dE, double a, double cr,
+                     double dtau, double cfl_e, int32_t max_substeps, double *lambda_out)
+{
+    double lam = 0.0;
+    for (int i = 0; i < nbins; ++i) {
+        double wl = -E[i] * (a + cr * E[i]);
+        double wr = -E[i + 1] * (a + cr * E[i + 1]);
+        double out = (fmax(wr, 0.0) - fmin(wl, 0.0)) / dE[i];
+        if (out > lam) lam = out;
+    }
+    if (lambda_out) *lambda_out = lam;
+    double need = ceil(dtau * lam / cfl_e);
+    int32_t n = need < 1.0 ? 1 : (need > 2.0e9 ? 2000000000 : (int32_t)need);
+    if (n > max_substeps) return -max_substeps;
+    return n;
+}
+
+/* ---------------------------------------------------------------- substeps (Eq. 6, R1, R10, R11) */
+
+/* n_sub explicit donor-cell steps of  d(chi)/d(tau) + d/d(eps)[w chi] = 0:
+ *   F_k   = max(w_k,0)*chi_{k-1} + min(w_k,0)*chi_k      (interior edges)
+ *   F_0   = min(w_0,0)*chi_0,  F_Nb = max(w_Nb,0)*chi_{Nb-1}   (no inflow, free outflow)
+ *   chi_i <- chi_i - (dtau_s/dE_i)*(F_{i+1} - F_i),   dtau_s = dtau/n_sub
+ * lost accumulates dtau_s*(F_Nb - F_0), the number that left through the ends. */
+void orc_spectral_row(int32_t nbins, const double *E, const double *dE, double a, double cr,
+                      double dtau, int32_t nsub, double *chi /*[nbins] in/out*/, double *lost)
+{
+    double *w = (double *)malloc((size_t)(nbins + 1) * sizeof(double));
+    double *F = (double *)malloc((size_t)(nbins + 1) * sizeof(double));
+    const double dts = dtau / (double)nsub;
+    double lo = 0.0;
+    for (int k = 0; k <= nbins; ++k) w[k] = -E[k] * (a + cr * E[k]);
+    for (int s = 0; s < nsub; ++s) {
+        F[0] = fmin(w[0], 0.0) * chi[0];
+        for (int k = 1; k < nbins; ++k)
+            F[k] = fmax(w[k], 0.0) * chi[k - 1] + fmin(w[k], 0.0) * chi[k];
+        F[nbins] = fmax(w[nbins], 0.0) * chi[nbins - 1];
+        for (int i = 0; i < nbins; ++i)
+            chi[i] = chi[i] - (dts / dE[i]) * (F[i + 1] - F[i]);
+        lo = lo + dts * (F[nbins] - F[0]);
+    }
+    if (lost) *lost = lo;
+    free(w); free(F);
+}
+
+/* number of a row: sum_i chi_i dE_i  (diagnostic a10) */
+double orc_row_number(int32_t nbins, const double *dE, const double *chi)
+{
+    double s = 0.0;
+    for (int i = 0; i < nbins; ++i) s = s + chi[i] * dE[i];
+    return s;
+}
+
+/* ---------------------------------------------------------------- whole update / step */
+
+/* Particles_Spectra: for every particle, gather v,B,rho at the
+ * current position from the current fields, form the coefficients, the substep count
+ * and run the substeps on its row chi[p*nbins .. ].  nsub_out gets n_sub (negative if
+ * capped), lost_out the number lost this call.  nthreads > 1 splits the particle loop
+ * with OpenMP (here and in the two push stages); the arithmetic per particle is unchanged. */
+void orc_spectral_update(const orc_params *g, const double *const *fields7, int64_t np,
+                         const double *x, const double *y, const double *z,
+                         const double *rho_old, double dt, double *chi /*[np][nbins]*/,
+                         int32_t *nsub_out /*or NULL*/, double *lost_out /*or NULL*/,
+                         int32_t nthreads)
+{
+    const int nb = g->nbins;
+    double *E = (double *)malloc((size_t)(nb + 1) * sizeof(double));
+    double *dE = (double *)malloc((size_t)nb * sizeof(double));
+    double *Ec = (double *)malloc((size_t)nb * sizeof(double));
+    orc_bin_table(nb, g->e_min, g->e_max, E, dE, Ec);
+    (void)nthreads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads > 0 ? nthreads : 1)
+#endif
+    for (int64_t p = 0; p < np; ++p) {
+        double o[7], a, cr, dtau, lost;
+        gather_point(g, 7, fields7, x[p], y[p], z[p], o);
+        orc_coefficients(g, dt, &o[0], &o[3], o[6], rho_old[p], &a, &cr, &dtau);
+        int32_t n = orc_cfl_nsub(nb, E, dE, a, cr, dtau, g->cfl_e, g->max_substeps, NULL);
+        orc_spectral_row(nb, E, dE, a, cr, dtau, n < 0 ? -n : n, chi + p * nb, &lost);
+        if (nsub_out) nsub_out[p] = n;
+        if (lost_out) lost_out[p] = lost;
+    }
+    free(E); free(dE); free(Ec);
+}
+
+/* One step with frozen fields (the build's lp_step): stage 0, stage 1 + wrap,
+ * spectral update at x^{n+1} with rho_old from stage 0.  Order of Table 1
+ * with the fluid stages removed. */
+void orc_step(const orc_params *g, const double *const *fields7, int64_t np,
+              double *x, double *y, double *z, double dt, double *chi,
+              int32_t *nsub_out, double *lost_out, int32_t *status, int32_t nthreads)
+{
+    double *k1 = (double *)malloc((size_t)np * 3 * sizeof(double));
+    double *xs = (double *)malloc((size_t)np * 3 * sizeof(double));
+    double *rho_old = (double *)malloc((size_t)np * sizeof(double));
+    orc_push_stage0(g, fields7, np, x, y, z, dt, k1, rho_old, xs, nthreads);
+    orc_push_stage1(g, fields7, np, x, y, z, xs, k1, dt, status, nthreads);
+    orc_spectral_update(g, fields7, np, x, y, z, rho_old, dt, chi, nsub_out, lost_out, nthreads);
+    free(k1); free(xs); free(rho_old);
+}
