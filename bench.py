@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- particle-steps/s of the LP hot path on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 1..5]
+
+A "step" is one lp_step (sort when due -> push 0 -> push 1 -> spectral update) over the whole
+particle set of the workload (default: BASELINE.json configs[3], "Large single-GPU load").
+`value` is device-timed with the state resident in HBM; `e2e` goes through lp_step_host with
+pinned HOST buffers (H2D + D2H inside the timed region).  `roofline` is for the dominant kernel
+(the spectral update), timed with CUDA events on its own stream inside the timed region.
+`cpu_baseline` times the CPU oracle (test infrastructure) on a bounded sample on the host cores.
+N > 1 (torchrun): particles are independent, so every rank runs its own particle set on a replica
+of the grid -- no data-path collective; "scaling": "weak".
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle-steps/sec"
+UNIT = "particle-steps/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", type=int, default=4)
+    ap.add_argument("--nbins", type=int, default=0, help="override the bin count (workload 5 sweep)")
+    ap.add_argument("--np", type=int, default=0, help="override the particle count (debugging only)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def stored_traffic(wname, nbins):
+    """dram bytes per spectral launch from the committed ncu --set full summary, or None."""
+    p = os.path.join(ROOT, "profiles", "spectral_traffic.json")
+    try:
+        return json.load(open(p)).get("%s/nb%d" % (wname, nbins))
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                r = self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.004)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def pick_workload(args):
+    import lp_inputs as I
+    w = I.workload(args.workload)
+    kw = {}
+    if args.nbins:
+        kw["nbins"] = args.nbins
+    if args.np:
+        kw["np"] = args.np
+    return w.scaled(**kw) if kw else w
+
+
+def step_dt(w):
+    if w.dt > 0:
+        return w.dt
+    import lp_inputs as I          # workload 1: dt from the loss CFL (reading R13)
+    E = I.bin_edges(w.nbins, w.e_min, w.e_max)
+    lam_top = w.kappa * 0.5 * w.b0 ** 2 * E[-2] ** 2 / (E[-1] - E[-2])
+    return 0.9 * w.cfl_e / lam_top
+
+
+def config_dict(w, n_gpus):
+    return {"workload": "BASELINE.json configs[%d] %s" % (w.index - 1, w.name), "grid": "%d^3" % w.n,
+            "particles_per_gpu": w.np, "nbins": w.nbins, "sort_every": w.sort_every,
+            "parallelism": "replicas x%d (particles independent, no collective)" % n_gpus,
+            "l2": "inputs larger than L2 (chi rows %.2f GB per GPU)" % (w.np * w.nbins * 8 / 1e9)}
+
+
+# ------------------------------------------------------------------------------- CPU oracle legs
+
+def oracle_state(w, fields_np, u_rad, x, y, z, pid, chi, nsel):
+    from oracle import lp_oracle as orc
+    prm = orc.make_params(w.n, w.n, w.n, w.xlo, w.xhi, w.periodic, w.nbins, w.e_min, w.e_max,
+                          kappa=w.kappa, u_rad=u_rad, cfl_e=w.cfl_e, max_substeps=w.max_substeps)
+    return orc, prm, [a[:nsel].copy() for a in (x, y, z, pid)] + [chi[:nsel].copy()]
+
+
+def oracle_steps(orc, prm, fields_np, st, dt, nsteps, sort_every, step0, threads):
+    """nsteps oracle steps (with its own sort every sort_every steps) on the sample; returns seconds."""
+    x, y, z, pid, chi = st
+    t0 = time.perf_counter()
+    for s in range(nsteps):
+        if sort_every and (step0 + s) % sort_every == 0:
+            perm = orc.sort_perm(orc.cell_key(prm, x, y, z), pid)
+            x, y, z, pid, chi = x[perm], y[perm], z[perm], pid[perm], chi[perm]
+        x, y, z, chi, nsub, lost, status = orc.step(prm, fields_np, x, y, z, dt, chi, nthreads=threads)
+    el = time.perf_counter() - t0
+    st[:] = [x, y, z, pid, chi]
+    return el
+
+
+def cpu_baseline(w, fields_np, u_rad, x, y, z, pid, chi_host_fn, dt, seconds):
+    threads = os.cpu_count() or 1
+    ncal = min(w.np, 32768)
+    orc, prm, st = oracle_state(w, fields_np, u_rad, x, y, z, pid, chi_host_fn(ncal), ncal)
+    t = oracle_steps(orc, prm, fields_np, st, dt, 1, 0, 1, threads)
+    rate = ncal / max(t, 1e-6)
+    nsteps = 2
+    nsel = int(min(w.np, max(ncal, rate * seconds / nsteps)))
+    orc, prm, st = oracle_state(w, fields_np, u_rad, x, y, z, pid, chi_host_fn(nsel), nsel)
+    t = oracle_steps(orc, prm, fields_np, st, dt, nsteps, w.sort_every, 0, threads)
+    return {"value": nsel * nsteps / t, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "first %d particles of the workload, %d steps (one sort), %.1f s, full %d^3 fields"
+                      % (nsel, nsteps, t, w.n)}
+
+
+# ------------------------------------------------------------------------------- inputs
+
+def make_inputs(w, device):
+    """fields on `device`, u_rad, positions/ids (numpy) and a function building chi rows."""
+    import numpy as np
+    import torch
+    import lp_inputs as I
+    fields = I.make_fields(w, device=device)
+    u_rad = w.u_rad_frac * I.mean_magnetic_energy(fields) if w.u_rad_frac > 0 else 0.0
+    x, y, z, pid = I.make_particles(w, shuffle_ids=True)
+    row = I.make_spectrum(w.scaled(np=1), jitter=False)[0]
+    amp = 1.0 + 0.5 * np.random.Generator(np.random.PCG64(w.seed + 2000)).uniform(size=w.np)
+
+    def chi_host(n):
+        return amp[:n, None] * row[None, :]
+
+    def chi_device():
+        return (torch.from_numpy(amp).to(device)[:, None] * torch.from_numpy(row).to(device)[None, :]).contiguous()
+
+    return fields, u_rad, x, y, z, pid, chi_host, chi_device
+
+
+# ------------------------------------------------------------------------------- arms
+
+def run_reference(args):
+    """The oracle, as it stands, on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import torch
+    w = pick_workload(args)
+    dt = step_dt(w)
+    dev = "cuda" if torch.cuda.is_available() else "cpu"      # input synthesis only
+    fields, u_rad, x, y, z, pid, chi_host, _ = make_inputs(w, dev)
+    fields_np = [f.cpu().numpy() for f in fields]
+    del fields
+    threads = os.cpu_count() or 1
+    ncal = min(w.np, 32768)
+    orc, prm, st = oracle_state(w, fields_np, u_rad, x, y, z, pid, chi_host(ncal), ncal)
+    rate = ncal / max(oracle_steps(orc, prm, fields_np, st, dt, 1, 0, 1, threads), 1e-6)
+    budget = 120.0                                            # seconds for warmup + steps
+    nsel = int(min(w.np, max(4096, rate * budget / max(1, args.steps + args.warmup))))
+    orc, prm, st = oracle_state(w, fields_np, u_rad, x, y, z, pid, chi_host(nsel), nsel)
+    oracle_steps(orc, prm, fields_np, st, dt, args.warmup, w.sort_every, 0, threads)
+    t = oracle_steps(orc, prm, fields_np, st, dt, args.steps, w.sort_every, args.warmup, threads)
+    value = nsel * args.steps / t
+    sample = "first %d particles per step (bounded sample of %d), full %d^3 fields" % (nsel, w.np, w.n)
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "config": config_dict(w, args.gpus),
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import paper_2602_23434_b200 as P
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device: the product has no CPU path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    w = pick_workload(args)
+    if rank:
+        w = w.scaled(seed=w.seed + 7919 * rank)          # every rank its own particle set (and grid)
+    dt = step_dt(w)
+    fields, u_rad, x, y, z, pid, chi_host, chi_device = make_inputs(w, dev)
+    lp = P.LP(P.config_from_workload(w, u_rad=u_rad, device=local))
+    lp.set_fields(fields)
+    lp.bind_particles(x, y, z, pid, chi_device())
+    B = P.binding
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        lp.step(dt)
+    barrier()
+    B.lp_timing_enable(lp.ctx, args.steps)
+    launches0 = lp.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        lp.step(dt)
+    e1.record()
+    torch.cuda.synchronize(dev)
+    clocks = sampler.stop()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = lp.launch_count() - launches0
+    spec_ms, spec_n = B.lp_timing_read(lp.ctx)
+    B.lp_timing_enable(lp.ctx, 0)
+    d = lp.diag()
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * w.np * args.steps / (ms * 1e-3)
+
+    # ---- end to end through lp_step_host: pinned host buffers, H2D + D2H every step
+    e2e = None
+    if not args.no_e2e:
+        hx, hy, hz = (t.cpu().pin_memory() for t in (lp.x, lp.y, lp.z))
+        hid = lp.id.cpu().pin_memory()
+        hchi = lp.chi.cpu().pin_memory()
+        lp.step_host(dt, hx, hy, hz, hid, hchi)             # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            lp.step_host(dt, hx, hy, hz, hid, hchi)         # synchronises the stream itself
+        torch.cuda.synchronize(dev)
+        te = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([te], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            te = float(t.item())
+        nbytes = w.np * (8 * w.nbins + 32)
+        e2e = {"value": world * w.np * args.e2e_steps / te, "unit": UNIT, "h2d_bytes_per_step": nbytes,
+               "d2h_bytes_per_step": nbytes, "steps": args.e2e_steps,
+               "api": "lp_step_host (pinned host x,y,z,id,chi in and out every step)"}
+        del hx, hy, hz, hid, hchi
+
+    if rank != 0:
+        return
+    peak, peak_src = measured_peak()
+    alg_bytes = (16 * w.nbins + 32) * w.np                   # chi r+w, x,y,z, rho_old
+    spec_avg_ms = spec_ms / max(spec_n, 1)
+    achieved = alg_bytes / (spec_avg_ms * 1e-3) / 1e9 if spec_n else None
+    roofline = {"bound": "hbm", "kernel": "lp_spectral_kernel<%d>" % w.nbins, "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
+                "traffic": stored_traffic(w.name, w.nbins), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": spec_avg_ms,
+                "share_of_step": spec_ms / ms if ms else None}
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world),
+           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+           "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],
+                    "sorts_total": d["sorts"]}}
+    if world == 1 and not args.no_cpu_baseline:
+        fields_np = [f.cpu().numpy() for f in fields]
+        out["cpu_baseline"] = cpu_baseline(w, fields_np, u_rad, x, y, z, pid, chi_host, dt, args.cpu_seconds)
+    print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.barrier()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+        try:
+            import torch.distributed as dist
+            if dist.is_initialized():
+                dist.destroy_process_group()
+        except Exception:
+            pass
+
+
+if __name__ == "__main__":
+    main()

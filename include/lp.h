@@ -1,0 +1,153 @@
+/*
+ * lp.h -- C ABI of the B200-native Lagrangian-Particle (LP) hot path.
+ *
+ * The library advances N_p macro-particles through one time step of the LP module of
+ * arxiv/paper_2602_23434 (/root/reference/PAPER.md, cited below as PAPER.md:<line>):
+ *   1. sample the cell-centred fluid state (v, B, rho) at x_LP      PAPER.md:81-85 (Eq. 1 and text)
+ *   2. advance x_LP with a two-stage predictor-corrector            PAPER.md:83, 218-227 (Table 1:
+ *                                                                    Particles_RK#1/#2, _Boundary)
+ *   3. update each particle's spectrum chi(eps) on N_b log bins by   PAPER.md:87-108 (Eq. 2-6),
+ *      a conservative upwind, CFL-substepped solve of Eq. 6          218-231 (Particles_Spectra)
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ * The precise arithmetic (and the readings taken where the paper is silent) is in DESIGN.md.
+ *
+ * Conventions
+ *  - All arithmetic is IEEE fp64.  Cell keys are uint32, ids uint64, substep counts int32.
+ *  - Grid arrays are cell-centred, [nz][ny][nx] with i (x) fastest.
+ *  - chi is particle-major: chi[p*nbins + i], i = 0..nbins-1 (as chi_ of Listing 3).
+ *  - Unless a parameter says "host", every pointer is a DEVICE pointer on `device`, BORROWED:
+ *    the caller owns it and keeps it alive until the stream it was used on is synchronised.
+ *    The library allocates only small tables itself; bulk scratch is the caller's workspace.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls only enqueue
+ *    work on it and return; lp_get_diag and the *_host call are the ones that synchronise.
+ *  - Every function returns an lp_status; nothing aborts, throws or prints.
+ *    lp_last_error gives a human-readable detail for the last failure on that context.
+ */
+#ifndef LP_H
+#define LP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define LP_API __attribute__((visibility("default")))
+#else
+#define LP_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    LP_OK              =  0,
+    LP_ERR_INVALID_ARG = -1,   /* NULL where not allowed, bad size, bad struct_size          */
+    LP_ERR_STATE       = -2,   /* call order: fields/particles/workspace not set, stage order */
+    LP_ERR_CUDA        = -3,   /* a CUDA runtime/driver call failed (see lp_last_error)      */
+    LP_ERR_UNSUPPORTED = -4,   /* nbins not in {16,32,64,128,256,512}; grid > 2^31 cells      */
+    LP_ERR_WORKSPACE   = -5    /* workspace missing, misaligned or smaller than required      */
+} lp_status;
+
+typedef struct lp_ctx lp_ctx;  /* opaque; owned by the library, released by lp_destroy */
+
+typedef struct {
+    uint32_t struct_size;      /* = sizeof(lp_config), checked                                   */
+    int32_t  nx, ny, nz;       /* cells per axis                                                  */
+    double   xlo[3], xhi[3];   /* domain; cell (i,j,k) covers xlo + [i,i+1)*dx ...                */
+    int32_t  periodic[3];      /* 1 periodic, 0 zero-gradient (clamped stencil)     */
+    int64_t  np;               /* particles                                                       */
+    int32_t  nbins;            /* N_b in {16,32,64,128,256,512}; log-spaced edges on [e_min,e_max] */
+    double   e_min, e_max;
+    double   kappa, u_rad;     /* c_r = kappa*(|B|^2/2 + u_rad)   (Eq. 4)         */
+    double   cfl_e;            /* energy-space CFL number C_E, 0 < C_E <= 1                       */
+    int32_t  max_substeps;     /* cap on n_sub (>= 1); capped particles are counted in lp_diag    */
+    int32_t  sort_every;       /* lp_step re-sorts by cell every this many steps; 0 = never       */
+    int32_t  device;           /* CUDA device ordinal                                             */
+} lp_config;
+
+typedef struct {
+    int64_t np;
+    int64_t sum_substeps;      /* sum over particles of n_sub of the last spectral update        */
+    int32_t max_substeps;      /* max over particles                                              */
+    int64_t n_capped;          /* particles whose n_sub hit config.max_substeps                   */
+    int64_t n_outside;         /* particles outside the box on a non-periodic axis                */
+    double  number;            /* sum_p sum_i chi_i dE_i now                                      */
+    double  lost;              /* sum_p number that left through the energy ends, last update     */
+    int64_t steps;             /* lp_step calls so far                                            */
+    int64_t sorts;             /* sorts so far                                                    */
+} lp_diag;
+
+/* Create / destroy.  lp_create validates the config, selects the device, builds the bin table
+ * (E_k = e_min*(e_max/e_min)^(k/N_b)) and uploads it.  *out is NULL on error
+ * except that a context is still returned for LP_ERR_CUDA so lp_last_error can be read. */
+LP_API lp_status lp_create(const lp_config *cfg, lp_ctx **out);
+LP_API lp_status lp_destroy(lp_ctx *ctx);
+LP_API const char *lp_last_error(const lp_ctx *ctx);     /* host string, valid until the next call */
+
+/* Bytes of caller-supplied device scratch the context needs (repacked grid records, stage
+ * buffers k1, x_star, rho_old, coefficients, sort buffers and the alternate chi rows used by the
+ * re-sort).  Bind a 256-byte aligned device buffer of at least that size before any other call. */
+LP_API lp_status lp_workspace_bytes(const lp_config *cfg, size_t *out_bytes /*host*/);
+LP_API lp_status lp_bind_workspace(lp_ctx *ctx, void *workspace, size_t bytes);
+
+/* Particle state, advanced in place: positions x,y,z [np], ids [np] (unique), chi [np][nbins]
+ * (16-byte aligned).  What a particle carries: PAPER.md:598-613 (Listing 3). */
+LP_API lp_status lp_bind_particles(lp_ctx *ctx, double *x, double *y, double *z, uint64_t *id, double *chi);
+
+/* Optional per-particle outputs of the spectral update: n_sub [np] (negative = capped) and
+ * the number lost through the energy boundaries in that update [np].  NULL = not written. */
+LP_API lp_status lp_bind_diag(lp_ctx *ctx, int32_t *nsub, double *lost);
+
+/* Stage the fluid state (7 cell-centred arrays [nz][ny][nx]) for the gathers: repacked into
+ * interleaved per-cell records inside the workspace; the inputs are not referenced afterwards.
+ * May be called between lp_push stages (time-dependent fields). */
+LP_API lp_status lp_set_fields(lp_ctx *ctx, const double *vx, const double *vy, const double *vz,
+                        const double *bx, const double *by, const double *bz, const double *rho,
+                        void *stream);
+
+/* Trilinear sampling at the current positions: out7 [7][np] in the order
+ * vx,vy,vz,bx,by,bz,rho (or NULL) and the containing-cell key (k*ny+j)*nx+i [np] (or NULL). */
+LP_API lp_status lp_interpolate(lp_ctx *ctx, double *out7, uint32_t *cell_key, void *stream);
+
+/* Reorder all particle arrays ascending by (cell key, id); bound arrays hold the result. */
+LP_API lp_status lp_sort(lp_ctx *ctx, void *stream);
+
+/* stage 0: k1 = v(x^n), rho_old = rho(x^n), x* = x^n + dt k1 (kept in the workspace).
+ * stage 1: x^{n+1} = x^n + dt/2 (k1 + v(x*)) with the fields set now; periodic wrap.
+ * stage 1 without a preceding stage 0 returns LP_ERR_STATE. */
+LP_API lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream);
+
+/* Spectral update at the current positions with the current fields:
+ * coefficients, CFL substep count, n_sub donor-cell upwind substeps of Eq. 6 per particle.
+ * Consumes rho_old of the last lp_push(stage 0); LP_ERR_STATE if there was none. */
+LP_API lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream);
+
+/* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
+ * spectral update (order of Table 1, without the fluid stages). */
+LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);
+
+/* The same step on HOST buffers (pinned or pageable): copies x,y,z,id,chi to the bound device
+ * arrays, runs lp_step, copies them back and synchronises the stream. */
+LP_API lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *hz,
+                       uint64_t *hid, double *hchi, void *stream);
+
+/* Aggregate diagnostics; synchronises `stream`. */
+LP_API lp_status lp_get_diag(lp_ctx *ctx, lp_diag *out /*host*/, void *stream);
+
+/* Number of kernel launches the library has enqueued so far on this context. */
+LP_API lp_status lp_launch_count(const lp_ctx *ctx, int64_t *out /*host*/);
+
+/* Optional device timing of the spectral-update kernel (the dominant kernel): after
+ * lp_timing_enable(ctx, n) the next n spectral launches are bracketed by CUDA events on the stream
+ * they are launched on; lp_timing_read waits for them, returns the summed kernel time in ms and the
+ * number of launches recorded, and re-arms the records.  n = 0 disables. */
+LP_API lp_status lp_timing_enable(lp_ctx *ctx, int max_records);
+LP_API lp_status lp_timing_read(lp_ctx *ctx, double *spectral_ms_sum /*host*/, int32_t *n_records /*host*/);
+
+/* Copy the library's bin table to host arrays: edges [nbins+1], widths [nbins] (either may be NULL). */
+LP_API lp_status lp_get_bins(const lp_ctx *ctx, double *edges /*host*/, double *widths /*host*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LP_H */

@@ -1,0 +1,203 @@
+"""ctypes binding of include/lp.h -- same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of liblp_b200.so; this module never computes.
+It fails loudly (ImportError / LPError) when the library cannot be built or loaded: there is
+no CPU fallback.  PyTorch appears only in `LP`, the convenience holder that keeps the device
+tensors alive and hands their data_ptr() and the current stream to the C ABI.
+"""
+import ctypes as C
+import os
+
+from . import build as _build
+
+LP_OK, LP_ERR_INVALID_ARG, LP_ERR_STATE, LP_ERR_CUDA, LP_ERR_UNSUPPORTED, LP_ERR_WORKSPACE = 0, -1, -2, -3, -4, -5
+_STATUS_NAMES = {0: "LP_OK", -1: "LP_ERR_INVALID_ARG", -2: "LP_ERR_STATE", -3: "LP_ERR_CUDA",
+                 -4: "LP_ERR_UNSUPPORTED", -5: "LP_ERR_WORKSPACE"}
+
+EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp_bind_workspace",
+           "lp_bind_particles", "lp_bind_diag", "lp_set_fields", "lp_interpolate", "lp_sort", "lp_push",
+           "lp_spectral_update", "lp_step", "lp_step_host", "lp_get_diag", "lp_launch_count", "lp_get_bins",
+           "lp_timing_enable", "lp_timing_read")
+
+
+class LPError(RuntimeError):
+    def __init__(self, status, detail=""):
+        self.status = status
+        super().__init__("%s (%d)%s" % (_STATUS_NAMES.get(status, "?"), status, (": " + detail) if detail else ""))
+
+
+class lp_config(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32),
+                ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("xlo", C.c_double * 3), ("xhi", C.c_double * 3), ("periodic", C.c_int32 * 3),
+                ("np", C.c_int64), ("nbins", C.c_int32),
+                ("e_min", C.c_double), ("e_max", C.c_double),
+                ("kappa", C.c_double), ("u_rad", C.c_double), ("cfl_e", C.c_double),
+                ("max_substeps", C.c_int32), ("sort_every", C.c_int32), ("device", C.c_int32)]
+
+
+class lp_diag(C.Structure):
+    _fields_ = [("np", C.c_int64), ("sum_substeps", C.c_int64), ("max_substeps", C.c_int32),
+                ("n_capped", C.c_int64), ("n_outside", C.c_int64), ("number", C.c_double),
+                ("lost", C.c_double), ("steps", C.c_int64), ("sorts", C.c_int64)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def library_path():
+    return _build.LIB
+
+
+def load():
+    """Build (if stale) and load liblp_b200.so; raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    lib = C.CDLL(path)
+    vp, dp = C.c_void_p, C.c_void_p
+    lib.lp_create.argtypes = [C.POINTER(lp_config), C.POINTER(vp)]
+    lib.lp_destroy.argtypes = [vp]
+    lib.lp_last_error.argtypes = [vp]
+    lib.lp_last_error.restype = C.c_char_p
+    lib.lp_workspace_bytes.argtypes = [C.POINTER(lp_config), C.POINTER(C.c_size_t)]
+    lib.lp_bind_workspace.argtypes = [vp, dp, C.c_size_t]
+    lib.lp_bind_particles.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.lp_bind_diag.argtypes = [vp, dp, dp]
+    lib.lp_set_fields.argtypes = [vp] + [dp] * 7 + [vp]
+    lib.lp_interpolate.argtypes = [vp, dp, dp, vp]
+    lib.lp_sort.argtypes = [vp, vp]
+    lib.lp_push.argtypes = [vp, C.c_double, C.c_int, vp]
+    lib.lp_spectral_update.argtypes = [vp, C.c_double, vp]
+    lib.lp_step.argtypes = [vp, C.c_double, vp]
+    lib.lp_step_host.argtypes = [vp, C.c_double, dp, dp, dp, dp, dp, vp]
+    lib.lp_get_diag.argtypes = [vp, C.POINTER(lp_diag), vp]
+    lib.lp_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    lib.lp_get_bins.argtypes = [vp, dp, dp]
+    lib.lp_timing_enable.argtypes = [vp, C.c_int]
+    lib.lp_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
+    for name in EXPORTS:
+        if name != "lp_last_error":
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _check(ctx, st):
+    if st != LP_OK:
+        detail = load().lp_last_error(ctx).decode() if ctx else ""
+        raise LPError(st, detail)
+
+
+def make_config(nx, ny, nz, xlo, xhi, periodic, np, nbins, e_min, e_max, kappa=1.0, u_rad=0.0,
+                cfl_e=0.5, max_substeps=4096, sort_every=0, device=0):
+    c = lp_config()
+    c.struct_size = C.sizeof(lp_config)
+    c.nx, c.ny, c.nz = int(nx), int(ny), int(nz)
+    for d in range(3):
+        c.xlo[d] = float(xlo[d]); c.xhi[d] = float(xhi[d]); c.periodic[d] = int(periodic[d])
+    c.np, c.nbins = int(np), int(nbins)
+    c.e_min, c.e_max = float(e_min), float(e_max)
+    c.kappa, c.u_rad, c.cfl_e = float(kappa), float(u_rad), float(cfl_e)
+    c.max_substeps, c.sort_every, c.device = int(max_substeps), int(sort_every), int(device)
+    return c
+
+
+# ---- the C ABI, one Python function per entry point (pointers are ints / None) -------------
+
+def lp_create(cfg):
+    out = C.c_void_p()
+    st = load().lp_create(C.byref(cfg), C.byref(out))
+    if st != LP_OK:
+        detail = load().lp_last_error(out).decode() if out else ""
+        if out:
+            load().lp_destroy(out)
+        raise LPError(st, detail)
+    return out
+
+
+def lp_destroy(ctx):
+    _check(None, load().lp_destroy(ctx))
+
+
+def lp_last_error(ctx):
+    return load().lp_last_error(ctx).decode()
+
+
+def lp_workspace_bytes(cfg):
+    out = C.c_size_t()
+    _check(None, load().lp_workspace_bytes(C.byref(cfg), C.byref(out)))
+    return out.value
+
+
+def lp_bind_workspace(ctx, ptr, nbytes):
+    _check(ctx, load().lp_bind_workspace(ctx, ptr, nbytes))
+
+
+def lp_bind_particles(ctx, x, y, z, pid, chi):
+    _check(ctx, load().lp_bind_particles(ctx, x, y, z, pid, chi))
+
+
+def lp_bind_diag(ctx, nsub, lost):
+    _check(ctx, load().lp_bind_diag(ctx, nsub, lost))
+
+
+def lp_set_fields(ctx, vx, vy, vz, bx, by, bz, rho, stream=None):
+    _check(ctx, load().lp_set_fields(ctx, vx, vy, vz, bx, by, bz, rho, stream))
+
+
+def lp_interpolate(ctx, out7, cell_key, stream=None):
+    _check(ctx, load().lp_interpolate(ctx, out7, cell_key, stream))
+
+
+def lp_sort(ctx, stream=None):
+    _check(ctx, load().lp_sort(ctx, stream))
+
+
+def lp_push(ctx, dt, stage, stream=None):
+    _check(ctx, load().lp_push(ctx, float(dt), int(stage), stream))
+
+
+def lp_spectral_update(ctx, dt, stream=None):
+    _check(ctx, load().lp_spectral_update(ctx, float(dt), stream))
+
+
+def lp_step(ctx, dt, stream=None):
+    _check(ctx, load().lp_step(ctx, float(dt), stream))
+
+
+def lp_step_host(ctx, dt, hx, hy, hz, hid, hchi, stream=None):
+    _check(ctx, load().lp_step_host(ctx, float(dt), hx, hy, hz, hid, hchi, stream))
+
+
+def lp_get_diag(ctx, stream=None):
+    d = lp_diag()
+    _check(ctx, load().lp_get_diag(ctx, C.byref(d), stream))
+    return d.as_dict()
+
+
+def lp_launch_count(ctx):
+    out = C.c_int64()
+    _check(ctx, load().lp_launch_count(ctx, C.byref(out)))
+    return out.value
+
+
+def lp_timing_enable(ctx, max_records):
+    _check(ctx, load().lp_timing_enable(ctx, int(max_records)))
+
+
+def lp_timing_read(ctx):
+    ms = C.c_double(); n = C.c_int32()
+    _check(ctx, load().lp_timing_read(ctx, C.byref(ms), C.byref(n)))
+    return ms.value, n.value
+
+
+def lp_get_bins(ctx, nbins):
+    import numpy as np
+    E = np.empty(nbins + 1); dE = np.empty(nbins)
+    _check(ctx, load().lp_get_bins(ctx, E.ctypes.data, dE.ctypes.data))
+    return E, dE

@@ -1,0 +1,529 @@
+// lp_api.cu -- the C ABI of include/lp.h: context, validation, workspace layout, launch order.
+// Host code only; every step of the path runs in the kernels of lp_particles.cu, lp_spectral.cu
+// and lp_sort.cu.  No CPU fallback exists.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "lp_internal.h"
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+    size_t recA, recB, k1, xs, rho_old, nsub, lost, status, key, idx_a, idx_b, hist, alt_id, chi_alt,
+        partial, diag, maxid, total;
+    size_t hist_elems;
+};
+
+Layout make_layout(const lp_config &c)
+{
+    Layout L{};
+    const size_t ncell = (size_t)c.nx * c.ny * c.nz;
+    const size_t np = (size_t)c.np;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    L.recA = take(ncell * 32);
+    L.recB = take(ncell * 32);
+    L.k1 = take(np * 24);
+    L.xs = take(np * 24);
+    L.rho_old = take(np * 8);
+    L.nsub = take(np * 4);
+    L.lost = take(np * 8);
+    L.status = take(np * 4);
+    L.key = take(np * 4);
+    L.idx_a = take(np * 4);
+    L.idx_b = take(np * 4);
+    L.hist_elems = lp_sort_hist_elems(c.np);
+    L.hist = take(L.hist_elems * 4);
+    L.alt_id = take(np * 8);
+    L.chi_alt = take(np * (size_t)c.nbins * 8);
+    L.partial = take(2 * 296 * 8);
+    L.diag = take(sizeof(LpDiagDev));
+    L.maxid = take(8);
+    L.total = off;
+    return L;
+}
+
+bool nbins_ok(int nb) { return nb == 16 || nb == 32 || nb == 64 || nb == 128 || nb == 256 || nb == 512; }
+
+int bit_length(unsigned long long v) { int b = 0; while (v) { ++b; v >>= 1; } return b; }
+
+}  // namespace
+
+struct lp_ctx {
+    lp_config cfg;
+    LpGeom geom;
+    Layout lay;
+    std::string err;
+    int sm_count = 148;
+    // bound buffers
+    unsigned char *ws = nullptr;
+    double *x = nullptr, *y = nullptr, *z = nullptr, *chi = nullptr;
+    uint64_t *id = nullptr;
+    int32_t *nsub_user = nullptr;
+    double *lost_user = nullptr;
+    // owned small tables
+    double *tab = nullptr;                 // E[nb+1] | dE[nb] | rdE[nb]
+    std::vector<double> h_edges, h_widths;
+    // state
+    bool have_fields = false, stage0_done = false, spectra_done = false;
+    int id_bits = 0, key_bits = 0;
+    long long launches = 0, steps = 0, sorts = 0;
+    // optional timing of the spectral kernel (lp_timing_enable): event pairs, resolved on read
+    std::vector<cudaEvent_t> ev;
+    size_t ev_used = 0;
+    bool timing = false;
+
+    template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
+    LpCells cells() const { return LpCells{ at<const double4>(lay.recA), at<const double4>(lay.recB) }; }
+};
+
+namespace {
+
+lp_status fail(lp_ctx *c, lp_status st, const std::string &msg)
+{
+    if (c) c->err = msg;
+    return st;
+}
+
+lp_status cuda_fail(lp_ctx *c, const char *what, cudaError_t e)
+{
+    return fail(c, LP_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define LP_CUDA(c, call)                                           \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail((c), #call, e_);   \
+    } while (0)
+
+lp_status count(lp_ctx *c, int n, const char *what)
+{
+    if (n < 0) {
+        cudaError_t e = cudaGetLastError();
+        return cuda_fail(c, what, e);
+    }
+    c->launches += n;
+    return LP_OK;
+}
+
+lp_status validate(const lp_config *cfg, std::string &why)
+{
+    if (!cfg) { why = "cfg is NULL"; return LP_ERR_INVALID_ARG; }
+    if (cfg->struct_size != sizeof(lp_config)) { why = "cfg->struct_size != sizeof(lp_config)"; return LP_ERR_INVALID_ARG; }
+    if (cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1) { why = "grid size must be >= 1"; return LP_ERR_INVALID_ARG; }
+    if ((long long)cfg->nx * cfg->ny * cfg->nz > (1ll << 31)) { why = "more than 2^31 cells"; return LP_ERR_UNSUPPORTED; }
+    for (int d = 0; d < 3; ++d)
+        if (!(cfg->xhi[d] > cfg->xlo[d])) { why = "xhi must exceed xlo"; return LP_ERR_INVALID_ARG; }
+    if (cfg->np < 0 || cfg->np > 0xffffffffll) { why = "np out of range [0, 2^32)"; return LP_ERR_INVALID_ARG; }
+    if (!nbins_ok(cfg->nbins)) { why = "nbins must be one of 16,32,64,128,256,512"; return LP_ERR_UNSUPPORTED; }
+    if (!(cfg->e_min > 0.0) || !(cfg->e_max > cfg->e_min)) { why = "need 0 < e_min < e_max"; return LP_ERR_INVALID_ARG; }
+    if (!(cfg->cfl_e > 0.0) || cfg->cfl_e > 1.0) { why = "need 0 < cfl_e <= 1"; return LP_ERR_INVALID_ARG; }
+    if (cfg->max_substeps < 1) { why = "max_substeps must be >= 1"; return LP_ERR_INVALID_ARG; }
+    if (cfg->sort_every < 0) { why = "sort_every must be >= 0"; return LP_ERR_INVALID_ARG; }
+    if (!(cfg->kappa >= 0.0) || !(cfg->u_rad >= 0.0)) { why = "kappa and u_rad must be >= 0"; return LP_ERR_INVALID_ARG; }
+    return LP_OK;
+}
+
+lp_status need_ready(lp_ctx *c, bool fields)
+{
+    if (!c) return LP_ERR_INVALID_ARG;
+    if (!c->ws) return fail(c, LP_ERR_STATE, "no workspace bound (lp_bind_workspace)");
+    if (c->cfg.np > 0 && !c->x) return fail(c, LP_ERR_STATE, "no particles bound (lp_bind_particles)");
+    if (fields && !c->have_fields) return fail(c, LP_ERR_STATE, "fields not set (lp_set_fields)");
+    return LP_OK;
+}
+
+LpPushArgs push_args(lp_ctx *c, double dt)
+{
+    LpPushArgs a;
+    a.g = c->geom;
+    a.cells = c->cells();
+    a.x = c->x; a.y = c->y; a.z = c->z;
+    a.k1 = c->at<double>(c->lay.k1);
+    a.xs = c->at<double>(c->lay.xs);
+    a.rho_old = c->at<double>(c->lay.rho_old);
+    a.status = c->at<int32_t>(c->lay.status);
+    a.np = c->cfg.np;
+    a.dt = dt;
+    return a;
+}
+
+lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, cudaStream_t s)
+{
+    LpSpectralArgs a;
+    a.g = c->geom;
+    a.cells = c->cells();
+    a.x = c->x; a.y = c->y; a.z = c->z;
+    a.rho_old = c->at<double>(c->lay.rho_old);
+    a.chi_in = chi_in;
+    a.chi_out = c->chi;
+    a.tab = c->tab;
+    a.nsub_ws = c->at<int32_t>(c->lay.nsub);
+    a.nsub_user = c->nsub_user;
+    a.lost_ws = c->at<double>(c->lay.lost);
+    a.lost_user = c->lost_user;
+    a.np = c->cfg.np;
+    a.dt = dt;
+    a.kappa = c->cfg.kappa;
+    a.u_rad = c->cfg.u_rad;
+    a.cfl_e = c->cfg.cfl_e;
+    a.max_substeps = c->cfg.max_substeps;
+    const bool rec = c->timing && c->ev_used + 2 <= c->ev.size();
+    if (rec) LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used], s));
+    lp_status st = count(c, lp_launch_spectral(a, c->cfg.nbins, c->lost_user != nullptr, c->sm_count, s),
+                         "lp_spectral_kernel launch");
+    if (rec) {
+        LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], s));
+        c->ev_used += 2;
+    }
+    if (st == LP_OK) { c->spectra_done = true; c->stage0_done = false; }
+    return st;
+}
+
+// sort: permutation, then x,y,z,id through scratch and back; chi rows into chi_alt.
+// copy_chi_back = false leaves the permuted rows in chi_alt for the caller to consume.
+lp_status do_sort(lp_ctx *c, bool copy_chi_back, cudaStream_t s)
+{
+    const long long np = c->cfg.np;
+    if (np == 0) return LP_OK;
+    LpSortBufs b;
+    b.key = c->at<uint32_t>(c->lay.key);
+    b.idx_a = c->at<uint32_t>(c->lay.idx_a);
+    b.idx_b = c->at<uint32_t>(c->lay.idx_b);
+    b.hist = c->at<uint32_t>(c->lay.hist);
+    b.hist_elems = c->lay.hist_elems;
+    uint32_t *perm = nullptr;
+    lp_status st = count(c, lp_launch_sort_perm(c->geom, c->x, c->y, c->z, c->id, np, c->id_bits, c->key_bits, b, &perm, s),
+                         "sort kernels launch");
+    if (st != LP_OK) return st;
+    double *sx = c->at<double>(c->lay.xs);
+    uint64_t *sid = c->at<uint64_t>(c->lay.alt_id);
+    double *chi_alt = c->at<double>(c->lay.chi_alt);
+    double *pos[3] = { c->x, c->y, c->z };
+    for (int d = 0; d < 3; ++d)
+        if ((st = count(c, lp_launch_permute_f64(perm, pos[d], sx + (size_t)d * np, np, s), "permute launch")) != LP_OK) return st;
+    if ((st = count(c, lp_launch_permute_u64(perm, c->id, sid, np, s), "permute launch")) != LP_OK) return st;
+    if ((st = count(c, lp_launch_permute_rows(perm, c->chi, chi_alt, np, c->cfg.nbins, s), "permute launch")) != LP_OK) return st;
+    for (int d = 0; d < 3; ++d)
+        LP_CUDA(c, cudaMemcpyAsync(pos[d], sx + (size_t)d * np, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
+    LP_CUDA(c, cudaMemcpyAsync(c->id, sid, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
+    if (copy_chi_back)
+        LP_CUDA(c, cudaMemcpyAsync(c->chi, chi_alt, (size_t)np * c->cfg.nbins * 8, cudaMemcpyDeviceToDevice, s));
+    c->stage0_done = false;      // k1 / x* / rho_old refer to the old order
+    c->spectra_done = false;     // so do the per-particle n_sub / lost of the last update
+    ++c->sorts;
+    return LP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+lp_status lp_create(const lp_config *cfg, lp_ctx **out)
+{
+    if (!out) return LP_ERR_INVALID_ARG;
+    *out = nullptr;
+    std::string why;
+    lp_status st = validate(cfg, why);
+    if (st != LP_OK) return st;
+    lp_ctx *c = new (std::nothrow) lp_ctx();
+    if (!c) return LP_ERR_INVALID_ARG;
+    c->cfg = *cfg;
+    c->lay = make_layout(*cfg);
+    LpGeom &g = c->geom;
+    g.nx = cfg->nx; g.ny = cfg->ny; g.nz = cfg->nz;
+    const int n[3] = { cfg->nx, cfg->ny, cfg->nz };
+    for (int d = 0; d < 3; ++d) {
+        g.per[d] = cfg->periodic[d] ? 1 : 0;
+        g.xlo[d] = cfg->xlo[d];
+        g.xhi[d] = cfg->xhi[d];
+        g.len[d] = cfg->xhi[d] - cfg->xlo[d];
+        g.inv_dx[d] = (double)n[d] / (cfg->xhi[d] - cfg->xlo[d]);
+    }
+    c->key_bits = bit_length((unsigned long long)cfg->nx * cfg->ny * cfg->nz - 1ull);
+    // bin table: N_b + 1 log-spaced edges on [e_min, e_max]
+    const int nb = cfg->nbins;
+    std::vector<double> tab((size_t)3 * nb + 1);
+    for (int k = 0; k <= nb; ++k) tab[k] = cfg->e_min * std::pow(cfg->e_max / cfg->e_min, (double)k / (double)nb);
+    for (int i = 0; i < nb; ++i) {
+        tab[nb + 1 + i] = tab[i + 1] - tab[i];
+        tab[2 * nb + 1 + i] = 1.0 / tab[nb + 1 + i];
+    }
+    c->h_edges.assign(tab.begin(), tab.begin() + nb + 1);
+    c->h_widths.assign(tab.begin() + nb + 1, tab.begin() + 2 * nb + 1);
+    *out = c;
+    LP_CUDA(c, cudaSetDevice(cfg->device));
+    int sm = 0;
+    LP_CUDA(c, cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, cfg->device));
+    c->sm_count = sm > 0 ? sm : 148;
+    LP_CUDA(c, cudaMalloc(&c->tab, tab.size() * sizeof(double)));
+    LP_CUDA(c, cudaMemcpy(c->tab, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice));
+    return LP_OK;
+}
+
+lp_status lp_destroy(lp_ctx *ctx)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (ctx->tab) cudaFree(ctx->tab);
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    delete ctx;
+    return LP_OK;
+}
+
+const char *lp_last_error(const lp_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+lp_status lp_workspace_bytes(const lp_config *cfg, size_t *out_bytes)
+{
+    if (!out_bytes) return LP_ERR_INVALID_ARG;
+    std::string why;
+    lp_status st = validate(cfg, why);
+    if (st != LP_OK) return st;
+    *out_bytes = make_layout(*cfg).total;
+    return LP_OK;
+}
+
+lp_status lp_bind_workspace(lp_ctx *ctx, void *workspace, size_t bytes)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (!workspace) return fail(ctx, LP_ERR_WORKSPACE, "workspace is NULL");
+    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return fail(ctx, LP_ERR_WORKSPACE, "workspace not 256-byte aligned");
+    if (bytes < ctx->lay.total) return fail(ctx, LP_ERR_WORKSPACE, "workspace smaller than lp_workspace_bytes");
+    ctx->ws = static_cast<unsigned char *>(workspace);
+    ctx->have_fields = false;
+    ctx->stage0_done = false;
+    ctx->spectra_done = false;
+    return LP_OK;
+}
+
+lp_status lp_bind_particles(lp_ctx *ctx, double *x, double *y, double *z, uint64_t *id, double *chi)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (!ctx->ws) return fail(ctx, LP_ERR_STATE, "bind the workspace first");
+    if (ctx->cfg.np > 0 && (!x || !y || !z || !id || !chi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL particle array");
+    if (reinterpret_cast<uintptr_t>(chi) % 16) return fail(ctx, LP_ERR_INVALID_ARG, "chi not 16-byte aligned");
+    ctx->x = x; ctx->y = y; ctx->z = z; ctx->id = id; ctx->chi = chi;
+    ctx->stage0_done = false;
+    ctx->spectra_done = false;
+    ctx->id_bits = 0;
+    if (ctx->cfg.np > 0) {      // number of radix passes over the ids: bit length of the largest id
+        LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+        unsigned long long *d = ctx->at<unsigned long long>(ctx->lay.maxid), h = 0;
+        LP_CUDA(ctx, cudaMemset(d, 0, 8));
+        lp_status st = count(ctx, lp_launch_max_u64(id, ctx->cfg.np, d, 0), "lp_max_u64_kernel launch");
+        if (st != LP_OK) return st;
+        LP_CUDA(ctx, cudaMemcpy(&h, d, 8, cudaMemcpyDeviceToHost));
+        ctx->id_bits = bit_length(h);
+    }
+    return LP_OK;
+}
+
+lp_status lp_bind_diag(lp_ctx *ctx, int32_t *nsub, double *lost)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    ctx->nsub_user = nsub;
+    ctx->lost_user = lost;
+    return LP_OK;
+}
+
+lp_status lp_set_fields(lp_ctx *ctx, const double *vx, const double *vy, const double *vz, const double *bx,
+                        const double *by, const double *bz, const double *rho, void *stream)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (!ctx->ws) return fail(ctx, LP_ERR_STATE, "no workspace bound (lp_bind_workspace)");
+    if (!vx || !vy || !vz || !bx || !by || !bz || !rho) return fail(ctx, LP_ERR_INVALID_ARG, "NULL field array");
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const double *f[7] = { vx, vy, vz, bx, by, bz, rho };
+    const long long ncell = (long long)ctx->cfg.nx * ctx->cfg.ny * ctx->cfg.nz;
+    lp_status st = count(ctx, lp_launch_repack(f, ctx->at<double4>(ctx->lay.recA), ctx->at<double4>(ctx->lay.recB), ncell,
+                                               static_cast<cudaStream_t>(stream)), "lp_repack_kernel launch");
+    if (st == LP_OK) ctx->have_fields = true;
+    return st;
+}
+
+lp_status lp_interpolate(lp_ctx *ctx, double *out7, uint32_t *cell_key, void *stream)
+{
+    lp_status st = need_ready(ctx, out7 != nullptr);
+    if (st != LP_OK) return st;
+    if (!out7 && !cell_key) return LP_OK;
+    if (ctx->cfg.np == 0) return LP_OK;
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    return count(ctx, lp_launch_interpolate(ctx->geom, ctx->cells(), ctx->x, ctx->y, ctx->z, ctx->cfg.np, out7, cell_key,
+                                            static_cast<cudaStream_t>(stream)), "lp_interpolate_kernel launch");
+}
+
+lp_status lp_sort(lp_ctx *ctx, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    return do_sort(ctx, true, static_cast<cudaStream_t>(stream));
+}
+
+lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream)
+{
+    lp_status st = need_ready(ctx, true);
+    if (st != LP_OK) return st;
+    if (stage != 0 && stage != 1) return fail(ctx, LP_ERR_INVALID_ARG, "stage must be 0 or 1");
+    if (stage == 1 && !ctx->stage0_done) return fail(ctx, LP_ERR_STATE, "lp_push stage 1 without stage 0");
+    if (ctx->cfg.np == 0) { ctx->stage0_done = true; return LP_OK; }
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    LpPushArgs a = push_args(ctx, dt);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (stage == 0) {
+        st = count(ctx, lp_launch_push0(a, s), "lp_push0_kernel launch");
+        if (st == LP_OK) ctx->stage0_done = true;
+        return st;
+    }
+    return count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch");
+}
+
+lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
+{
+    lp_status st = need_ready(ctx, true);
+    if (st != LP_OK) return st;
+    if (!ctx->stage0_done) return fail(ctx, LP_ERR_STATE, "lp_spectral_update needs rho_old of lp_push stage 0");
+    if (ctx->cfg.np == 0) return LP_OK;
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    return do_spectral(ctx, dt, ctx->chi, static_cast<cudaStream_t>(stream));
+}
+
+lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
+{
+    lp_status st = need_ready(ctx, true);
+    if (st != LP_OK) return st;
+    ++ctx->steps;
+    if (ctx->cfg.np == 0) return LP_OK;
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const double *chi_in = ctx->chi;
+    const bool sort_now = ctx->cfg.sort_every > 0 && (ctx->steps - 1) % ctx->cfg.sort_every == 0;
+    if (sort_now) {
+        // the permuted rows stay in the workspace; the spectral kernel reads them from there
+        // and writes the bound chi, which saves one copy of the whole spectrum array.
+        if ((st = do_sort(ctx, false, s)) != LP_OK) return st;
+        chi_in = ctx->at<double>(ctx->lay.chi_alt);
+    }
+    LpPushArgs a = push_args(ctx, dt);
+    if ((st = count(ctx, lp_launch_push0(a, s), "lp_push0_kernel launch")) != LP_OK) return st;
+    ctx->stage0_done = true;
+    if ((st = count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch")) != LP_OK) return st;
+    return do_spectral(ctx, dt, chi_in, s);
+}
+
+lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *hz, uint64_t *hid, double *hchi,
+                       void *stream)
+{
+    lp_status st = need_ready(ctx, true);
+    if (st != LP_OK) return st;
+    if (ctx->cfg.np > 0 && (!hx || !hy || !hz || !hid || !hchi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL host array");
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t np = (size_t)ctx->cfg.np, nb = (size_t)ctx->cfg.nbins;
+    if (np) {
+        LP_CUDA(ctx, cudaMemcpyAsync(ctx->x, hx, np * 8, cudaMemcpyHostToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(ctx->y, hy, np * 8, cudaMemcpyHostToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(ctx->z, hz, np * 8, cudaMemcpyHostToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(ctx->id, hid, np * 8, cudaMemcpyHostToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(ctx->chi, hchi, np * nb * 8, cudaMemcpyHostToDevice, s));
+    }
+    if ((st = lp_step(ctx, dt, stream)) != LP_OK) return st;
+    if (np) {
+        LP_CUDA(ctx, cudaMemcpyAsync(hx, ctx->x, np * 8, cudaMemcpyDeviceToHost, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(hy, ctx->y, np * 8, cudaMemcpyDeviceToHost, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(hz, ctx->z, np * 8, cudaMemcpyDeviceToHost, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(hid, ctx->id, np * 8, cudaMemcpyDeviceToHost, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(hchi, ctx->chi, np * nb * 8, cudaMemcpyDeviceToHost, s));
+    }
+    LP_CUDA(ctx, cudaStreamSynchronize(s));
+    return LP_OK;
+}
+
+lp_status lp_get_diag(lp_ctx *ctx, lp_diag *out, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    if (!out) return fail(ctx, LP_ERR_INVALID_ARG, "out is NULL");
+    std::memset(out, 0, sizeof *out);
+    out->np = ctx->cfg.np;
+    out->steps = ctx->steps;
+    out->sorts = ctx->sorts;
+    if (ctx->cfg.np == 0) return LP_OK;
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    LpDiagDev *d = ctx->at<LpDiagDev>(ctx->lay.diag), h;
+    LP_CUDA(ctx, cudaMemsetAsync(d, 0, sizeof(LpDiagDev), s));
+    const bool have = ctx->spectra_done;
+    // before the first spectral update n_sub / lost / status hold no data: reduce chi only
+    if (!have) LP_CUDA(ctx, cudaMemsetAsync(ctx->at<int32_t>(ctx->lay.nsub), 0, (size_t)ctx->cfg.np * 4, s));
+    st = count(ctx, lp_launch_diag(ctx->at<int32_t>(ctx->lay.nsub),
+                                   (have && ctx->lost_user) ? ctx->at<double>(ctx->lay.lost) : nullptr,
+                                   have ? ctx->at<int32_t>(ctx->lay.status) : nullptr, ctx->chi, ctx->tab,
+                                   ctx->cfg.nbins, ctx->cfg.np, ctx->at<double>(ctx->lay.partial), d, s),
+               "lp_diag_kernel launch");
+    if (st != LP_OK) return st;
+    LP_CUDA(ctx, cudaMemcpyAsync(&h, d, sizeof h, cudaMemcpyDeviceToHost, s));
+    LP_CUDA(ctx, cudaStreamSynchronize(s));
+    out->sum_substeps = h.sum_substeps;
+    out->max_substeps = h.max_substeps;
+    out->n_capped = h.n_capped;
+    out->n_outside = h.n_outside;
+    out->number = h.number;
+    out->lost = h.lost;
+    return LP_OK;
+}
+
+lp_status lp_launch_count(const lp_ctx *ctx, int64_t *out)
+{
+    if (!ctx || !out) return LP_ERR_INVALID_ARG;
+    *out = ctx->launches;
+    return LP_OK;
+}
+
+lp_status lp_timing_enable(lp_ctx *ctx, int max_records)
+{
+    if (!ctx || max_records < 0) return LP_ERR_INVALID_ARG;
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    ctx->ev.clear();
+    ctx->ev_used = 0;
+    ctx->timing = max_records > 0;
+    for (int i = 0; i < 2 * max_records; ++i) {
+        cudaEvent_t e;
+        LP_CUDA(ctx, cudaEventCreate(&e));
+        ctx->ev.push_back(e);
+    }
+    return LP_OK;
+}
+
+lp_status lp_timing_read(lp_ctx *ctx, double *spectral_ms_sum, int32_t *n_records)
+{
+    if (!ctx || !spectral_ms_sum || !n_records) return LP_ERR_INVALID_ARG;
+    double sum = 0.0;
+    for (size_t i = 0; i + 1 < ctx->ev_used; i += 2) {
+        LP_CUDA(ctx, cudaEventSynchronize(ctx->ev[i + 1]));
+        float ms = 0.f;
+        LP_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev[i], ctx->ev[i + 1]));
+        sum += ms;
+    }
+    *spectral_ms_sum = sum;
+    *n_records = (int32_t)(ctx->ev_used / 2);
+    ctx->ev_used = 0;
+    return LP_OK;
+}
+
+lp_status lp_get_bins(const lp_ctx *ctx, double *edges, double *widths)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (edges) std::memcpy(edges, ctx->h_edges.data(), ctx->h_edges.size() * sizeof(double));
+    if (widths) std::memcpy(widths, ctx->h_widths.data(), ctx->h_widths.size() * sizeof(double));
+    return LP_OK;
+}
+
+}  // extern "C"

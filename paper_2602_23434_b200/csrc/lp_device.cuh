@@ -1,0 +1,127 @@
+// lp_device.cuh -- device helpers of the CUDA path: cell index, trilinear stencil, gather.
+//
+// Arithmetic contract (reading R14): everything that decides an index or a position
+// uses the explicit round-to-nearest intrinsics (__dadd_rn, __dmul_rn, ...), which nvcc never
+// contracts into an FMA, in a fixed order.  Each is one correctly rounded IEEE-754 operation, so
+// cell keys, sort order and positions are reproducible bit for bit.
+#pragma once
+#include <cuda_runtime.h>
+#include "lp_internal.h"
+
+__device__ __forceinline__ double2 ldg2(const double *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
+
+__device__ __forceinline__ int lp_wrap(int i, int n, int periodic)
+{
+    if (periodic) { int m = i % n; return m < 0 ? m + n : m; }
+    return min(max(i, 0), n - 1);
+}
+
+// containing cell of one coordinate: floor((x - lo) * inv_dx), clamped   (R15)
+__device__ __forceinline__ int lp_cell_1d(double x, double lo, double inv_dx, int n)
+{
+    double s = __dmul_rn(__dsub_rn(x, lo), inv_dx);
+    int c = (int)floor(s);
+    return min(max(c, 0), n - 1);
+}
+
+__device__ __forceinline__ uint32_t lp_cell_key(const LpGeom &g, double x, double y, double z)
+{
+    int ci = lp_cell_1d(x, g.xlo[0], g.inv_dx[0], g.nx);
+    int cj = lp_cell_1d(y, g.xlo[1], g.inv_dx[1], g.ny);
+    int ck = lp_cell_1d(z, g.xlo[2], g.inv_dx[2], g.nz);
+    return (uint32_t)((ck * g.ny + cj) * g.nx + ci);
+}
+
+// Trilinear stencil of a position: 8 cell indices and weights, corners ordered z outer, y, x inner;
+// weight = (wz*wy)*wx.  Cell-centred data: s = (x - lo)*inv_dx - 1/2, i0 = floor(s), f = s - i0.
+struct LpStencil {
+    long long c[8];
+    double w[8];
+};
+
+__device__ __forceinline__ void lp_axis(double x, double lo, double inv_dx, int n, int periodic,
+                                        int &i0, int &i1, double &w0, double &w1)
+{
+    double s = __dsub_rn(__dmul_rn(__dsub_rn(x, lo), inv_dx), 0.5);
+    double fl = floor(s);
+    double f = __dsub_rn(s, fl);
+    int b = (int)fl;
+    i0 = lp_wrap(b, n, periodic);
+    i1 = lp_wrap(b + 1, n, periodic);
+    w0 = __dsub_rn(1.0, f);
+    w1 = f;
+}
+
+__device__ __forceinline__ void lp_stencil(const LpGeom &g, double x, double y, double z, LpStencil &st)
+{
+    int ii[2], jj[2], kk[2];
+    double wx[2], wy[2], wz[2];
+    lp_axis(x, g.xlo[0], g.inv_dx[0], g.nx, g.per[0], ii[0], ii[1], wx[0], wx[1]);
+    lp_axis(y, g.xlo[1], g.inv_dx[1], g.ny, g.per[1], jj[0], jj[1], wy[0], wy[1]);
+    lp_axis(z, g.xlo[2], g.inv_dx[2], g.nz, g.per[2], kk[0], kk[1], wz[0], wz[1]);
+#pragma unroll
+    for (int cz = 0; cz < 2; ++cz)
+#pragma unroll
+        for (int cy = 0; cy < 2; ++cy)
+#pragma unroll
+            for (int cx = 0; cx < 2; ++cx) {
+                int n = (cz * 2 + cy) * 2 + cx;
+                st.w[n] = __dmul_rn(__dmul_rn(wz[cz], wy[cy]), wx[cx]);
+                st.c[n] = ((long long)kk[cz] * g.ny + jj[cy]) * g.nx + ii[cx];
+            }
+}
+
+__device__ __forceinline__ double lp_acc(double acc, double w, double q) { return __dadd_rn(acc, __dmul_rn(w, q)); }
+
+// (vx, vy, vz, rho) from record A
+__device__ __forceinline__ void lp_gather_A(const LpCells &cells, const LpStencil &st, double out[4])
+{
+    out[0] = out[1] = out[2] = out[3] = 0.0;
+#pragma unroll
+    for (int n = 0; n < 8; ++n) {
+        const double *r = reinterpret_cast<const double *>(cells.recA + st.c[n]);
+        double2 a = ldg2(r), b = ldg2(r + 2);
+        out[0] = lp_acc(out[0], st.w[n], a.x);
+        out[1] = lp_acc(out[1], st.w[n], a.y);
+        out[2] = lp_acc(out[2], st.w[n], b.x);
+        out[3] = lp_acc(out[3], st.w[n], b.y);
+    }
+}
+
+// (vx, vy, vz) only: rho is loaded (same 32-byte record) but not accumulated
+__device__ __forceinline__ void lp_gather_v(const LpCells &cells, const LpStencil &st, double out[3])
+{
+    out[0] = out[1] = out[2] = 0.0;
+#pragma unroll
+    for (int n = 0; n < 8; ++n) {
+        const double *r = reinterpret_cast<const double *>(cells.recA + st.c[n]);
+        double2 a = ldg2(r);
+        double vz = __ldg(r + 2);
+        out[0] = lp_acc(out[0], st.w[n], a.x);
+        out[1] = lp_acc(out[1], st.w[n], a.y);
+        out[2] = lp_acc(out[2], st.w[n], vz);
+    }
+}
+
+// (bx, by, bz) from record B
+__device__ __forceinline__ void lp_gather_B(const LpCells &cells, const LpStencil &st, double out[3])
+{
+    out[0] = out[1] = out[2] = 0.0;
+#pragma unroll
+    for (int n = 0; n < 8; ++n) {
+        const double *r = reinterpret_cast<const double *>(cells.recB + st.c[n]);
+        double2 a = ldg2(r);
+        double bz = __ldg(r + 2);
+        out[0] = lp_acc(out[0], st.w[n], a.x);
+        out[1] = lp_acc(out[1], st.w[n], a.y);
+        out[2] = lp_acc(out[2], st.w[n], bz);
+    }
+}
+
+// periodic wrap into [lo, hi): x -= L*floor((x - lo)/L); a result >= hi becomes lo   (R15)
+__device__ __forceinline__ double lp_wrap_pos(double x, double lo, double hi, double L)
+{
+    double t = floor(__ddiv_rn(__dsub_rn(x, lo), L));
+    x = __dsub_rn(x, __dmul_rn(L, t));
+    return x >= hi ? lo : x;
+}

@@ -1,0 +1,93 @@
+// lp_internal.h -- host-side declarations shared by the translation units of liblp_b200.so.
+// Product code (CUDA path).  Shares nothing with oracle/.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/lp.h"
+
+// Grid geometry handed to kernels by value (fits in kernel-parameter constant bank).
+struct LpGeom {
+    int nx, ny, nz;
+    int per[3];
+    double xlo[3], xhi[3];
+    double inv_dx[3];        // n / (xhi - xlo), computed on the host in fp64
+    double len[3];           // xhi - xlo
+};
+
+// Interleaved per-cell records built by lp_set_fields:
+//   recA[c] = (vx, vy, vz, rho)   32 B     recB[c] = (bx, by, bz, 0)   32 B
+struct LpCells {
+    const double4 *recA;
+    const double4 *recB;
+};
+
+struct LpSpectralArgs {
+    LpGeom g;
+    LpCells cells;
+    const double *x, *y, *z;     // positions at which the coefficients are gathered (x^{n+1})
+    const double *rho_old;       // from push stage 0
+    const double *chi_in;        // [np][nbins]  (may differ from chi_out after a re-sort)
+    double *chi_out;             // [np][nbins]
+    const double *tab;           // device bin table: E[nb+1] | dE[nb] | rdE[nb]
+    int32_t *nsub_ws;            // [np] always written (workspace)
+    int32_t *nsub_user;          // [np] or NULL
+    double *lost_ws;             // [np] always written when DIAG
+    double *lost_user;           // [np] or NULL
+    long long np;
+    double dt, kappa, u_rad, cfl_e;
+    int max_substeps;
+};
+
+struct LpPushArgs {
+    LpGeom g;
+    LpCells cells;
+    double *x, *y, *z;           // bound positions (x^n in, x^{n+1} out at stage 1)
+    double *k1;                  // [3][np]
+    double *xs;                  // [3][np]  predictor positions
+    double *rho_old;             // [np]
+    int32_t *status;             // [np]
+    long long np;
+    double dt;
+};
+
+// ---- launchers (each returns the number of kernels it enqueued, or -1 with cudaGetLastError set)
+int lp_launch_repack(const double *const f[7], double4 *recA, double4 *recB, long long ncell,
+                     cudaStream_t s);
+int lp_launch_interpolate(const LpGeom &g, const LpCells &c, const double *x, const double *y,
+                          const double *z, long long np, double *out7, uint32_t *key, cudaStream_t s);
+int lp_launch_push0(const LpPushArgs &a, cudaStream_t s);
+int lp_launch_push1(const LpPushArgs &a, cudaStream_t s);
+int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, int sm_count, cudaStream_t s);
+
+// sort: fills perm[n] = source index of the n-th particle in (key, id) order.
+struct LpSortBufs {
+    uint32_t *key;       // [np]
+    uint32_t *idx_a;     // [np]
+    uint32_t *idx_b;     // [np]
+    uint32_t *hist;      // [256 * nblocks]
+    size_t hist_elems;
+};
+size_t lp_sort_hist_elems(long long np);
+int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const double *z,
+                        const uint64_t *id, long long np, int id_bits, int key_bits,
+                        const LpSortBufs &b, uint32_t **perm_out, cudaStream_t s);
+int lp_launch_permute_f64(const uint32_t *perm, const double *src, double *dst, long long np, cudaStream_t s);
+int lp_launch_permute_u64(const uint32_t *perm, const uint64_t *src, uint64_t *dst, long long np, cudaStream_t s);
+int lp_launch_permute_rows(const uint32_t *perm, const double *src, double *dst, long long np,
+                           int nbins, cudaStream_t s);
+int lp_launch_max_u64(const uint64_t *v, long long np, unsigned long long *out, cudaStream_t s);
+
+// diagnostics reduction
+struct LpDiagDev {
+    long long sum_substeps;
+    long long n_capped;
+    long long n_outside;
+    int max_substeps;
+    int pad;
+    double number;
+    double lost;
+};
+int lp_launch_diag(const int32_t *nsub, const double *lost, const int32_t *status, const double *chi,
+                   const double *tab, int nbins, long long np, double *partial /*scratch*/,
+                   LpDiagDev *out, cudaStream_t s);

@@ -1,0 +1,127 @@
+// lp_particles.cu -- field repack, cell key + trilinear gather, two-stage push (thread per particle).
+// Steps a1, a3-a6 of DESIGN.md section 1.  sm_100a.
+#include "lp_device.cuh"
+
+namespace {
+
+constexpr int kThreads = 256;
+
+inline int blocks_for(long long n, int threads)
+{
+    long long b = (n + threads - 1) / threads;
+    return (int)(b < 1 ? 1 : b);
+}
+
+// a3: seven SoA grid arrays -> two interleaved 32-byte records per cell.
+__global__ void __launch_bounds__(kThreads)
+lp_repack_kernel(const double *__restrict__ vx, const double *__restrict__ vy, const double *__restrict__ vz,
+                 const double *__restrict__ bx, const double *__restrict__ by, const double *__restrict__ bz,
+                 const double *__restrict__ rho, double4 *__restrict__ recA, double4 *__restrict__ recB,
+                 long long ncell)
+{
+    long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    double2 *a = reinterpret_cast<double2 *>(recA + c);
+    double2 *b = reinterpret_cast<double2 *>(recB + c);
+    a[0] = make_double2(vx[c], vy[c]);
+    a[1] = make_double2(vz[c], rho[c]);
+    b[0] = make_double2(bx[c], by[c]);
+    b[1] = make_double2(bz[c], 0.0);
+}
+
+// a1 + a4: key and/or the seven sampled fields at the current positions.
+__global__ void __launch_bounds__(kThreads)
+lp_interpolate_kernel(LpGeom g, LpCells cells, const double *__restrict__ x, const double *__restrict__ y,
+                      const double *__restrict__ z, long long np, double *__restrict__ out7,
+                      uint32_t *__restrict__ key)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    double px = x[p], py = y[p], pz = z[p];
+    if (key) key[p] = lp_cell_key(g, px, py, pz);
+    if (out7) {
+        LpStencil st;
+        lp_stencil(g, px, py, pz, st);
+        double a[4], b[3];
+        lp_gather_A(cells, st, a);
+        lp_gather_B(cells, st, b);
+        out7[p] = a[0];
+        out7[np + p] = a[1];
+        out7[2 * np + p] = a[2];
+        out7[3 * np + p] = b[0];
+        out7[4 * np + p] = b[1];
+        out7[5 * np + p] = b[2];
+        out7[6 * np + p] = a[3];
+    }
+}
+
+// a5: k1 = v(x^n), rho_old = rho(x^n), x* = x^n + dt*k1
+__global__ void __launch_bounds__(kThreads) lp_push0_kernel(LpPushArgs A)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= A.np) return;
+    double px = A.x[p], py = A.y[p], pz = A.z[p];
+    LpStencil st;
+    lp_stencil(A.g, px, py, pz, st);
+    double q[4];
+    lp_gather_A(A.cells, st, q);
+    const long long np = A.np;
+    A.k1[p] = q[0];
+    A.k1[np + p] = q[1];
+    A.k1[2 * np + p] = q[2];
+    A.rho_old[p] = q[3];
+    A.xs[p] = __dadd_rn(px, __dmul_rn(A.dt, q[0]));
+    A.xs[np + p] = __dadd_rn(py, __dmul_rn(A.dt, q[1]));
+    A.xs[2 * np + p] = __dadd_rn(pz, __dmul_rn(A.dt, q[2]));
+}
+
+// a6: x^{n+1} = x^n + (dt/2)(k1 + v(x*)), periodic wrap / outside flag
+__global__ void __launch_bounds__(kThreads) lp_push1_kernel(LpPushArgs A)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= A.np) return;
+    const long long np = A.np;
+    LpStencil st;
+    lp_stencil(A.g, A.xs[p], A.xs[np + p], A.xs[2 * np + p], st);
+    double k2[3];
+    lp_gather_v(A.cells, st, k2);
+    const double hdt = __dmul_rn(0.5, A.dt);
+    double *pos[3] = { A.x, A.y, A.z };
+    int stt = 0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        double xn = __dadd_rn(pos[d][p], __dmul_rn(hdt, __dadd_rn(A.k1[(long long)d * np + p], k2[d])));
+        if (A.g.per[d]) xn = lp_wrap_pos(xn, A.g.xlo[d], A.g.xhi[d], A.g.len[d]);
+        else if (xn < A.g.xlo[d] || xn >= A.g.xhi[d]) stt |= (1 << d);
+        pos[d][p] = xn;
+    }
+    A.status[p] = stt;
+}
+
+}  // namespace
+
+int lp_launch_repack(const double *const f[7], double4 *recA, double4 *recB, long long ncell, cudaStream_t s)
+{
+    lp_repack_kernel<<<blocks_for(ncell, kThreads), kThreads, 0, s>>>(f[0], f[1], f[2], f[3], f[4], f[5], f[6],
+                                                                      recA, recB, ncell);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+int lp_launch_interpolate(const LpGeom &g, const LpCells &c, const double *x, const double *y, const double *z,
+                          long long np, double *out7, uint32_t *key, cudaStream_t s)
+{
+    lp_interpolate_kernel<<<blocks_for(np, kThreads), kThreads, 0, s>>>(g, c, x, y, z, np, out7, key);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+int lp_launch_push0(const LpPushArgs &a, cudaStream_t s)
+{
+    lp_push0_kernel<<<blocks_for(a.np, kThreads), kThreads, 0, s>>>(a);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+int lp_launch_push1(const LpPushArgs &a, cudaStream_t s)
+{
+    lp_push1_kernel<<<blocks_for(a.np, kThreads), kThreads, 0, s>>>(a);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}

@@ -1,0 +1,304 @@
+// lp_sort.cu -- step a2 of DESIGN.md section 1: order particles ascending by (cell key, id) and
+// apply the permutation.  A stable LSD radix sort (8-bit digits) over a u32 index array: first the
+// digits of id, then the digits of the cell key, so ties in the key keep ascending id.  Stability
+// and the unique ids make the result the one total order the oracle's comparison sort produces.
+// Also: the aggregate diagnostics reduction (a10).  sm_100a.
+#include "lp_device.cuh"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kItems = 16;                       // rounds per tile
+constexpr int kTile = kThreads * kItems;         // elements per block
+constexpr unsigned kFull = 0xffffffffu;
+
+inline int blocks_for(long long n, int per) { long long b = (n + per - 1) / per; return (int)(b < 1 ? 1 : b); }
+
+__global__ void __launch_bounds__(kThreads)
+lp_key_kernel(LpGeom g, const double *__restrict__ x, const double *__restrict__ y,
+              const double *__restrict__ z, long long np, uint32_t *__restrict__ key)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < np) key[p] = lp_cell_key(g, x[p], y[p], z[p]);
+}
+
+// digit of element e of the current sequence (idx_in == NULL means the identity sequence)
+__device__ __forceinline__ uint32_t lp_digit(const uint32_t *idx_in, const uint64_t *id, const uint32_t *key,
+                                             long long e, int use_key, int shift, uint32_t &src)
+{
+    src = idx_in ? idx_in[e] : (uint32_t)e;
+    return use_key ? ((key[src] >> shift) & 255u) : (uint32_t)((id[src] >> shift) & 255ull);
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_radix_hist_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__restrict__ id,
+                     const uint32_t *__restrict__ key, long long np, int use_key, int shift,
+                     uint32_t *__restrict__ hist, int nblocks)
+{
+    __shared__ uint32_t sh[256];
+    sh[threadIdx.x] = 0;
+    __syncthreads();
+    const long long t0 = (long long)blockIdx.x * kTile;
+    for (int r = 0; r < kItems; ++r) {
+        long long e = t0 + r * kThreads + threadIdx.x;
+        if (e < np) {
+            uint32_t src;
+            atomicAdd(&sh[lp_digit(idx_in, id, key, e, use_key, shift, src)], 1u);
+        }
+    }
+    __syncthreads();
+    hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = sh[threadIdx.x];
+}
+
+// exclusive scan of n u32 values in place, one block of 1024 threads
+__global__ void __launch_bounds__(1024) lp_scan_kernel(uint32_t *__restrict__ v, long long n)
+{
+    __shared__ uint32_t wsum[32];
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const long long per = (n + 1023) / 1024;
+    const long long b = (long long)t * per;
+    const long long e = b + per < n ? b + per : n;
+    uint32_t s = 0;
+    for (long long i = b; i < e; ++i) s += v[i];
+    uint32_t inc = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t u = __shfl_up_sync(kFull, inc, o);
+        if (lane >= o) inc += u;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = wsum[lane], winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t u = __shfl_up_sync(kFull, winc, o);
+            if (lane >= o) winc += u;
+        }
+        wsum[lane] = winc - w;
+    }
+    __syncthreads();
+    uint32_t run = wsum[warp] + inc - s;
+    for (long long i = b; i < e; ++i) { uint32_t x = v[i]; v[i] = run; run += x; }
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_radix_scatter_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__restrict__ id,
+                        const uint32_t *__restrict__ key, long long np, int use_key, int shift,
+                        const uint32_t *__restrict__ hist, int nblocks, uint32_t *__restrict__ idx_out)
+{
+    __shared__ uint32_t base[256];
+    __shared__ uint32_t wcount[kWarps][256];
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    base[t] = hist[(size_t)t * nblocks + blockIdx.x];
+    const long long t0 = (long long)blockIdx.x * kTile;
+    for (int r = 0; r < kItems; ++r) {
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) wcount[w][t] = 0;
+        __syncthreads();
+        const long long e = t0 + r * kThreads + t;
+        const bool valid = e < np;
+        uint32_t src = 0, d = 256u + lane;          // invalid lanes get distinct pseudo-digits
+        if (valid) d = lp_digit(idx_in, id, key, e, use_key, shift, src);
+        const unsigned same = __match_any_sync(kFull, d);
+        const int rank = __popc(same & ((1u << lane) - 1u));
+        if (valid && rank == 0) wcount[warp][d] = __popc(same);
+        __syncthreads();
+        {
+            uint32_t run = base[t];
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w) { uint32_t c = wcount[w][t]; wcount[w][t] = run; run += c; }
+            base[t] = run;
+        }
+        __syncthreads();
+        if (valid) idx_out[wcount[warp][d] + rank] = src;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_permute_f64_kernel(const uint32_t *__restrict__ perm, const double *__restrict__ src,
+                      double *__restrict__ dst, long long np)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < np) dst[p] = src[perm[p]];
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_permute_u64_kernel(const uint32_t *__restrict__ perm, const uint64_t *__restrict__ src,
+                      uint64_t *__restrict__ dst, long long np)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < np) dst[p] = src[perm[p]];
+}
+
+// one warp (or half warp for 16 bins) moves one row of nbins doubles with 16-byte accesses
+__global__ void __launch_bounds__(kThreads)
+lp_permute_rows_kernel(const uint32_t *__restrict__ perm, const double *__restrict__ src,
+                       double *__restrict__ dst, long long np, int nbins)
+{
+    const int lanes = nbins / 2 < 32 ? nbins / 2 : 32;      // lanes per row (16 B each per pass)
+    const int rows_per_warp = 32 / lanes;
+    const int lane = threadIdx.x & 31;
+    const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    const int sub = lane % lanes, grp = lane / lanes;
+    for (long long r0 = gw * rows_per_warp; r0 < np; r0 += nw * rows_per_warp) {
+        const long long r = r0 + grp;
+        if (r >= np) continue;
+        const double2 *s = reinterpret_cast<const double2 *>(src + (long long)perm[r] * nbins);
+        double2 *d = reinterpret_cast<double2 *>(dst + r * nbins);
+        for (int i = sub; i < nbins / 2; i += lanes) d[i] = s[i];
+    }
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_max_u64_kernel(const uint64_t *__restrict__ v, long long np, unsigned long long *out)
+{
+    unsigned long long m = 0;
+    for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += (long long)gridDim.x * blockDim.x)
+        m = v[p] > m ? v[p] : m;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long u = __shfl_xor_sync(kFull, m, o);
+        m = u > m ? u : m;
+    }
+    if ((threadIdx.x & 31) == 0) atomicMax(out, m);
+}
+
+// ---- diagnostics: integer sums by atomics (order independent), fp64 sums per block in a fixed
+// order and then over blocks in a fixed order (deterministic).
+__global__ void __launch_bounds__(kThreads)
+lp_diag_kernel(const int32_t *__restrict__ nsub, const double *__restrict__ lost,
+               const int32_t *__restrict__ status, const double *__restrict__ chi,
+               const double *__restrict__ tab, int nbins, long long np, double *__restrict__ partial,
+               LpDiagDev *out)
+{
+    __shared__ double snum[kWarps], slost[kWarps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double *dE = tab + (nbins + 1);
+    long long sum_ns = 0, capped = 0, outside = 0;
+    int max_ns = 0;
+    double lo = 0.0;
+    for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += (long long)gridDim.x * blockDim.x) {
+        int n = nsub[p];
+        if (n < 0) { ++capped; n = -n; }
+        sum_ns += n;
+        max_ns = n > max_ns ? n : max_ns;
+        if (status && status[p]) ++outside;
+        if (lost) lo += lost[p];
+    }
+    double num = 0.0;
+    const long long gw = (long long)blockIdx.x * kWarps + warp, nw = (long long)gridDim.x * kWarps;
+    for (long long r = gw; r < np; r += nw) {
+        const double *row = chi + r * nbins;
+        for (int i = lane; i < nbins; i += 32) num = fma(row[i], dE[i], num);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sum_ns += __shfl_xor_sync(kFull, sum_ns, o);
+        capped += __shfl_xor_sync(kFull, capped, o);
+        outside += __shfl_xor_sync(kFull, outside, o);
+        max_ns = max(max_ns, __shfl_xor_sync(kFull, max_ns, o));
+        lo += __shfl_xor_sync(kFull, lo, o);
+        num += __shfl_xor_sync(kFull, num, o);
+    }
+    if (lane == 0) {
+        atomicAdd((unsigned long long *)&out->sum_substeps, (unsigned long long)sum_ns);
+        atomicAdd((unsigned long long *)&out->n_capped, (unsigned long long)capped);
+        atomicAdd((unsigned long long *)&out->n_outside, (unsigned long long)outside);
+        atomicMax(&out->max_substeps, max_ns);
+        snum[warp] = num;
+        slost[warp] = lo;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int w = 0; w < kWarps; ++w) { a += snum[w]; b += slost[w]; }
+        partial[2 * blockIdx.x] = a;
+        partial[2 * blockIdx.x + 1] = b;
+    }
+}
+
+__global__ void lp_diag_final_kernel(const double *__restrict__ partial, int nblocks, LpDiagDev *out)
+{
+    double a = 0.0, b = 0.0;
+    for (int i = 0; i < nblocks; ++i) { a += partial[2 * i]; b += partial[2 * i + 1]; }
+    out->number = a;
+    out->lost = b;
+}
+
+inline bool ok() { return cudaPeekAtLastError() == cudaSuccess; }
+
+}  // namespace
+
+size_t lp_sort_hist_elems(long long np) { return (size_t)256 * (size_t)blocks_for(np, kTile); }
+
+int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const double *z, const uint64_t *id,
+                        long long np, int id_bits, int key_bits, const LpSortBufs &b, uint32_t **perm_out,
+                        cudaStream_t s)
+{
+    int launches = 0;
+    lp_key_kernel<<<blocks_for(np, kThreads), kThreads, 0, s>>>(g, x, y, z, np, b.key);
+    ++launches;
+    const int nblocks = blocks_for(np, kTile);
+    const uint32_t *in = nullptr;       // identity
+    uint32_t *bufs[2] = { b.idx_a, b.idx_b };
+    int cur = 0;
+    const int id_passes = (id_bits + 7) / 8, key_passes = (key_bits + 7) / 8;
+    const int total = id_passes + key_passes;
+    for (int pass = 0; pass < (total > 0 ? total : 1); ++pass) {
+        const int use_key = pass >= id_passes ? 1 : 0;
+        const int shift = 8 * (use_key ? pass - id_passes : pass);
+        lp_radix_hist_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, nblocks);
+        lp_scan_kernel<<<1, 1024, 0, s>>>(b.hist, (long long)256 * nblocks);
+        lp_radix_scatter_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, nblocks, bufs[cur]);
+        launches += 3;
+        in = bufs[cur];
+        cur ^= 1;
+    }
+    *perm_out = const_cast<uint32_t *>(in);
+    return ok() ? launches : -1;
+}
+
+int lp_launch_permute_f64(const uint32_t *perm, const double *src, double *dst, long long np, cudaStream_t s)
+{
+    lp_permute_f64_kernel<<<blocks_for(np, kThreads), kThreads, 0, s>>>(perm, src, dst, np);
+    return ok() ? 1 : -1;
+}
+
+int lp_launch_permute_u64(const uint32_t *perm, const uint64_t *src, uint64_t *dst, long long np, cudaStream_t s)
+{
+    lp_permute_u64_kernel<<<blocks_for(np, kThreads), kThreads, 0, s>>>(perm, src, dst, np);
+    return ok() ? 1 : -1;
+}
+
+int lp_launch_permute_rows(const uint32_t *perm, const double *src, double *dst, long long np, int nbins,
+                           cudaStream_t s)
+{
+    const int lanes = nbins / 2 < 32 ? nbins / 2 : 32;
+    const long long warps = (np + (32 / lanes) - 1) / (32 / lanes);
+    long long blocks = (warps + kWarps - 1) / kWarps;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks < 1) blocks = 1;
+    lp_permute_rows_kernel<<<(int)blocks, kThreads, 0, s>>>(perm, src, dst, np, nbins);
+    return ok() ? 1 : -1;
+}
+
+int lp_launch_max_u64(const uint64_t *v, long long np, unsigned long long *out, cudaStream_t s)
+{
+    int blocks = blocks_for(np, kThreads * 8);
+    if (blocks > 1024) blocks = 1024;
+    lp_max_u64_kernel<<<blocks, kThreads, 0, s>>>(v, np, out);
+    return ok() ? 1 : -1;
+}
+
+int lp_launch_diag(const int32_t *nsub, const double *lost, const int32_t *status, const double *chi,
+                   const double *tab, int nbins, long long np, double *partial, LpDiagDev *out, cudaStream_t s)
+{
+    const int blocks = 296;
+    lp_diag_kernel<<<blocks, kThreads, 0, s>>>(nsub, lost, status, chi, tab, nbins, np, partial, out);
+    lp_diag_final_kernel<<<1, 1, 0, s>>>(partial, blocks, out);
+    return ok() ? 2 : -1;
+}

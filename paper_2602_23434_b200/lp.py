@@ -1,0 +1,109 @@
+"""`LP`: a thin holder around one lp_ctx that owns the torch device tensors (memory and stream
+plumbing only) and forwards to the C ABI.  No arithmetic of the method lives here."""
+import torch
+
+from . import binding as B
+
+
+class LP:
+    def __init__(self, cfg, device=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2602_23434_b200 needs a CUDA device (sm_100a); there is no CPU path")
+        self.cfg = cfg
+        self.device = torch.device("cuda", cfg.device) if device is None else torch.device(device)
+        B.load()
+        self.ctx = B.lp_create(cfg)
+        nbytes = B.lp_workspace_bytes(cfg)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-self.workspace.data_ptr()) % 256
+        B.lp_bind_workspace(self.ctx, self.workspace.data_ptr() + off, nbytes)
+        self.workspace_bytes = nbytes
+        self.x = self.y = self.z = self.id = self.chi = None
+        self.nsub = self.lost = None
+        self._fields = None
+
+    def close(self):
+        if self.ctx is not None:
+            torch.cuda.synchronize(self.device)
+            B.lp_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def stream(self):
+        return torch.cuda.current_stream(self.device).cuda_stream
+
+    def _dev(self, a, dtype):
+        t = torch.as_tensor(a)
+        if dtype == torch.uint64 and t.dtype != torch.uint64:
+            t = t.to(torch.int64).view(torch.uint64) if t.dtype == torch.int64 else t
+        return t.to(device=self.device, dtype=dtype).contiguous()
+
+    def bind_particles(self, x, y, z, pid, chi):
+        import numpy as np
+        n, nb = self.cfg.np, self.cfg.nbins
+        self.x = self._dev(x, torch.float64); self.y = self._dev(y, torch.float64); self.z = self._dev(z, torch.float64)
+        pid = torch.as_tensor(np.ascontiguousarray(pid).view(np.int64)) if not torch.is_tensor(pid) else pid
+        self.id = pid.to(self.device).contiguous()
+        self.chi = self._dev(chi, torch.float64)
+        assert self.x.numel() == n and self.chi.shape == (n, nb) and self.id.numel() == n
+        B.lp_bind_particles(self.ctx, self.x.data_ptr(), self.y.data_ptr(), self.z.data_ptr(),
+                            self.id.data_ptr(), self.chi.data_ptr())
+
+    def bind_diag(self, nsub=True, lost=True):
+        n = self.cfg.np
+        self.nsub = torch.zeros(n, dtype=torch.int32, device=self.device) if nsub else None
+        self.lost = torch.zeros(n, dtype=torch.float64, device=self.device) if lost else None
+        B.lp_bind_diag(self.ctx, self.nsub.data_ptr() if nsub else None, self.lost.data_ptr() if lost else None)
+
+    def set_fields(self, fields7):
+        f = [self._dev(t, torch.float64) for t in fields7]
+        ncell = self.cfg.nx * self.cfg.ny * self.cfg.nz
+        assert len(f) == 7 and all(t.numel() == ncell for t in f)
+        B.lp_set_fields(self.ctx, *[t.data_ptr() for t in f], self.stream)
+        self._fields = f          # keep alive until the stream has consumed them
+
+    def interpolate(self, want_fields=True, want_key=True):
+        n = self.cfg.np
+        out7 = torch.empty((7, n), dtype=torch.float64, device=self.device) if want_fields else None
+        key = torch.empty(n, dtype=torch.int32, device=self.device) if want_key else None
+        B.lp_interpolate(self.ctx, out7.data_ptr() if want_fields else None,
+                         key.data_ptr() if want_key else None, self.stream)
+        return out7, key
+
+    def sort(self):
+        B.lp_sort(self.ctx, self.stream)
+
+    def push(self, dt, stage):
+        B.lp_push(self.ctx, dt, stage, self.stream)
+
+    def spectral_update(self, dt):
+        B.lp_spectral_update(self.ctx, dt, self.stream)
+
+    def step(self, dt):
+        B.lp_step(self.ctx, dt, self.stream)
+
+    def step_host(self, dt, hx, hy, hz, hid, hchi):
+        B.lp_step_host(self.ctx, dt, hx.data_ptr(), hy.data_ptr(), hz.data_ptr(), hid.data_ptr(),
+                       hchi.data_ptr(), self.stream)
+
+    def diag(self):
+        return B.lp_get_diag(self.ctx, self.stream)
+
+    def launch_count(self):
+        return B.lp_launch_count(self.ctx)
+
+    def bins(self):
+        return B.lp_get_bins(self.ctx, self.cfg.nbins)
+
+
+def config_from_workload(w, u_rad=0.0, device=0, np=None):
+    """lp_config for an lp_inputs.LPWorkload (duck-typed: only attributes are read)."""
+    return B.make_config(w.n, w.n, w.n, w.xlo, w.xhi, w.periodic, w.np if np is None else np, w.nbins,
+                         w.e_min, w.e_max, kappa=w.kappa, u_rad=u_rad, cfl_e=w.cfl_e,
+                         max_substeps=w.max_substeps, sort_every=w.sort_every, device=device)

@@ -1,0 +1,107 @@
+"""CPU-side checks of the boundary: the library builds, loads and exports every symbol that
+include/lp.h declares; argument validation that needs no GPU; binding struct layout."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import paper_2602_23434_b200 as P
+
+B = P.binding
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "lp.h")).read()
+    return sorted(set(re.findall(r"LP_API\s+[\w\s\*]+?\b(lp_\w+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = B.load()
+    names = declared_symbols()
+    assert len(names) == 19 and set(names) == set(B.EXPORTS)
+    for n in names:
+        assert getattr(lib, n) is not None
+
+
+def test_struct_sizes_match_the_header():
+    # compile a tiny C program against include/lp.h and compare sizeof with the ctypes mirrors
+    import subprocess, tempfile
+    with tempfile.TemporaryDirectory() as d:
+        c = os.path.join(d, "s.c")
+        open(c, "w").write('#include <stdio.h>\n#include "lp.h"\nint main(){printf("%zu %zu\\n",'
+                           'sizeof(lp_config),sizeof(lp_diag));return 0;}\n')
+        exe = os.path.join(d, "s")
+        subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), c, "-o", exe], check=True)
+        a, b = subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()
+    assert int(a) == C.sizeof(B.lp_config) and int(b) == C.sizeof(B.lp_diag)
+
+
+def cfg(**kw):
+    d = dict(nx=8, ny=8, nz=8, xlo=(-1,) * 3, xhi=(1,) * 3, periodic=(1, 1, 1), np=100, nbins=64,
+             e_min=1.0, e_max=1e6)
+    d.update(kw)
+    return P.make_config(**d)
+
+
+@pytest.mark.parametrize("bad,status", [
+    (dict(nbins=48), B.LP_ERR_UNSUPPORTED),
+    (dict(nbins=1024), B.LP_ERR_UNSUPPORTED),
+    (dict(nx=0), B.LP_ERR_INVALID_ARG),
+    (dict(nx=2048, ny=2048, nz=2048), B.LP_ERR_UNSUPPORTED),
+    (dict(e_min=0.0), B.LP_ERR_INVALID_ARG),
+    (dict(e_max=0.5), B.LP_ERR_INVALID_ARG),
+    (dict(cfl_e=1.5), B.LP_ERR_INVALID_ARG),
+    (dict(max_substeps=0), B.LP_ERR_INVALID_ARG),
+    (dict(np=-1), B.LP_ERR_INVALID_ARG),
+    (dict(xhi=(1, -1, 1)), B.LP_ERR_INVALID_ARG),
+])
+def test_config_validation_without_gpu(bad, status):
+    with pytest.raises(B.LPError) as e:
+        B.lp_workspace_bytes(cfg(**bad))
+    assert e.value.status == status
+
+
+def test_struct_size_is_checked():
+    c = cfg()
+    c.struct_size = 8
+    with pytest.raises(B.LPError) as e:
+        B.lp_workspace_bytes(c)
+    assert e.value.status == B.LP_ERR_INVALID_ARG
+
+
+def test_workspace_bytes_grow_with_problem():
+    a = B.lp_workspace_bytes(cfg())
+    b = B.lp_workspace_bytes(cfg(np=200))
+    c = B.lp_workspace_bytes(cfg(nx=16))
+    assert a % 256 == 0 and b > a and c > a
+    # dominated by the alternate chi rows + cell records: np*nbins*8 + 64*ncell
+    assert a >= 100 * 64 * 8 + 64 * 512
+
+
+def test_null_arguments_are_rejected_not_crashed():
+    lib = B.load()
+    assert lib.lp_create(None, None) == B.LP_ERR_INVALID_ARG
+    out = C.c_void_p()
+    assert lib.lp_create(None, C.byref(out)) == B.LP_ERR_INVALID_ARG and not out
+    assert lib.lp_destroy(None) == B.LP_ERR_INVALID_ARG
+    assert lib.lp_step(None, 0.1, None) == B.LP_ERR_INVALID_ARG
+    assert lib.lp_last_error(None) == b"null context"
+
+
+def test_product_path_has_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError):
+        P.LP(cfg())
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2602_23434_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "lp_oracle" not in src, f

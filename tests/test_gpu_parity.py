@@ -1,0 +1,253 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle on the same seeded
+inputs, element by element.  Bit-exact for keys, sort order, gathered values and positions
+(R14); relative 1e-10 for spectra; n_sub compared exactly."""
+import numpy as np
+import pytest
+import torch
+
+import lp_inputs as I
+import paper_2602_23434_b200 as P
+from oracle import lp_oracle as orc
+
+from lp_testlib import (REL_TOL, assert_chi_close, assert_nsub_equal, fields_to_numpy, oracle_params,
+                        oracle_sort_state, u_rad_of, workload1_dt)
+
+pytestmark = pytest.mark.gpu
+B = P.binding
+
+
+def small_turbulent(n=12, np_=1000 + 37, nbins=64, **kw):
+    return I.workload(3).scaled(n=n, np=np_, nbins=nbins, **kw)
+
+
+def setup_pair(w, shuffle_ids=False, diag=True, jitter=True):
+    """Returns (lp, prm, fields_np, x, y, z, pid, chi) with the GPU side bound to copies."""
+    fields = I.make_fields(w, device="cpu")
+    u_rad = u_rad_of(w, fields)
+    f_np = fields_to_numpy(fields)
+    x, y, z, pid = I.make_particles(w, shuffle_ids=shuffle_ids)
+    chi = I.make_spectrum(w, jitter=jitter)
+    lp = P.LP(P.config_from_workload(w, u_rad=u_rad))
+    lp.set_fields(fields)
+    lp.bind_particles(x, y, z, pid, chi)
+    if diag:
+        lp.bind_diag()
+    return lp, oracle_params(w, u_rad), f_np, x, y, z, pid, chi
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+# ------------------------------------------------------------------ a1, a4: key and gather
+
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 0, 0), (1, 0, 1)])
+def test_key_and_gather_bit_exact(periodic):
+    w = small_turbulent(np_=4096 + 5, periodic=periodic)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    # put some particles on faces, on the domain edges and slightly outside
+    x[:8] = [-1.0, 1.0 - 1e-16, -1.0 + 2.0 / w.n, 0.0, 1.0, -1.0000001, 0.999999999, -0.5]
+    y[:4] = [-1.0, 0.0, 1.0 / 3.0, -1.0 + 2.0 / w.n * 5]
+    lp.bind_particles(x, y, z, pid, chi)
+    out7, key = lp.interpolate()
+    torch.cuda.synchronize()
+    want_key = orc.cell_key(prm, x, y, z)
+    assert np.array_equal(host(key).view(np.uint32), want_key)
+    want = orc.gather(prm, f_np, x, y, z)
+    assert np.array_equal(host(out7), want), "gather not bit-identical: max abs diff %g" % np.max(np.abs(host(out7) - want))
+
+
+def test_key_non_cubic_grid():
+    cfg = P.make_config(5, 7, 3, (-1, 0, 2), (1, 3.5, 2.75), (1, 1, 1), 500, 16, 1.0, 1e4)
+    rng = np.random.default_rng(0)
+    x = rng.uniform(-1, 1, 500); y = rng.uniform(0, 3.5, 500); z = rng.uniform(2, 2.75, 500)
+    lp = P.LP(cfg)
+    lp.bind_particles(x, y, z, np.arange(500, dtype=np.uint64), np.ones((500, 16)))
+    _, key = lp.interpolate(want_fields=False)
+    prm = orc.make_params(5, 7, 3, (-1, 0, 2), (1, 3.5, 2.75), (1, 1, 1), 16, 1.0, 1e4)
+    assert np.array_equal(host(key).view(np.uint32), orc.cell_key(prm, x, y, z))
+    f = [rng.normal(size=(3, 7, 5)) for _ in range(7)]
+    lp.set_fields([torch.from_numpy(a) for a in f])
+    out7, _ = lp.interpolate(want_key=False)
+    assert np.array_equal(host(out7), orc.gather(prm, f, x, y, z))
+
+
+# ------------------------------------------------------------------ a5, a6: push
+
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 0, 0)])
+def test_push_positions_bit_exact_over_steps(periodic):
+    w = small_turbulent(np_=3000 + 11, periodic=periodic)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    dt = w.dt * 3.0          # large steps: many wraps on the periodic box
+    for _ in range(25):
+        lp.push(dt, 0)
+        lp.push(dt, 1)
+        k1, rho_old, xs = orc.push_stage0(prm, f_np, x, y, z, dt)
+        x, y, z, st = orc.push_stage1(prm, f_np, x, y, z, xs, k1, dt)
+    torch.cuda.synchronize()
+    assert np.array_equal(host(lp.x), x) and np.array_equal(host(lp.y), y) and np.array_equal(host(lp.z), z)
+    if periodic == (1, 1, 1):
+        assert (x >= -1).all() and (x < 1).all()
+    d = lp.diag()
+    assert d["n_outside"] == 0 or periodic != (1, 1, 1)
+
+
+# ------------------------------------------------------------------ a2: sort
+
+@pytest.mark.parametrize("np_", [1, 31, 4097, 50000])
+def test_sort_order_and_permutation_bit_exact(np_):
+    w = small_turbulent(n=6, np_=np_, nbins=16)          # 216 cells: many ties per key
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
+    pid = pid + np.uint64(1 << 33) * (pid % np.uint64(3))        # ids wider than 32 bits
+    lp.bind_particles(x, y, z, pid, chi)
+    lp.sort()
+    torch.cuda.synchronize()
+    sx, sy, sz, sid, schi, skey, perm = oracle_sort_state(prm, x, y, z, pid, chi)
+    assert np.array_equal(host(lp.id).view(np.uint64), sid)
+    assert np.array_equal(host(lp.x), sx) and np.array_equal(host(lp.y), sy) and np.array_equal(host(lp.z), sz)
+    assert np.array_equal(host(lp.chi), schi)
+    _, key = lp.interpolate(want_fields=False)
+    assert np.array_equal(host(key).view(np.uint32), skey)
+
+
+# ------------------------------------------------------------------ a7-a10: spectral update
+
+@pytest.mark.parametrize("nbins", [16, 32, 64, 128, 256, 512])
+def test_spectral_update_matches_oracle(nbins):
+    # e range of workload 5 so that n_sub spans 1..~10 across the bin counts
+    w = small_turbulent(np_=2000 + 45, nbins=nbins, e_min=1.0, e_max=1e8, brms=3e-3)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    dt = w.dt
+    lp.push(dt, 0); lp.push(dt, 1); lp.spectral_update(dt)
+    k1, rho_old, xs = orc.push_stage0(prm, f_np, x, y, z, dt)
+    x1, y1, z1, st = orc.push_stage1(prm, f_np, x, y, z, xs, k1, dt)
+    chi1, nsub, lost = orc.spectral_update(prm, f_np, x1, y1, z1, rho_old, dt, chi, nthreads=8)
+    torch.cuda.synchronize()
+    assert np.array_equal(host(lp.x), x1)
+    assert_nsub_equal(host(lp.nsub), nsub, "(nbins=%d)" % nbins)
+    assert_chi_close(host(lp.chi), chi1)
+    E, dE, _ = orc.bin_table(nbins, w.e_min, w.e_max)
+    number = chi @ dE
+    assert np.max(np.abs(host(lp.lost) - lost) / number) < REL_TOL
+    if nbins >= 256:
+        assert nsub.max() > 1
+    # the library's bin table against the oracle's
+    Eg, dEg = lp.bins()
+    assert np.max(np.abs(Eg / E - 1)) < 1e-15 and np.max(np.abs(dEg / dE - 1)) < 1e-13
+
+
+def test_spectral_update_sign_changing_advection_and_cap():
+    """Strong compression/expansion (a of both signs) with losses; and the n_sub cap."""
+    w = small_turbulent(np_=3000, nbins=64, sigma_rho=2.0, brms=1e-2, max_substeps=3)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    dt = 4 * w.dt
+    lp.push(dt, 0); lp.push(dt, 1); lp.spectral_update(dt)
+    x1, y1, z1, chi1, nsub, lost, st = orc.step(prm, f_np, x, y, z, dt, chi, nthreads=8)
+    torch.cuda.synchronize()
+    assert (nsub < 0).any() and (nsub > 0).any()           # some capped, some not
+    assert_nsub_equal(host(lp.nsub), nsub)
+    capped = nsub < 0
+    assert_chi_close(host(lp.chi)[~capped], chi1[~capped])
+    # capped rows violate the CFL bound, the scheme may amplify rounding there: 1e-8 is enough
+    assert_chi_close(host(lp.chi)[capped], chi1[capped], tol=1e-8, what="capped chi")
+    d = lp.diag()
+    assert d["n_capped"] == int(capped.sum()) and d["max_substeps"] == 3
+    assert d["sum_substeps"] == int(np.abs(nsub).sum())
+
+
+def test_number_conservation_diag():
+    w = small_turbulent(np_=5000, nbins=128)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    n0 = lp.diag()["number"]
+    E, dE, _ = orc.bin_table(w.nbins, w.e_min, w.e_max)
+    assert abs(n0 / float((chi @ dE).sum()) - 1) < 1e-12
+    lp.step(w.dt)
+    d = lp.diag()
+    assert abs((d["number"] + d["lost"]) / n0 - 1) < 1e-12
+    assert d["steps"] == 1 and d["sorts"] == 0
+
+
+# ------------------------------------------------------------------ whole step, with re-sort
+
+@pytest.mark.parametrize("nbins,np_", [(64, 6000 + 3), (16, 2500), (128, 1500)])
+def test_lp_step_with_resort_matches_oracle(nbins, np_):
+    w = small_turbulent(n=10, np_=np_, nbins=nbins, sort_every=3)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
+    dt = w.dt
+    for s in range(8):
+        lp.step(dt)
+        if s % 3 == 0:
+            x, y, z, pid, chi, _, _ = oracle_sort_state(prm, x, y, z, pid, chi)
+        x, y, z, chi, nsub, lost, st = orc.step(prm, f_np, x, y, z, dt, chi, nthreads=8)
+    torch.cuda.synchronize()
+    assert np.array_equal(host(lp.id).view(np.uint64), pid)       # same order => compare in place
+    assert np.array_equal(host(lp.x), x) and np.array_equal(host(lp.z), z)
+    assert_nsub_equal(host(lp.nsub), nsub)
+    assert_chi_close(host(lp.chi), chi)
+    d = lp.diag()
+    assert d["steps"] == 8 and d["sorts"] == 3
+
+
+def test_lp_step_host_roundtrip():
+    w = small_turbulent(np_=4000, nbins=32)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    hx, hy, hz = (torch.from_numpy(a.copy()).pin_memory() for a in (x, y, z))
+    hid = torch.from_numpy(pid.view(np.int64).copy()).pin_memory()
+    hchi = torch.from_numpy(chi.copy()).pin_memory()
+    lp.step_host(w.dt, hx, hy, hz, hid, hchi)
+    x1, y1, z1, chi1, nsub, lost, st = orc.step(prm, f_np, x, y, z, w.dt, chi, nthreads=8)
+    assert np.array_equal(hx.numpy(), x1) and np.array_equal(hy.numpy(), y1)
+    assert_chi_close(hchi.numpy(), chi1)
+
+
+# ------------------------------------------------------------------ edge cases and error paths
+
+def test_empty_and_tiny_particle_sets():
+    for n_p in (0, 1, 2, 33):
+        w = small_turbulent(np_=n_p, nbins=16 if n_p % 2 else 64, sort_every=1)
+        lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+        lp.step(w.dt)
+        lp.step(w.dt)
+        torch.cuda.synchronize()
+        if n_p:
+            for _ in range(2):
+                x, y, z, pid, chi, _, _ = oracle_sort_state(prm, x, y, z, pid, chi)
+                x, y, z, chi, nsub, lost, st = orc.step(prm, f_np, x, y, z, w.dt, chi)
+            assert np.array_equal(host(lp.x), x)
+            assert_chi_close(host(lp.chi), chi)
+        assert lp.diag()["np"] == n_p
+
+
+def test_state_errors():
+    w = small_turbulent(np_=100)
+    cfg = P.config_from_workload(w)
+    lp = P.LP(cfg)
+    with pytest.raises(B.LPError) as e:
+        lp.step(0.1)                       # no particles bound
+    assert e.value.status == B.LP_ERR_STATE
+    x, y, z, pid = I.make_particles(w)
+    lp.bind_particles(x, y, z, pid, I.make_spectrum(w))
+    with pytest.raises(B.LPError) as e:
+        lp.push(0.1, 0)                    # fields not set
+    assert e.value.status == B.LP_ERR_STATE and "fields" in str(e.value)
+    lp.set_fields(I.make_fields(w))
+    with pytest.raises(B.LPError) as e:
+        lp.push(0.1, 1)                    # stage 1 before stage 0
+    assert e.value.status == B.LP_ERR_STATE
+    with pytest.raises(B.LPError) as e:
+        lp.spectral_update(0.1)            # needs rho_old of stage 0
+    assert e.value.status == B.LP_ERR_STATE
+    with pytest.raises(B.LPError) as e:
+        lp.push(0.1, 2)
+    assert e.value.status == B.LP_ERR_INVALID_ARG
+    ctx2 = B.lp_create(cfg)
+    with pytest.raises(B.LPError) as e:
+        B.lp_bind_workspace(ctx2, lp.workspace.data_ptr() + 8, lp.workspace_bytes)
+    assert e.value.status == B.LP_ERR_WORKSPACE
+    with pytest.raises(B.LPError) as e:
+        B.lp_bind_workspace(ctx2, lp.workspace.data_ptr() + (-lp.workspace.data_ptr()) % 256, 1024)
+    assert e.value.status == B.LP_ERR_WORKSPACE
+    B.lp_destroy(ctx2)
+    lp.push(0.1, 0); lp.push(0.1, 1); lp.spectral_update(0.1)      # and the good order works
+    torch.cuda.synchronize()
+    assert lp.launch_count() >= 4
