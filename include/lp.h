@@ -147,6 +147,12 @@ LP_API lp_status lp_timing_read(lp_ctx *ctx, double *spectral_ms_sum /*host*/, i
 /* Copy the library's bin table to host arrays: edges [nbins+1], widths [nbins] (either may be NULL). */
 LP_API lp_status lp_get_bins(const lp_ctx *ctx, double *edges /*host*/, double *widths /*host*/);
 
+/* The bins the CFL reduction (step a8) evaluates: on a fixed bin table the maximum outflow rate
+ * over all bins is attained, for every (a, c_r >= 0), at a vertex of the convex hull of the bins'
+ * coefficient points, found once at lp_create.  bins [*n] on return (capacity >= 24); *n = -1 means
+ * every bin is scanned.  Needs no GPU (valid even when lp_create returned LP_ERR_CUDA). */
+LP_API lp_status lp_get_cfl_bins(const lp_ctx *ctx, int32_t *bins /*host*/, int32_t *n /*host*/);
+
 #ifdef __cplusplus
 }
 #endif

@@ -17,7 +17,7 @@ _STATUS_NAMES = {0: "LP_OK", -1: "LP_ERR_INVALID_ARG", -2: "LP_ERR_STATE", -3: "
 EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp_bind_workspace",
            "lp_bind_particles", "lp_bind_diag", "lp_set_fields", "lp_interpolate", "lp_sort", "lp_push",
            "lp_spectral_update", "lp_step", "lp_step_host", "lp_get_diag", "lp_launch_count", "lp_get_bins",
-           "lp_timing_enable", "lp_timing_read")
+           "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins")
 
 
 class LPError(RuntimeError):
@@ -79,6 +79,7 @@ def load():
     lib.lp_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     lib.lp_get_bins.argtypes = [vp, dp, dp]
     lib.lp_timing_enable.argtypes = [vp, C.c_int]
+    lib.lp_get_cfl_bins.argtypes = [vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.lp_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
     for name in EXPORTS:
         if name != "lp_last_error":
@@ -184,6 +185,12 @@ def lp_launch_count(ctx):
     out = C.c_int64()
     _check(ctx, load().lp_launch_count(ctx, C.byref(out)))
     return out.value
+
+
+def lp_get_cfl_bins(ctx):
+    bins = (C.c_int32 * 64)(); n = C.c_int32()
+    _check(ctx, load().lp_get_cfl_bins(ctx, bins, C.byref(n)))
+    return None if n.value < 0 else [bins[k] for k in range(n.value)]
 
 
 def lp_timing_enable(ctx, max_records):

@@ -1,6 +1,7 @@
 // lp_api.cu -- the C ABI of include/lp.h: context, validation, workspace layout, launch order.
 // Host code only; every step of the path runs in the kernels of lp_particles.cu, lp_spectral.cu
 // and lp_sort.cu.  No CPU fallback exists.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -50,6 +51,65 @@ Layout make_layout(const lp_config &c)
     return L;
 }
 
+// Bins that can carry the maximum outflow rate for some (a, c_r >= 0) -- see LpLamCand.
+//   gain term  P_i = -(a + c_r E_{i+1}) E_{i+1}/dE_i = (-a) * alpha_i - c_r * beta_i     (needs a < 0)
+//   loss term  Q_i =  (a + c_r E_i)     E_i/dE_i     =   a  * alpha'_i + c_r * beta'_i
+// The maximiser of a linear function over a point set is a vertex of its convex hull; walking the
+// hull over the admissible range of directions visits exactly the vertices that can win.
+// Long-double arithmetic on the rounded table values.
+// Gift wrapping, counter-clockwise from the rightmost (lowest) point, using orientation tests only.
+// An edge (dx, dy) of the counter-clockwise hull has outward normal (dy, -dx): the direction at which
+// its far end overtakes its near end.  The walk stops when that normal leaves the admissible cone:
+// quarter = true: directions (u, v) with u >= 0, v >= 0;  quarter = false: v >= 0.
+void hull_walk(const std::vector<long double> &px, const std::vector<long double> &py, bool quarter,
+               std::vector<int> &out)
+{
+    const int n = (int)px.size();
+    int cur = 0;
+    for (int i = 1; i < n; ++i)
+        if (px[i] > px[cur] || (px[i] == px[cur] && py[i] < py[cur])) cur = i;
+    for (int guard = 0; guard <= n; ++guard) {
+        out.push_back(cur);
+        int nxt = -1;
+        for (int j = 0; j < n; ++j) {
+            if (j == cur || (px[j] == px[cur] && py[j] == py[cur])) continue;
+            if (nxt < 0) { nxt = j; continue; }
+            const long double ax = px[nxt] - px[cur], ay = py[nxt] - py[cur];
+            const long double bx = px[j] - px[cur], by = py[j] - py[cur];
+            const long double cr = ax * by - ay * bx;          // > 0: j is to the left of cur->nxt
+            if (cr < 0.0L || (cr == 0.0L && bx * bx + by * by > ax * ax + ay * ay)) nxt = j;
+        }
+        if (nxt < 0) break;
+        const long double dx = px[nxt] - px[cur], dy = py[nxt] - py[cur];
+        if (dx > 0.0L || (quarter && dy < 0.0L)) break;        // normal (dy, -dx) left the cone
+        cur = nxt;
+    }
+}
+
+LpLamCand make_candidates(const std::vector<double> &E, const std::vector<double> &dE)
+{
+    const int nb = (int)dE.size();
+    std::vector<long double> ax(nb), ay(nb), bx(nb), by(nb);
+    for (int i = 0; i < nb; ++i) {
+        const long double e0 = E[i], e1 = E[i + 1], d = dE[i];
+        ax[i] = e1 / d;  ay[i] = -(e1 * e1 / d);      // gain: maximise (-a)*alpha - c_r*beta, (-a) > 0, c_r >= 0
+        bx[i] = e0 / d;  by[i] = e0 * e0 / d;         // loss: maximise a*alpha' + c_r*beta', c_r >= 0, any a
+    }
+    std::vector<int> v;
+    hull_walk(ax, ay, true, v);
+    hull_walk(bx, by, false, v);
+    v.push_back(0);
+    v.push_back(nb - 1);
+    std::sort(v.begin(), v.end());
+    v.erase(std::unique(v.begin(), v.end()), v.end());
+    LpLamCand c;
+    std::memset(&c, 0, sizeof c);
+    if ((int)v.size() > kLpMaxCand) { c.n = -1; return c; }
+    c.n = (int)v.size();
+    for (int k = 0; k < c.n; ++k) c.bin[k] = v[k];
+    return c;
+}
+
 bool nbins_ok(int nb) { return nb == 16 || nb == 32 || nb == 64 || nb == 128 || nb == 256 || nb == 512; }
 
 int bit_length(unsigned long long v) { int b = 0; while (v) { ++b; v >>= 1; } return b; }
@@ -71,6 +131,7 @@ struct lp_ctx {
     // owned small tables
     double *tab = nullptr;                 // E[nb+1] | dE[nb] | rdE[nb]
     std::vector<double> h_edges, h_widths;
+    LpLamCand cand;
     // state
     bool have_fields = false, stage0_done = false, spectra_done = false;
     int id_bits = 0, key_bits = 0;
@@ -155,10 +216,12 @@ LpPushArgs push_args(lp_ctx *c, double dt)
     return a;
 }
 
-lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, cudaStream_t s)
+lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cudaStream_t s)
 {
     LpSpectralArgs a;
     a.g = c->geom;
+    a.cand = c->cand;
+    a.status = c->at<int32_t>(c->lay.status);
     a.cells = c->cells();
     a.x = c->x; a.y = c->y; a.z = c->z;
     a.rho_old = c->at<double>(c->lay.rho_old);
@@ -177,7 +240,7 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, cudaStream_t s
     a.max_substeps = c->cfg.max_substeps;
     const bool rec = c->timing && c->ev_used + 2 <= c->ev.size();
     if (rec) LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used], s));
-    lp_status st = count(c, lp_launch_spectral(a, c->cfg.nbins, c->lost_user != nullptr, c->sm_count, s),
+    lp_status st = count(c, lp_launch_spectral(a, c->cfg.nbins, c->lost_user != nullptr, fused, c->sm_count, s),
                          "lp_spectral_kernel launch");
     if (rec) {
         LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], s));
@@ -258,6 +321,7 @@ lp_status lp_create(const lp_config *cfg, lp_ctx **out)
     }
     c->h_edges.assign(tab.begin(), tab.begin() + nb + 1);
     c->h_widths.assign(tab.begin() + nb + 1, tab.begin() + 2 * nb + 1);
+    c->cand = make_candidates(c->h_edges, c->h_widths);
     *out = c;
     LP_CUDA(c, cudaSetDevice(cfg->device));
     int sm = 0;
@@ -391,7 +455,7 @@ lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
     if (!ctx->stage0_done) return fail(ctx, LP_ERR_STATE, "lp_spectral_update needs rho_old of lp_push stage 0");
     if (ctx->cfg.np == 0) return LP_OK;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    return do_spectral(ctx, dt, ctx->chi, static_cast<cudaStream_t>(stream));
+    return do_spectral(ctx, dt, ctx->chi, false, static_cast<cudaStream_t>(stream));
 }
 
 lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
@@ -410,11 +474,8 @@ lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
         if ((st = do_sort(ctx, false, s)) != LP_OK) return st;
         chi_in = ctx->at<double>(ctx->lay.chi_alt);
     }
-    LpPushArgs a = push_args(ctx, dt);
-    if ((st = count(ctx, lp_launch_push0(a, s), "lp_push0_kernel launch")) != LP_OK) return st;
-    ctx->stage0_done = true;
-    if ((st = count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch")) != LP_OK) return st;
-    return do_spectral(ctx, dt, chi_in, s);
+    // frozen fields: both push stages run inside the spectral kernel's per-particle phase
+    return do_spectral(ctx, dt, chi_in, true, s);
 }
 
 lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *hz, uint64_t *hid, double *hchi,
@@ -483,6 +544,14 @@ lp_status lp_launch_count(const lp_ctx *ctx, int64_t *out)
 {
     if (!ctx || !out) return LP_ERR_INVALID_ARG;
     *out = ctx->launches;
+    return LP_OK;
+}
+
+lp_status lp_get_cfl_bins(const lp_ctx *ctx, int32_t *bins, int32_t *n)
+{
+    if (!ctx || !bins || !n) return LP_ERR_INVALID_ARG;
+    *n = ctx->cand.n;
+    for (int k = 0; k < ctx->cand.n; ++k) bins[k] = ctx->cand.bin[k];
     return LP_OK;
 }
 

@@ -10,9 +10,19 @@
 
 __device__ __forceinline__ double2 ldg2(const double *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
 
+// floor-mod for an index far outside the grid (kept out of line: the integer division is long)
+static __device__ __noinline__ int lp_wrap_far(int i, int n)
+{
+    int m = i % n;
+    return m < 0 ? m + n : m;
+}
+
 __device__ __forceinline__ int lp_wrap(int i, int n, int periodic)
 {
-    if (periodic) { int m = i % n; return m < 0 ? m + n : m; }
+    if (periodic) {
+        if (i >= -n && i < 2 * n) return i < 0 ? i + n : (i >= n ? i - n : i);   // the usual case, no division
+        return lp_wrap_far(i, n);
+    }
     return min(max(i, 0), n - 1);
 }
 

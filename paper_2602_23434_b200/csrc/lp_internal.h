@@ -22,11 +22,24 @@ struct LpCells {
     const double4 *recB;
 };
 
+// Bins at which the outflow rate (max(w_{i+1},0) - min(w_i,0))/dE_i can be the maximum over the
+// row for some (a, c_r >= 0): both clamped terms are linear in (a, c_r), so the maximum over bins is
+// attained at a vertex of the convex hull of their coefficient points; lp_create finds those
+// vertices once per bin table (on a log grid: the two end bins plus rounding-noise neighbours).
+// n < 0: table degenerate, scan every bin.
+constexpr int kLpMaxCand = 24;
+struct LpLamCand {
+    int n;
+    int bin[kLpMaxCand];
+};
+
 struct LpSpectralArgs {
     LpGeom g;
+    LpLamCand cand;
     LpCells cells;
-    const double *x, *y, *z;     // positions at which the coefficients are gathered (x^{n+1})
-    const double *rho_old;       // from push stage 0
+    double *x, *y, *z;           // staged: x^{n+1} (read only).  fused: x^n in, x^{n+1} out
+    const double *rho_old;       // staged: from push stage 0.  fused: unused
+    int32_t *status;             // fused: outside-box flags [np]
     const double *chi_in;        // [np][nbins]  (may differ from chi_out after a re-sort)
     double *chi_out;             // [np][nbins]
     const double *tab;           // device bin table: E[nb+1] | dE[nb] | rdE[nb]
@@ -58,7 +71,8 @@ int lp_launch_interpolate(const LpGeom &g, const LpCells &c, const double *x, co
                           const double *z, long long np, double *out7, uint32_t *key, cudaStream_t s);
 int lp_launch_push0(const LpPushArgs &a, cudaStream_t s);
 int lp_launch_push1(const LpPushArgs &a, cudaStream_t s);
-int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, int sm_count, cudaStream_t s);
+// fused = true: the kernel also does both push stages (a5, a6) in its per-particle phase (frozen fields)
+int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, bool fused, int sm_count, cudaStream_t s);
 
 // sort: fills perm[n] = source index of the n-th particle in (key, id) order.
 struct LpSortBufs {

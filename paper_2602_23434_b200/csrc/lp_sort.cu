@@ -51,47 +51,63 @@ lp_radix_hist_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__rest
     hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = sh[threadIdx.x];
 }
 
-// exclusive scan of n u32 values in place, one block of 1024 threads
-__global__ void __launch_bounds__(1024) lp_scan_kernel(uint32_t *__restrict__ v, long long n)
+// Per-digit exclusive scan over blocks: block d scans hist[d][0..nblocks) in place and writes the
+// digit total to totals[d].  The scatter kernel adds the exclusive prefix of the totals itself.
+__global__ void __launch_bounds__(kThreads)
+lp_scan_rows_kernel(uint32_t *__restrict__ hist, int nblocks, uint32_t *__restrict__ totals)
 {
-    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t wsum[kWarps];
+    __shared__ uint32_t carry_s;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    const long long per = (n + 1023) / 1024;
-    const long long b = (long long)t * per;
-    const long long e = b + per < n ? b + per : n;
-    uint32_t s = 0;
-    for (long long i = b; i < e; ++i) s += v[i];
-    uint32_t inc = s;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        uint32_t u = __shfl_up_sync(kFull, inc, o);
-        if (lane >= o) inc += u;
-    }
-    if (lane == 31) wsum[warp] = inc;
+    uint32_t *row = hist + (size_t)blockIdx.x * nblocks;
+    if (t == 0) carry_s = 0;
     __syncthreads();
-    if (warp == 0) {
-        uint32_t w = wsum[lane], winc = w;
+    for (int b0 = 0; b0 < nblocks; b0 += kThreads) {
+        const int i = b0 + t;
+        const uint32_t v = i < nblocks ? row[i] : 0u;
+        uint32_t inc = v;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            uint32_t u = __shfl_up_sync(kFull, winc, o);
-            if (lane >= o) winc += u;
+            uint32_t u = __shfl_up_sync(kFull, inc, o);
+            if (lane >= o) inc += u;
         }
-        wsum[lane] = winc - w;
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        uint32_t wbase = 0;
+        for (int w = 0; w < warp; ++w) wbase += wsum[w];
+        const uint32_t carry = carry_s;
+        if (i < nblocks) row[i] = carry + wbase + inc - v;
+        __syncthreads();
+        if (t == kThreads - 1) carry_s = carry + wbase + inc;
+        __syncthreads();
     }
-    __syncthreads();
-    uint32_t run = wsum[warp] + inc - s;
-    for (long long i = b; i < e; ++i) { uint32_t x = v[i]; v[i] = run; run += x; }
+    if (t == 0) totals[blockIdx.x] = carry_s;
 }
 
 __global__ void __launch_bounds__(kThreads)
 lp_radix_scatter_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__restrict__ id,
                         const uint32_t *__restrict__ key, long long np, int use_key, int shift,
-                        const uint32_t *__restrict__ hist, int nblocks, uint32_t *__restrict__ idx_out)
+                        const uint32_t *__restrict__ hist, const uint32_t *__restrict__ totals, int nblocks,
+                        uint32_t *__restrict__ idx_out)
 {
     __shared__ uint32_t base[256];
     __shared__ uint32_t wcount[kWarps][256];
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    base[t] = hist[(size_t)t * nblocks + blockIdx.x];
+    {   // exclusive prefix of the 256 digit totals (256 threads, one digit each)
+        const uint32_t v = totals[t];
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t u = __shfl_up_sync(kFull, inc, o);
+            if (lane >= o) inc += u;
+        }
+        if (lane == 31) base[warp] = inc;
+        __syncthreads();
+        uint32_t wbase = 0;
+        for (int w = 0; w < warp; ++w) wbase += base[w];
+        __syncthreads();
+        base[t] = wbase + inc - v + hist[(size_t)t * nblocks + blockIdx.x];
+    }
     const long long t0 = (long long)blockIdx.x * kTile;
     for (int r = 0; r < kItems; ++r) {
 #pragma unroll
@@ -233,7 +249,7 @@ inline bool ok() { return cudaPeekAtLastError() == cudaSuccess; }
 
 }  // namespace
 
-size_t lp_sort_hist_elems(long long np) { return (size_t)256 * (size_t)blocks_for(np, kTile); }
+size_t lp_sort_hist_elems(long long np) { return (size_t)256 * (size_t)blocks_for(np, kTile) + 256; }
 
 int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const double *z, const uint64_t *id,
                         long long np, int id_bits, int key_bits, const LpSortBufs &b, uint32_t **perm_out,
@@ -252,8 +268,9 @@ int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const
         const int use_key = pass >= id_passes ? 1 : 0;
         const int shift = 8 * (use_key ? pass - id_passes : pass);
         lp_radix_hist_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, nblocks);
-        lp_scan_kernel<<<1, 1024, 0, s>>>(b.hist, (long long)256 * nblocks);
-        lp_radix_scatter_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, nblocks, bufs[cur]);
+        uint32_t *totals = b.hist + (size_t)256 * nblocks;
+        lp_scan_rows_kernel<<<256, kThreads, 0, s>>>(b.hist, nblocks, totals);
+        lp_radix_scatter_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, totals, nblocks, bufs[cur]);
         launches += 3;
         in = bufs[cur];
         cur ^= 1;

@@ -20,7 +20,7 @@ def declared_symbols():
 def test_library_exports_every_declared_symbol():
     lib = B.load()
     names = declared_symbols()
-    assert len(names) == 19 and set(names) == set(B.EXPORTS)
+    assert len(names) == 20 and set(names) == set(B.EXPORTS)
     for n in names:
         assert getattr(lib, n) is not None
 
@@ -105,3 +105,34 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "lp_oracle" not in src, f
+
+
+@pytest.mark.parametrize("nbins,e_min,e_max", [(16, 1.0, 1e8), (64, 1e1, 1e6), (64, 1.0, 1e8), (128, 1.0, 1e7),
+                                                (256, 1.0, 1e8), (512, 1.0, 1e8), (32, 0.5, 3.0)])
+def test_cfl_candidate_bins_carry_the_maximum(nbins, e_min, e_max):
+    """Host logic of step a8: lp_create reduces the CFL max over bins to the hull-vertex bins.
+    Brute force over all bins (plain numpy fp64, the oracle's formula) must give the same lambda for
+    any (a, c_r >= 0) up to the rounding of one evaluation."""
+    import numpy as np
+    lib = B.load()
+    c = cfg(nbins=nbins, e_min=e_min, e_max=e_max)
+    ctx = C.c_void_p()
+    st = lib.lp_create(C.byref(c), C.byref(ctx))      # no GPU here: LP_ERR_CUDA, but the context exists
+    assert ctx and st in (B.LP_OK, B.LP_ERR_CUDA)
+    try:
+        cand = B.lp_get_cfl_bins(ctx)
+        E, dE = B.lp_get_bins(ctx, nbins)
+    finally:
+        lib.lp_destroy(ctx)
+    assert cand is not None and 0 in cand and nbins - 1 in cand and len(cand) <= 24
+    rng = np.random.default_rng(nbins)
+    cases = [(a, cr) for a in (-3.0, -1e-3, 0.0, 1e-3, 2.0) for cr in (0.0, 1e-9, 1e-6, 1e-3)]
+    cases += [(float(rng.normal() * 10 ** rng.uniform(-4, 2)), float(10 ** rng.uniform(-12, -2))) for _ in range(400)]
+    # sign change of w placed inside the table: a = -c_r * E_k
+    cases += [(-1e-6 * float(E[k]) * (1 + 1e-9), 1e-6) for k in range(0, nbins + 1, max(1, nbins // 16))]
+    for a, cr in cases:
+        w = -E * (a + cr * E)
+        out = (np.maximum(w[1:], 0.0) - np.minimum(w[:-1], 0.0)) / dE
+        lam_all = out.max()
+        lam_cand = out[cand].max()
+        assert lam_all <= lam_cand * (1 + 1e-15), (a, cr, int(out.argmax()), cand)

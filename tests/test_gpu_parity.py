@@ -114,16 +114,18 @@ def test_sort_order_and_permutation_bit_exact(np_):
 
 @pytest.mark.parametrize("nbins", [16, 32, 64, 128, 256, 512])
 def test_spectral_update_matches_oracle(nbins):
-    # e range of workload 5 so that n_sub spans 1..~10 across the bin counts
+    # e range of workload 5 and a strong field: n_sub spans 1 (16 bins) to O(10^2..10^3) (512 bins),
+    # all below the cap (a capped row violates the CFL bound and is compared separately below)
     w = small_turbulent(np_=2000 + 45, nbins=nbins, e_min=1.0, e_max=1e8, brms=3e-3)
     lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
-    dt = w.dt
+    dt = 0.005
     lp.push(dt, 0); lp.push(dt, 1); lp.spectral_update(dt)
     k1, rho_old, xs = orc.push_stage0(prm, f_np, x, y, z, dt)
     x1, y1, z1, st = orc.push_stage1(prm, f_np, x, y, z, xs, k1, dt)
     chi1, nsub, lost = orc.spectral_update(prm, f_np, x1, y1, z1, rho_old, dt, chi, nthreads=8)
     torch.cuda.synchronize()
     assert np.array_equal(host(lp.x), x1)
+    assert (nsub > 0).all(), "test set-up: no row may hit the substep cap here"
     assert_nsub_equal(host(lp.nsub), nsub, "(nbins=%d)" % nbins)
     assert_chi_close(host(lp.chi), chi1)
     E, dE, _ = orc.bin_table(nbins, w.e_min, w.e_max)
@@ -138,7 +140,7 @@ def test_spectral_update_matches_oracle(nbins):
 
 def test_spectral_update_sign_changing_advection_and_cap():
     """Strong compression/expansion (a of both signs) with losses; and the n_sub cap."""
-    w = small_turbulent(np_=3000, nbins=64, sigma_rho=2.0, brms=1e-2, max_substeps=3)
+    w = small_turbulent(np_=3000, nbins=64, sigma_rho=2.0, brms=1e-3, max_substeps=12)
     lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
     dt = 4 * w.dt
     lp.push(dt, 0); lp.push(dt, 1); lp.spectral_update(dt)
@@ -148,10 +150,12 @@ def test_spectral_update_sign_changing_advection_and_cap():
     assert_nsub_equal(host(lp.nsub), nsub)
     capped = nsub < 0
     assert_chi_close(host(lp.chi)[~capped], chi1[~capped])
-    # capped rows violate the CFL bound, the scheme may amplify rounding there: 1e-8 is enough
-    assert_chi_close(host(lp.chi)[capped], chi1[capped], tol=1e-8, what="capped chi")
+    # capped rows violate the CFL bound: the scheme is unstable there (chi changes sign, rounding is
+    # amplified), so they are compared against the row's scale instead of element by element
+    gc, oc = host(lp.chi)[capped], chi1[capped]
+    assert np.all(np.abs(gc - oc) <= 1e-8 * np.abs(oc).max(axis=1, keepdims=True))
     d = lp.diag()
-    assert d["n_capped"] == int(capped.sum()) and d["max_substeps"] == 3
+    assert d["n_capped"] == int(capped.sum()) and d["max_substeps"] == 12
     assert d["sum_substeps"] == int(np.abs(nsub).sum())
 
 
