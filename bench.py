@@ -36,6 +36,7 @@ def parse():
     ap.add_argument("--workload", type=int, default=4)
     ap.add_argument("--nbins", type=int, default=0, help="override the bin count (workload 5 sweep)")
     ap.add_argument("--np", type=int, default=0, help="override the particle count (debugging only)")
+    ap.add_argument("--grid", type=int, default=0, help="override the cells per axis (debugging only)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -110,6 +111,8 @@ def pick_workload(args):
         kw["nbins"] = args.nbins
     if args.np:
         kw["np"] = args.np
+    if args.grid:
+        kw["n"] = args.grid
     return w.scaled(**kw) if kw else w
 
 

@@ -83,55 +83,100 @@ __device__ __forceinline__ void lp_stencil(const LpGeom &g, double x, double y, 
 
 __device__ __forceinline__ double lp_acc(double acc, double w, double q) { return __dadd_rn(acc, __dmul_rn(w, q)); }
 
+// One 32-byte cell record per request: sm_100a has 256-bit global loads (LDG.E.256), which halve
+// the L1 request count of the gather (the per-particle phase is bound by L1 requests, one per lane
+// and divergent address, not by bytes).
+struct LpRec { double a, b, c, d; };
+__device__ __forceinline__ LpRec lp_ldg_rec(const double4 *p)
+{
+    LpRec r;
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.a), "=d"(r.b), "=d"(r.c), "=d"(r.d) : "l"(p));
+    return r;
+}
+
+// The eight (vx, vy, vz, rho) corner records of a stencil, kept in registers across the gathers of
+// one step: x^n, x* and x^{n+1} of a particle mostly share their stencil (|v| dt < dx/2), and a
+// record that is already in registers costs no L1 request.  The records are reloaded only by the
+// lanes whose stencil moved; values are the same bits either way.
+struct LpCornersA {
+    LpRec r[8];
+    long long c0, c7;           // cells of corners 0 and 7 of the loaded stencil (they fix all eight)
+    __device__ __forceinline__ void load(const LpCells &cells, const LpStencil &st)
+    {
+#pragma unroll
+        for (int n = 0; n < 8; ++n) r[n] = lp_ldg_rec(cells.recA + st.c[n]);
+        c0 = st.c[0];
+        c7 = st.c[7];
+    }
+    __device__ __forceinline__ void update(const LpCells &cells, const LpStencil &st)
+    {
+        if (st.c[0] != c0 || st.c[7] != c7) load(cells, st);
+    }
+    // (vx, vy, vz, rho)
+    __device__ __forceinline__ void gather4(const LpStencil &st, double out[4]) const
+    {
+        out[0] = out[1] = out[2] = out[3] = 0.0;
+#pragma unroll
+        for (int n = 0; n < 8; ++n) {
+            out[0] = lp_acc(out[0], st.w[n], r[n].a);
+            out[1] = lp_acc(out[1], st.w[n], r[n].b);
+            out[2] = lp_acc(out[2], st.w[n], r[n].c);
+            out[3] = lp_acc(out[3], st.w[n], r[n].d);
+        }
+    }
+    // (vx, vy, vz)
+    __device__ __forceinline__ void gather3(const LpStencil &st, double out[3]) const
+    {
+        out[0] = out[1] = out[2] = 0.0;
+#pragma unroll
+        for (int n = 0; n < 8; ++n) {
+            out[0] = lp_acc(out[0], st.w[n], r[n].a);
+            out[1] = lp_acc(out[1], st.w[n], r[n].b);
+            out[2] = lp_acc(out[2], st.w[n], r[n].c);
+        }
+    }
+};
+
 // (vx, vy, vz, rho) from record A
 __device__ __forceinline__ void lp_gather_A(const LpCells &cells, const LpStencil &st, double out[4])
 {
-    out[0] = out[1] = out[2] = out[3] = 0.0;
-#pragma unroll
-    for (int n = 0; n < 8; ++n) {
-        const double *r = reinterpret_cast<const double *>(cells.recA + st.c[n]);
-        double2 a = ldg2(r), b = ldg2(r + 2);
-        out[0] = lp_acc(out[0], st.w[n], a.x);
-        out[1] = lp_acc(out[1], st.w[n], a.y);
-        out[2] = lp_acc(out[2], st.w[n], b.x);
-        out[3] = lp_acc(out[3], st.w[n], b.y);
-    }
+    LpCornersA k;
+    k.load(cells, st);
+    k.gather4(st, out);
 }
 
 // (vx, vy, vz) only: rho is loaded (same 32-byte record) but not accumulated
 __device__ __forceinline__ void lp_gather_v(const LpCells &cells, const LpStencil &st, double out[3])
 {
-    out[0] = out[1] = out[2] = 0.0;
-#pragma unroll
-    for (int n = 0; n < 8; ++n) {
-        const double *r = reinterpret_cast<const double *>(cells.recA + st.c[n]);
-        double2 a = ldg2(r);
-        double vz = __ldg(r + 2);
-        out[0] = lp_acc(out[0], st.w[n], a.x);
-        out[1] = lp_acc(out[1], st.w[n], a.y);
-        out[2] = lp_acc(out[2], st.w[n], vz);
-    }
+    LpCornersA k;
+    k.load(cells, st);
+    k.gather3(st, out);
 }
 
 // (bx, by, bz) from record B
 __device__ __forceinline__ void lp_gather_B(const LpCells &cells, const LpStencil &st, double out[3])
 {
+    LpRec r[8];
+#pragma unroll
+    for (int n = 0; n < 8; ++n) r[n] = lp_ldg_rec(cells.recB + st.c[n]);
     out[0] = out[1] = out[2] = 0.0;
 #pragma unroll
     for (int n = 0; n < 8; ++n) {
-        const double *r = reinterpret_cast<const double *>(cells.recB + st.c[n]);
-        double2 a = ldg2(r);
-        double bz = __ldg(r + 2);
-        out[0] = lp_acc(out[0], st.w[n], a.x);
-        out[1] = lp_acc(out[1], st.w[n], a.y);
-        out[2] = lp_acc(out[2], st.w[n], bz);
+        out[0] = lp_acc(out[0], st.w[n], r[n].a);
+        out[1] = lp_acc(out[1], st.w[n], r[n].b);
+        out[2] = lp_acc(out[2], st.w[n], r[n].c);
     }
 }
 
 // periodic wrap into [lo, hi): x -= L*floor((x - lo)/L); a result >= hi becomes lo   (R15)
+// For 0 <= x - lo < L (both rounded) the rounded quotient is in [0, 1): its floor is 0 and x is
+// unchanged, so the division is skipped there; the result is bit-identical either way.
 __device__ __forceinline__ double lp_wrap_pos(double x, double lo, double hi, double L)
 {
-    double t = floor(__ddiv_rn(__dsub_rn(x, lo), L));
-    x = __dsub_rn(x, __dmul_rn(L, t));
+    const double d = __dsub_rn(x, lo);
+    if (!(d >= 0.0 && d < L)) {
+        const double t = floor(__ddiv_rn(d, L));
+        x = __dsub_rn(x, __dmul_rn(L, t));
+    }
     return x >= hi ? lo : x;
 }

@@ -2,15 +2,17 @@
 // when fused, the two push stages (a5, a6) in front of it.
 //
 // Phase 1 (one thread = one particle): [push 0, push 1,] gather v, B, rho at x^{n+1}, coefficients,
-// CFL substep count.  Phase 2 (one warp = one row, N_b bins spread over the lanes, M = N_b/32
-// contiguous bins per lane in registers): n_sub donor-cell upwind substeps of Eq. 6
-// with the loss term of Eq. 4; the only cross-lane traffic per substep is one
-// shuffle up and one shuffle down of a double.
+// CFL substep count.  Phase 2 (a group of G = N_b/M lanes = one row, M contiguous bins per lane in
+// registers): n_sub donor-cell upwind substeps of Eq. 6 with the loss term of Eq. 4
+// (PAPER.md:96); the only cross-lane traffic per substep is one shuffle up and one shuffle down.
 //
-// Two row movers:
-//  * lp_spectral_bulk_kernel (N_b <= 128): every warp streams its rows through a private ring of
-//    shared-memory slots filled and drained by the TMA engine (cp.async.bulk + mbarrier), so that
-//    several KB per warp are in flight while the warp computes, independent of registers.
+// Two kernels:
+//  * lp_spectral_bulk_kernel (N_b <= 128), warp-specialised: particle warps run phase 1 and hand the
+//    coefficients through a shared-memory ring (mbarrier full/empty) to row warps, which stream the
+//    rows through private rings of shared-memory slots filled and drained by the TMA engine
+//    (cp.async.bulk + mbarrier).  Measured on B200: phase 1 is a chain of dependent gathers (latency)
+//    and phase 2 a stream (HBM); run by the same warp one after the other their times add, run by
+//    different warps they overlap.
 //  * lp_spectral_direct_kernel (N_b >= 256): rows go global -> registers -> global; these bin counts
 //    are bound by the fp64 pipe (n_sub ~ 5-10), not by HBM.
 // sm_100a.
@@ -20,12 +22,12 @@ namespace {
 
 constexpr unsigned kFull = 0xffffffffu;
 
-struct __align__(16) LpCoef {      // per-particle scalars handed from phase 1 to phase 2
-    double a;      // (1/3) div_mu u^mu
-    double cr;     // c_r
-    double dts;    // dtau / n_sub
+// Per-particle scalars handed from phase 1 to phase 2.  The substeps only ever need the products
+// (dtau/n_sub)/2 * a and (dtau/n_sub)/2 * c_r, so phase 1 (one thread per particle) forms them once.
+struct LpCoef {
+    double a2;     // (dts/2) * a,    a = (1/3) div_mu u^mu,   dts = dtau / n_sub
+    double cr2;    // (dts/2) * c_r
     int ns;        // n_sub (0 = no particle)
-    int pad;
 };
 
 // outflow rate of bin i:  (max(w_{i+1},0) - min(w_i,0)) / dE_i,   w_k = -E_k (a + c_r E_k)
@@ -44,17 +46,20 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
                                           const double *sR, LpCoef &c, int &ns_signed)
 {
     LpStencil st;
+    LpCornersA ka;
     double px = A.x[p], py = A.y[p], pz = A.z[p];
     double rho_old;
     double qa[4], qb[3];
     if (FUSED) {
         lp_stencil(A.g, px, py, pz, st);
-        lp_gather_A(A.cells, st, qa);                       // k1 = v(x^n), rho_old = rho(x^n)
+        ka.load(A.cells, st);
+        ka.gather4(st, qa);                                 // k1 = v(x^n), rho_old = rho(x^n)
         rho_old = qa[3];
         lp_stencil(A.g, __dadd_rn(px, __dmul_rn(A.dt, qa[0])), __dadd_rn(py, __dmul_rn(A.dt, qa[1])),
                    __dadd_rn(pz, __dmul_rn(A.dt, qa[2])), st);
         double k2[3];
-        lp_gather_v(A.cells, st, k2);
+        ka.update(A.cells, st);
+        ka.gather3(st, k2);
         const double hdt = __dmul_rn(0.5, A.dt);
         double pos[3] = { px, py, pz };
         int stt = 0;
@@ -68,11 +73,14 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
         px = pos[0]; py = pos[1]; pz = pos[2];
         A.x[p] = px; A.y[p] = py; A.z[p] = pz;
         A.status[p] = stt;
+        lp_stencil(A.g, px, py, pz, st);
+        ka.update(A.cells, st);
     } else {
         rho_old = A.rho_old[p];
+        lp_stencil(A.g, px, py, pz, st);
+        ka.load(A.cells, st);
     }
-    lp_stencil(A.g, px, py, pz, st);
-    lp_gather_A(A.cells, st, qa);
+    ka.gather4(st, qa);
     lp_gather_B(A.cells, st, qb);
     // gamma_g, dtau, c_r (Eq. 4), a (continuity)
     const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(qa[0], qa[0]), __dmul_rn(qa[1], qa[1])), __dmul_rn(qa[2], qa[2]));
@@ -93,11 +101,10 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
     int n = !(need >= 1.0) ? 1 : (need > 2.0e9 ? 2000000000 : (int)need);
     const bool capped = n > A.max_substeps;
     if (capped) n = A.max_substeps;
-    c.a = a;
-    c.cr = cr;
-    c.dts = __ddiv_rn(dtau, (double)n);
+    const double hdts = 0.5 * __ddiv_rn(dtau, (double)n);      // (dtau / n_sub) / 2, the /2 is exact
+    c.a2 = hdts * a;
+    c.cr2 = hdts * cr;
     c.ns = n;
-    c.pad = 0;
     ns_signed = capped ? -n : n;
 }
 
@@ -148,36 +155,41 @@ struct LpLaneTab {
     __device__ __forceinline__ double R(int i) const { return IN_REGS ? rR[i] : pR[i]; }
 };
 
-// Phase 2 for one row held as M bins per lane over G lanes.  Donor-cell upwind:
+// Phase 2 for one row held as M bins per lane over G lanes (32/G rows per warp at once).
+// Donor-cell upwind:
 //   chi_i <- chi_i - c_i (F_{i+1} - F_i),  F_k = max(w_k,0) chi_{k-1} + min(w_k,0) chi_k,  chi_{-1} = chi_{Nb} = 0,
 // with c_i = dts/dE_i.  The coefficients do not change over the substeps, so the update is applied as
 // the tridiagonal form it is,
 //   chi_i <- D_i chi_i + L_i chi_{i-1} + U_i chi_{i+1},
 //   L_i = c_i max(w_i,0),  U_i = -c_i min(w_{i+1},0),  D_i = 1 + c_i (min(w_i,0) - max(w_{i+1},0)),
-// three fp64 operations per bin and substep, no selects in the loop.  The zero ghost bins are folded
-// in by L = 0 on the first bin of the row and U = 0 on the last.
-template <int M, int G, bool DIAG, class Tab>
-__device__ __forceinline__ void lp_row_substeps(double (&chi)[M], const Tab &tab, const LpCoef &c, int nloop,
-                                                int sub, double &lost)
-{
-    double D[M], L[M], U[M];
-    double w_first, w_last;
+// three fp64 operations per bin and substep, no selects in the loop.  With W_k = (dts/2) w_k
+// = -E_k (a2 + cr2 E_k):  2 max(W,0) = W + |W| and 2 min(W,0) = W - |W| exactly, so
+//   L_i = (W_i + |W_i|)/dE_i,  U_i = -(W_{i+1} - |W_{i+1}|)/dE_i,  D_i = 1 + ((W_i - |W_i|) - (W_{i+1} + |W_{i+1}|))/dE_i.
+// The zero ghost bins are folded in by L = 0 on the first bin of the row and U = 0 on the last.
+// nloop >= c.ns is the trip count shared by the rows a warp works on at once.
+template <int M, int G, bool DIAG>
+struct LpRow {
+    double chi[M], D[M], L[M], U[M];
+    double w_first, w_last, s0, s1;
+    int ns;
+
+    template <class Tab>
+    __device__ __forceinline__ void setup(const Tab &tab, double a2, double cr2, int ns_, int sub)
     {
-        // 2 max(w,0) = w + |w| and 2 min(w,0) = w - |w| are exact; the factor 1/2 goes into h = c_i/2
+        ns = ns_;
         const double e0 = tab.E(0);
-        double w = -e0 * fma(c.cr, e0, c.a);
+        double w = -e0 * fma(cr2, e0, a2);
         w_first = w;
         double p2 = w + fabs(w), n2 = w - fabs(w);
-        const double hdts = 0.5 * c.dts;
 #pragma unroll
         for (int i = 0; i < M; ++i) {
             const double e = tab.E(i + 1);
-            const double w1 = -e * fma(c.cr, e, c.a);
+            const double w1 = -e * fma(cr2, e, a2);
             const double p2n = w1 + fabs(w1), n2n = w1 - fabs(w1);
-            const double h = hdts * tab.R(i);
-            L[i] = h * p2;
-            U[i] = -h * n2n;
-            D[i] = fma(h, n2 - p2n, 1.0);
+            const double r = tab.R(i);
+            L[i] = r * p2;
+            U[i] = -r * n2n;
+            D[i] = fma(r, n2 - p2n, 1.0);
             p2 = p2n;
             n2 = n2n;
             w = w1;
@@ -185,49 +197,108 @@ __device__ __forceinline__ void lp_row_substeps(double (&chi)[M], const Tab &tab
         w_last = w;
         if (sub == 0) L[0] = 0.0;
         if (sub == G - 1) U[M - 1] = 0.0;
+        s0 = 0.0;
+        s1 = 0.0;
     }
-    double s0 = 0.0, s1 = 0.0;
-    constexpr bool kUniform = (G == 32);        // one row per warp: nloop == c.ns for every lane
-    for (int s = 0; s < nloop; ++s) {
+    // one substep, no test of ns (every lane of the warp calls)
+    __device__ __forceinline__ void advance()
+    {
         const double left = __shfl_up_sync(kFull, chi[M - 1], 1, G);
         const double right = __shfl_down_sync(kFull, chi[0], 1, G);
-        if (kUniform || s < c.ns) {
-            if (DIAG) { s0 += chi[0]; s1 += chi[M - 1]; }
-            double nx[M];
+        if (DIAG) { s0 += chi[0]; s1 += chi[M - 1]; }
+        double nx[M];
 #pragma unroll
-            for (int i = 0; i < M; ++i) {
-                const double lo = i == 0 ? left : chi[i - 1];
-                const double hi = i == M - 1 ? right : chi[i + 1];
-                nx[i] = fma(U[i], hi, fma(L[i], lo, D[i] * chi[i]));
+        for (int i = 0; i < M; ++i) {
+            const double lo = i == 0 ? left : chi[i - 1];
+            const double hi = i == M - 1 ? right : chi[i + 1];
+            nx[i] = fma(U[i], hi, fma(L[i], lo, D[i] * chi[i]));
+        }
+#pragma unroll
+        for (int i = 0; i < M; ++i) chi[i] = nx[i];
+    }
+    // substep number s (the row takes part while s < ns)
+    __device__ __forceinline__ void step(int s)
+    {
+        constexpr bool kUniform = (G == 32);        // one row per warp: ns is the same on every lane
+        if (kUniform) {
+            if (s < ns) advance();
+        } else {
+            const double left = __shfl_up_sync(kFull, chi[M - 1], 1, G);
+            const double right = __shfl_down_sync(kFull, chi[0], 1, G);
+            if (s < ns) {
+                if (DIAG) { s0 += chi[0]; s1 += chi[M - 1]; }
+                double nx[M];
+#pragma unroll
+                for (int i = 0; i < M; ++i) {
+                    const double lo = i == 0 ? left : chi[i - 1];
+                    const double hi = i == M - 1 ? right : chi[i + 1];
+                    nx[i] = fma(U[i], hi, fma(L[i], lo, D[i] * chi[i]));
+                }
+#pragma unroll
+                for (int i = 0; i < M; ++i) chi[i] = nx[i];
             }
-#pragma unroll
-            for (int i = 0; i < M; ++i) chi[i] = nx[i];
         }
     }
-    if (DIAG) {
-        double t1 = (sub == G - 1) ? fmax(w_last, 0.0) * s1 : 0.0;
-        double t0 = (sub == 0) ? fmin(w_first, 0.0) * s0 : 0.0;
+    // lost = dts (max(w_Nb,0) sum chi_{Nb-1} - min(w_0,0) sum chi_0),  dts w = 2 W   (all lanes call)
+    __device__ __forceinline__ double lost(int sub) const
+    {
+        double t1 = (sub == G - 1) ? (w_last + fabs(w_last)) * s1 : 0.0;
+        double t0 = (sub == 0) ? (w_first - fabs(w_first)) * s0 : 0.0;
         t1 = __shfl_sync(kFull, t1, G - 1, G);
         t0 = __shfl_sync(kFull, t0, 0, G);
-        lost = c.dts * (t1 - t0);
+        return t1 - t0;
+    }
+};
+
+// RI independent rows advance together, so that their dependent fp64 chains and shuffles interleave
+// (a single row is a chain of ~60 cycles per substep).  nmax = largest n_sub among them (warp-wide).
+template <int RI, int M, int G, bool DIAG>
+__device__ __forceinline__ void lp_rows_substeps(LpRow<M, G, DIAG> (&row)[RI], int nmin, int nmax)
+{
+    // the first nmin substeps are common to every row (nmin = smallest n_sub, warp-wide): straight-line
+    // code over the RI rows, which the scheduler interleaves
+#pragma unroll 1
+    for (int s = 0; s < nmin; ++s) {
+#pragma unroll
+        for (int r = 0; r < RI; ++r) row[r].advance();
+    }
+#pragma unroll 1
+    for (int s = nmin; s < nmax; ++s) {
+#pragma unroll
+        for (int r = 0; r < RI; ++r) row[r].step(s);
     }
 }
 
+// Per-particle phase for one chunk of 32 particles: coefficients into the warp's shared arrays.
 template <int NB, bool FUSED>
 __device__ __forceinline__ void lp_chunk_phase1(const LpSpectralArgs &A, long long base, int lane,
-                                                const double *sE, const double *sR, LpCoef *slot)
+                                                const double *sE, const double *sR, double2 *sAC, int *sNS)
 {
     const long long p = base + lane;
     LpCoef c;
-    c.a = 0.0; c.cr = 0.0; c.dts = 0.0; c.ns = 0; c.pad = 0;
+    c.a2 = 0.0; c.cr2 = 0.0; c.ns = 0;
     if (p < A.np) {
         int nss;
+#ifdef LP_DEBUG_SKIP_PHASE1
+        c.a2 = 1.0e-3; c.cr2 = 1.0e-12; c.ns = 2; nss = 2;
+#else
         lp_phase1<NB, FUSED>(A, p, sE, sR, c, nss);
+#endif
         A.nsub_ws[p] = nss;
         if (A.nsub_user) A.nsub_user[p] = nss;
     }
-    slot[lane] = c;
+    sAC[lane] = make_double2(c.a2, c.cr2);
+    sNS[lane] = c.ns;
     __syncwarp();
+}
+
+// max of n over the 32/G row groups of a warp (lanes with equal lane % G)
+template <int G>
+__device__ __forceinline__ int lp_group_max(int n)
+{
+#pragma unroll
+    for (int o = G; o < 32; o <<= 1) n = max(n, __shfl_xor_sync(kFull, n, o));
+    return n;
 }
 
 // ------------------------------------------------------------------ direct mover (N_b >= 256)
@@ -238,24 +309,23 @@ constexpr int kDirectWarps = kDirectThreads / 32;
 template <int NB, bool DIAG, bool FUSED>
 __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSpectralArgs A)
 {
-    constexpr int G = NB >= 32 ? 32 : NB;     // lanes that share one row
+    static_assert(NB >= 32, "one row per warp");
+    constexpr int G = 32;                     // lanes that share one row
     constexpr int M = NB / G;                 // bins per lane (contiguous)
-    constexpr int PPW = 32 / G;               // rows a warp works on at once
-    constexpr int ROWS = 32 / PPW;            // row iterations per chunk of 32 particles
     constexpr int U = (M <= 2) ? 4 : (M == 4 ? 2 : 1);   // rows in flight per warp
 
     __shared__ __align__(16) double sE[NB + 2];
     __shared__ __align__(16) double sR[NB];
-    __shared__ LpCoef sC[kDirectWarps][32];
+    __shared__ double2 sAC[kDirectWarps][32];
+    __shared__ int sNS[kDirectWarps][32];
 
     for (int i = threadIdx.x; i <= NB; i += kDirectThreads) sE[i] = A.tab[i];
     for (int i = threadIdx.x; i < NB; i += kDirectThreads) sR[i] = A.tab[(NB + 1) + NB + i];
     __syncthreads();
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int sub = lane % G, grp = lane / G;
     LpLaneTab<M, (M <= 4)> tab;
-    tab.init(sE, sR, sub);
+    tab.init(sE, sR, lane);
 
     const long long nchunks = (A.np + 31) >> 5;
     const long long gw = (long long)blockIdx.x * kDirectWarps + warp;
@@ -263,30 +333,39 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
 
     for (long long chunk = gw; chunk < nchunks; chunk += nw) {
         const long long base = chunk << 5;
-        lp_chunk_phase1<NB, FUSED>(A, base, lane, sE, sR, sC[warp]);
-        for (int j0 = 0; j0 < ROWS; j0 += U) {
+        lp_chunk_phase1<NB, FUSED>(A, base, lane, sE, sR, sAC[warp], sNS[warp]);
+        for (int j0 = 0; j0 < 32; j0 += U) {
             double buf[U][M];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const long long pj = base + (j0 + u) * PPW + grp;
-                if (pj < A.np) lp_load_row<M>(A.chi_in + pj * NB + sub * M, buf[u]);
+                const long long pj = base + j0 + u;
+                if (pj < A.np) lp_load_row<M>(A.chi_in + pj * NB + lane * M, buf[u]);
                 else {
 #pragma unroll
                     for (int i = 0; i < M; ++i) buf[u][i] = 0.0;
                 }
             }
+            LpRow<M, G, DIAG> row[U];
+            int nmax = 0, nmin = 0x7fffffff;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int r = (j0 + u) * PPW + grp;
-                const long long pj = base + r;
-                const LpCoef c = sC[warp][r];
-                int nloop = c.ns;
-                if (PPW > 1) nloop = max(nloop, __shfl_xor_sync(kFull, nloop, 16));
-                double lost = 0.0;
-                lp_row_substeps<M, G, DIAG>(buf[u], tab, c, nloop, sub, lost);
+                const int r = j0 + u;
+                const double2 ac = sAC[warp][r];
+                const int ns = sNS[warp][r];
+#pragma unroll
+                for (int i = 0; i < M; ++i) row[u].chi[i] = buf[u][i];
+                row[u].setup(tab, ac.x, ac.y, ns, lane);
+                nmax = max(nmax, ns);
+                nmin = min(nmin, ns);
+            }
+            lp_rows_substeps<U, M, G, DIAG>(row, nmin, nmax);
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const long long pj = base + j0 + u;
+                const double lost = DIAG ? row[u].lost(lane) : 0.0;
                 if (pj < A.np) {
-                    lp_store_row<M>(A.chi_out + pj * NB + sub * M, buf[u]);
-                    if (DIAG && sub == 0) {
+                    lp_store_row<M>(A.chi_out + pj * NB + lane * M, row[u].chi);
+                    if (DIAG && lane == 0) {
                         A.lost_ws[pj] = lost;
                         if (A.lost_user) A.lost_user[pj] = lost;
                     }
@@ -309,14 +388,26 @@ __device__ __forceinline__ void lp_mbar_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void lp_mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// Blocking wait for the phase with the given parity.  try_wait suspends the thread in hardware for
+// up to the hinted time, so a waiting warp does not take issue slots from the working ones.
+#ifndef LP_MBAR_SUSPEND_NS
+#define LP_MBAR_SUSPEND_NS 2000
+#endif
 __device__ __forceinline__ void lp_mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t done;
     do {
         asm volatile("{\n\t.reg .pred p;\n\t"
-                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
                      "selp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+                     : "=r"(done) : "r"(bar), "r"(parity), "r"((uint32_t)LP_MBAR_SUSPEND_NS) : "memory");
+#ifdef LP_MBAR_SLEEP_NS
+        if (!done) __nanosleep(LP_MBAR_SLEEP_NS);
+#endif
     } while (!done);
 }
 // global -> shared, completion counted in bytes on an mbarrier (TMA engine, UBLKCP in SASS)
@@ -338,143 +429,224 @@ template <int N> __device__ __forceinline__ void lp_bulk_wait_read()
 __device__ __forceinline__ void lp_bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// Tunables of the bulk mover (overridable at compile time for sweeps; defaults = measured best).
+#ifndef LP_BULK_MINB
+#define LP_BULK_MINB 2          // resident blocks per SM the register allocation is bounded for
+#endif
+#ifndef LP_BULK_SLOT_SMALL
+#define LP_BULK_SLOT_SMALL 4096 // ring slot bytes for N_b <= 64
+#endif
+#ifndef LP_BULK_SLOT_LARGE
+#define LP_BULK_SLOT_LARGE 4096 // ring slot bytes for N_b = 128
+#endif
+#ifndef LP_BULK_DEPTH
+#define LP_BULK_DEPTH 3         // ring slots per row warp
+#endif
+#ifndef LP_BULK_NP
+#define LP_BULK_NP 4            // particle warps per block
+#endif
+#ifndef LP_BULK_NR
+#define LP_BULK_NR 4            // row warps per block
+#endif
+#ifndef LP_BULK_COEF_DEPTH
+#define LP_BULK_COEF_DEPTH 16   // chunks of coefficients in flight between the two kinds of warp
+#endif
+#ifndef LP_BULK_CARVEOUT
+#define LP_BULK_CARVEOUT cudaSharedmemCarveoutDefault
+#endif
+#ifndef LP_BULK_M
+#define LP_BULK_M 2             // bins per lane (at least N_b/32)
+#endif
+#ifndef LP_BULK_RI
+#define LP_BULK_RI 2            // rows a lane group advances together (ILP)
+#endif
+#ifndef LP_BULK_TAB_REGS
+#define LP_BULK_TAB_REGS 1      // per-lane bin table in registers (1) or re-read from shared memory (0)
+#endif
+
 template <int NB>
 struct LpBulkCfg {
-    static constexpr int G = NB >= 32 ? 32 : NB;
-    static constexpr int M = NB / G;
-    static constexpr int PPW = 32 / G;
+    static constexpr int M = (NB / 32 > LP_BULK_M) ? NB / 32 : LP_BULK_M;   // bins per lane
+    static constexpr int G = NB / M;                              // lanes per row
+    static constexpr int PPW = 32 / G;                            // rows a warp works on at once
     static constexpr int ROW_BYTES = NB * 8;
-    static constexpr int SLOT_BYTES = NB <= 64 ? 2048 : 4096;     // one ring slot
-    static constexpr int R = SLOT_BYTES / ROW_BYTES;              // rows per slot: 16, 8, 4, 4
+    static constexpr int SLOT_BYTES = NB <= 64 ? LP_BULK_SLOT_SMALL : LP_BULK_SLOT_LARGE;     // one ring slot
+    static constexpr int R = SLOT_BYTES / ROW_BYTES;              // rows per slot
     static constexpr int GPC = 32 / R;                            // slots ("groups") per chunk of 32 rows
-    static constexpr int S = 3;                                   // ring depth per warp
-    static constexpr int WARPS = 4;                               // warps per block
-    static constexpr int THREADS = WARPS * 32;
-    static constexpr size_t SMEM_RING = (size_t)WARPS * S * SLOT_BYTES;
+    static constexpr int S = LP_BULK_DEPTH;                       // ring depth per row warp
+    static constexpr int NP = LP_BULK_NP, NR = LP_BULK_NR;        // particle warps, row warps
+    static constexpr int D = LP_BULK_COEF_DEPTH;                  // coefficient ring, in chunks
+    static constexpr int THREADS = (NP + NR) * 32;
+    static constexpr size_t SMEM_RING = (size_t)NR * S * SLOT_BYTES;
     static constexpr size_t SMEM_TAB = ((size_t)(2 * NB + 2) * 8 + 127) / 128 * 128;
-    static constexpr size_t SMEM_COEF = (size_t)WARPS * 32 * sizeof(LpCoef);
-    static constexpr size_t SMEM_BAR = 128;
+    static constexpr size_t SMEM_COEF = (size_t)D * 32 * (sizeof(double2) + sizeof(int));
+    static constexpr size_t SMEM_BAR = ((size_t)(NR * S + 2 * D) * 8 + 127) / 128 * 128;
     static constexpr size_t SMEM_TOTAL = SMEM_RING + SMEM_TAB + SMEM_COEF + SMEM_BAR + 128;
-    static_assert(R % PPW == 0 && GPC >= 1 && WARPS * S * 8 <= (int)SMEM_BAR, "ring geometry");
+    static constexpr int RI_WANT = (LP_BULK_RI * PPW <= R) ? LP_BULK_RI : R / PPW;
+    static constexpr int RI = RI_WANT < 1 ? 1 : RI_WANT;          // rows (per lane group) advanced together
+    static_assert(NB % M == 0 && G <= 32 && R % (PPW * RI) == 0 && GPC >= 1 && (GPC & (GPC - 1)) == 0 &&
+                  D >= 2 && NP >= 1 && NR >= 1, "ring geometry");
 };
 
+// Warp-specialised fused kernel.  A block owns the chunks (32 particles each) blockIdx.x + t*gridDim.x,
+// t = 0, 1, ...  Two kinds of warp work on them at their own pace:
+//  * particle warps (NP per block, one thread per particle): chunk t goes to particle warp t % NP, which
+//    runs phase 1 (push stages when FUSED, gathers, coefficients, n_sub) and leaves (a2, cr2, n_sub) in slot
+//    t % D of a shared coefficient ring.  Their time is spent waiting on dependent gathers.
+//  * row warps (NR per block): chunk t goes to row warp t % NR, which streams the chunk's rows through its
+//    private TMA ring (addresses do not depend on phase 1, so loads run ahead freely), waits for the
+//    chunk's coefficients, applies the substeps and stores the rows.
+// full[slot] / empty[slot] mbarriers (one arrival each) hand the coefficient slots back and forth.
+// Row indices are 32-bit inside the kernel (lp_create limits np to 2^32 - 1); only addresses are 64-bit.
 template <int NB, bool DIAG, bool FUSED>
-__global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS) lp_spectral_bulk_kernel(LpSpectralArgs A)
+__global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spectral_bulk_kernel(LpSpectralArgs A)
 {
     using C = LpBulkCfg<NB>;
-    constexpr int G = C::G, M = C::M, PPW = C::PPW, R = C::R, GPC = C::GPC, S = C::S;
+    constexpr int G = C::G, M = C::M, PPW = C::PPW, R = C::R, GPC = C::GPC, S = C::S, RI = C::RI;
+    constexpr int NP = C::NP, NR = C::NR, D = C::D;
 
     extern __shared__ __align__(128) unsigned char lp_smem_raw[];
     unsigned char *sm = lp_smem_raw;            // (no pointer casts: keeps the shared address space)
-    unsigned char *ring = sm;
     double *sE = reinterpret_cast<double *>(sm + C::SMEM_RING);
     double *sR = sE + (NB + 2);
-    LpCoef *sC = reinterpret_cast<LpCoef *>(sm + C::SMEM_RING + C::SMEM_TAB);
+    double2 *sAC = reinterpret_cast<double2 *>(sm + C::SMEM_RING + C::SMEM_TAB);
+    int *sNS = reinterpret_cast<int *>(sAC + D * 32);
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(sm + C::SMEM_RING + C::SMEM_TAB + C::SMEM_COEF);
+    // bars: [NR*S] ring slots | [D] coefficient slot full | [D] coefficient slot empty
 
     for (int i = threadIdx.x; i <= NB; i += C::THREADS) sE[i] = A.tab[i];
     for (int i = threadIdx.x; i < NB; i += C::THREADS) sR[i] = A.tab[(NB + 1) + NB + i];
-
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int sub = lane % G, grp = lane / G;
-    unsigned char *my_ring = ring + (size_t)warp * S * C::SLOT_BYTES;
-    const uint32_t ring_u32 = lp_smem_u32(my_ring);
-    const uint32_t bar_u32 = lp_smem_u32(bars + warp * S);
-    LpCoef *my_coef = sC + warp * 32;
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < S; ++s) lp_mbar_init(bar_u32 + 8 * s, 1);
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NR * S + 2 * D; ++i) lp_mbar_init(lp_smem_u32(bars + i), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         lp_fence_async_smem();
     }
     __syncthreads();
 
-    LpLaneTab<M, true> tab;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t full_u32 = lp_smem_u32(bars + NR * S);
+    const uint32_t empty_u32 = full_u32 + 8 * D;
+    const uint32_t np = (uint32_t)A.np;
+    const uint32_t nchunks = (uint32_t)((A.np + 31) >> 5);
+    const uint32_t nblk = blockIdx.x < nchunks ? (nchunks - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+
+    if (warp < NP) {
+        // ---------------------------------------------------------------- particle warp
+#pragma unroll 1
+        for (uint32_t t = warp; t < nblk; t += NP) {
+            const uint32_t cs = t % D, use = t / D;
+            if (use >= 1) lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u);
+            const uint32_t base = (blockIdx.x + t * gridDim.x) << 5;
+            lp_chunk_phase1<NB, FUSED>(A, (long long)base, lane, sE, sR, sAC + cs * 32, sNS + cs * 32);
+            if (lane == 0) lp_mbar_arrive(full_u32 + 8 * cs);      // (lp_chunk_phase1 ends with __syncwarp)
+        }
+        return;
+    }
+
+    // -------------------------------------------------------------------- row warp
+    const int rw = warp - NP;
+    const int sub = lane % G, grp = lane / G;
+    unsigned char *my_ring = sm + (size_t)rw * S * C::SLOT_BYTES;
+    const uint32_t ring_u32 = lp_smem_u32(my_ring);
+    const uint32_t bar_u32 = lp_smem_u32(bars + rw * S);
+    LpLaneTab<M, (LP_BULK_TAB_REGS != 0)> tab;
     tab.init(sE, sR, sub);
 
-    // this warp's chunks: gw, gw + nw, ...; its slots ("groups") are numbered q = 0 .. ngroups-1
-    const long long nchunks = (A.np + 31) >> 5;
-    const long long gw = (long long)blockIdx.x * C::WARPS + warp;
-    const long long nw = (long long)gridDim.x * C::WARPS;
-    const long long nmy = gw < nchunks ? (nchunks - gw + nw - 1) / nw : 0;
-    const long long ngroups = nmy * GPC;
+    // this warp's chunks: t = rw, rw + NR, ... (nmy of them); its ring slots ("groups") are numbered
+    // j = 0 .. ngroups-1, group j = rows [R * (j % GPC), +R) of its chunk number j / GPC
+    const uint32_t nmy = (uint32_t)rw < nblk ? (nblk - rw + NR - 1) / NR : 0;
+    const uint32_t ngroups = nmy * GPC;
 
-    auto rows_at = [&](long long row0) -> int {
-        const long long left = A.np - row0;
-        return left >= R ? R : (left > 0 ? (int)left : 0);
-    };
-    // loader state (lane 0): next group to load = (chunk base lbase, group lgi) into slot lslot
-    long long lbase = gw << 5, lq = 0;
-    int lgi = 0, lslot = 0;
-    auto issue_next_load = [&]() {              // lane 0 only; advances the loader state
-        if (lq < ngroups) {
-            const long long row0 = lbase + (long long)lgi * R;
-            const int nrows = rows_at(row0);
-            if (nrows > 0) {
-                const uint32_t bytes = (uint32_t)nrows * C::ROW_BYTES;
-                lp_mbar_expect_tx(bar_u32 + 8 * lslot, bytes);
-                lp_bulk_load(ring_u32 + lslot * C::SLOT_BYTES, A.chi_in + row0 * NB, bytes, bar_u32 + 8 * lslot);
-            }
-            ++lq;
-            if (++lgi == GPC) { lgi = 0; lbase += nw << 5; }
-            if (++lslot == S) lslot = 0;
+    auto chunk_base = [&](uint32_t k) -> uint32_t { return (blockIdx.x + (rw + k * NR) * gridDim.x) << 5; };
+    auto issue_load = [&](uint32_t j, int slot) {        // lane 0 only
+        const uint32_t row0 = chunk_base(j / GPC) + (j % GPC) * R;
+        if (row0 < np) {
+            const uint32_t left = np - row0;
+            const uint32_t bytes = (left < (uint32_t)R ? left : (uint32_t)R) * C::ROW_BYTES;
+            lp_mbar_expect_tx(bar_u32 + 8 * slot, bytes);
+            lp_bulk_load(ring_u32 + slot * C::SLOT_BYTES, A.chi_in + (size_t)row0 * NB, bytes, bar_u32 + 8 * slot);
         }
     };
     if (lane == 0) {
 #pragma unroll
-        for (int k = 0; k < S; ++k) issue_next_load();
+        for (int k = 0; k < S; ++k)
+            if ((uint32_t)k < ngroups) issue_load(k, k);
     }
 
-    long long base = gw << 5;
-    int gi = 0, slot = 0;
+    uint32_t q = 0;                 // group being consumed
+    int slot = 0, pslot = 0;
     uint32_t parity = 0;
-    for (long long q = 0; q < ngroups; ++q) {
-        if (gi == 0)        // a new chunk of 32 particles: per-particle phase while the rows fly in
-            lp_chunk_phase1<NB, FUSED>(A, base, lane, sE, sR, my_coef);
-        const long long row0 = base + (long long)gi * R;
-        const int nrows = rows_at(row0);
-        if (nrows > 0) {
-            lp_mbar_wait(bar_u32 + 8 * slot, parity);
-            double *srow = reinterpret_cast<double *>(my_ring + (size_t)slot * C::SLOT_BYTES);
-            const LpCoef *cf = my_coef + gi * R;
-#pragma unroll 2
-            for (int j = 0; j < R; j += PPW) {
-                const int rg = j + grp;                 // row within the slot
-                const bool valid = rg < nrows;
-                const LpCoef c = cf[rg];
-                double chi[M];
-                double *rp = srow + rg * NB + sub * M;
-                if (valid) lp_load_row<M>(rp, chi);
-                else {
+#pragma unroll 1
+    for (uint32_t k = 0; k < nmy; ++k) {
+        const uint32_t t = rw + k * NR;
+        const uint32_t cs = t % D, use = t / D;
+        const uint32_t base = chunk_base(k);
+        const int nchunk = (int)(np - base < 32u ? np - base : 32u);      // rows of this chunk
+        lp_mbar_wait(full_u32 + 8 * cs, use & 1u);                         // the chunk's coefficients
+        const double2 *my_ac = sAC + cs * 32;
+        const int *my_ns = sNS + cs * 32;
+#pragma unroll 1
+        for (int gi = 0; gi < GPC; ++gi, ++q) {
+            const int nrows = min(nchunk - gi * R, R);                    // rows of this group (<= 0: none)
+#ifndef LP_DEBUG_SKIP_ROWS
+            if (nrows > 0) {
+                lp_mbar_wait(bar_u32 + 8 * slot, parity);
+                double *srow = reinterpret_cast<double *>(my_ring + (size_t)slot * C::SLOT_BYTES);
+#pragma unroll 1
+                for (int j = 0; j < R; j += PPW * RI) {
+                    LpRow<M, G, DIAG> row[RI];
+                    int nmax = 0, nmin = 0x7fffffff;
 #pragma unroll
-                    for (int i = 0; i < M; ++i) chi[i] = 0.0;
-                }
-                int nloop = valid ? c.ns : 0;
-                if (PPW > 1) nloop = max(nloop, __shfl_xor_sync(kFull, nloop, 16));
-                double lost = 0.0;
-                lp_row_substeps<M, G, DIAG>(chi, tab, c, nloop, sub, lost);
-                if (valid) {
-                    lp_store_row<M>(rp, chi);
-                    if (DIAG && sub == 0) {
-                        A.lost_ws[row0 + rg] = lost;
-                        if (A.lost_user) A.lost_user[row0 + rg] = lost;
+                    for (int r = 0; r < RI; ++r) {
+                        const int rg = j + r * PPW + grp;           // row within the slot
+                        const bool valid = rg < nrows;
+                        const double2 ac = my_ac[gi * R + rg];
+                        const int ns = valid ? my_ns[gi * R + rg] : 0;
+                        const double *rp = srow + rg * NB + sub * M;
+                        if (valid) lp_load_row<M>(rp, row[r].chi);
+                        else {
+#pragma unroll
+                            for (int i = 0; i < M; ++i) row[r].chi[i] = 0.0;
+                        }
+                        row[r].setup(tab, ac.x, ac.y, ns, sub);
+                        nmax = max(nmax, ns);
+                        nmin = min(nmin, ns);
+                    }
+                    nmax = lp_group_max<G>(nmax);
+                    nmin = -lp_group_max<G>(-nmin);
+                    lp_rows_substeps<RI, M, G, DIAG>(row, nmin, nmax);
+#pragma unroll
+                    for (int r = 0; r < RI; ++r) {
+                        const int rg = j + r * PPW + grp;
+                        const double lost = DIAG ? row[r].lost(sub) : 0.0;
+                        if (rg < nrows) {
+                            lp_store_row<M>(srow + rg * NB + sub * M, row[r].chi);
+                            if (DIAG && sub == 0) {
+                                const size_t pj = (size_t)base + gi * R + rg;
+                                A.lost_ws[pj] = lost;
+                                if (A.lost_user) A.lost_user[pj] = lost;
+                            }
+                        }
                     }
                 }
+                lp_fence_async_smem();          // generic-proxy writes -> visible to the TMA store
+                __syncwarp();
+                if (lane == 0)
+                    lp_bulk_store(A.chi_out + ((size_t)base + gi * R) * NB, ring_u32 + slot * C::SLOT_BYTES,
+                                  (uint32_t)nrows * C::ROW_BYTES);
             }
-            lp_fence_async_smem();          // generic-proxy writes -> visible to the TMA store
-            __syncwarp();
-            if (lane == 0)
-                lp_bulk_store(A.chi_out + row0 * NB, ring_u32 + slot * C::SLOT_BYTES, (uint32_t)nrows * C::ROW_BYTES);
+            // refill the slot drained in the previous iteration (its store may still be reading: wait
+            // for all but the newest store group), keeping S-1 loads in flight
+            if (lane == 0 && q >= 1 && q + (S - 1) < ngroups) {
+                lp_bulk_wait_read<1>();
+                issue_load(q + (S - 1), pslot);
+            }
+#endif
+            pslot = slot;
+            if (++slot == S) { slot = 0; parity ^= 1u; }
         }
-        // refill the slot drained in the previous iteration (its store may still be reading: wait for
-        // all but the newest store group), keeping S-1 loads in flight
-        if (q >= 1 && lane == 0 && lq < ngroups) {
-            lp_bulk_wait_read<1>();
-            issue_next_load();
-        }
-        __syncwarp();
-        if (++gi == GPC) { gi = 0; base += nw << 5; }
-        if (++slot == S) { slot = 0; parity ^= 1u; }
+        __syncwarp();                                                     // every lane is done with the slot
+        if (lane == 0) lp_mbar_arrive(empty_u32 + 8 * cs);
     }
     if (lane == 0) lp_bulk_wait_all();
 }
@@ -498,9 +670,10 @@ int launch_variant(const LpSpectralArgs &a, int sm_count, cudaStream_t s)
         static bool configured = false;
         if (!configured) {
             if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_TOTAL) != cudaSuccess) return -1;
+            if (cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, LP_BULK_CARVEOUT) != cudaSuccess) return -1;
             configured = true;
         }
-        const long long want = (nchunks + C::WARPS - 1) / C::WARPS;
+        const long long want = nchunks;                      // a block takes whole chunks
         const long long cap = (long long)sm_count * lp_blocks_per_sm(kernel, C::THREADS, C::SMEM_TOTAL);
         int blocks = (int)(want < cap ? want : cap);
         if (blocks < 1) blocks = 1;
