@@ -106,7 +106,12 @@ LpLamCand make_candidates(const std::vector<double> &E, const std::vector<double
     std::memset(&c, 0, sizeof c);
     if ((int)v.size() > kLpMaxCand) { c.n = -1; return c; }
     c.n = (int)v.size();
-    for (int k = 0; k < c.n; ++k) c.bin[k] = v[k];
+    for (int k = 0; k < c.n; ++k) {
+        c.bin[k] = v[k];
+        c.el[k] = E[v[k]];
+        c.er[k] = E[v[k] + 1];
+        c.rde[k] = 1.0 / dE[v[k]];          // the same value as the device table's rdE
+    }
     return c;
 }
 

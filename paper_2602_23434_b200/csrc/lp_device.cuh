@@ -45,7 +45,7 @@ __device__ __forceinline__ uint32_t lp_cell_key(const LpGeom &g, double x, doubl
 // Trilinear stencil of a position: 8 cell indices and weights, corners ordered z outer, y, x inner;
 // weight = (wz*wy)*wx.  Cell-centred data: s = (x - lo)*inv_dx - 1/2, i0 = floor(s), f = s - i0.
 struct LpStencil {
-    long long c[8];
+    unsigned int c[8];          // cell index < 2^31 (lp_create rejects larger grids)
     double w[8];
 };
 
@@ -57,7 +57,8 @@ __device__ __forceinline__ void lp_axis(double x, double lo, double inv_dx, int 
     double f = __dsub_rn(s, fl);
     int b = (int)fl;
     i0 = lp_wrap(b, n, periodic);
-    i1 = lp_wrap(b + 1, n, periodic);
+    if (periodic) i1 = (i0 + 1 == n) ? 0 : i0 + 1;          // floor-mod of b + 1
+    else i1 = min(max(b + 1, 0), n - 1);
     w0 = __dsub_rn(1.0, f);
     w1 = f;
 }
@@ -77,7 +78,7 @@ __device__ __forceinline__ void lp_stencil(const LpGeom &g, double x, double y, 
             for (int cx = 0; cx < 2; ++cx) {
                 int n = (cz * 2 + cy) * 2 + cx;
                 st.w[n] = __dmul_rn(__dmul_rn(wz[cz], wy[cy]), wx[cx]);
-                st.c[n] = ((long long)kk[cz] * g.ny + jj[cy]) * g.nx + ii[cx];
+                st.c[n] = (unsigned int)((kk[cz] * g.ny + jj[cy]) * g.nx + ii[cx]);
             }
 }
 
@@ -100,7 +101,7 @@ __device__ __forceinline__ LpRec lp_ldg_rec(const double4 *p)
 // lanes whose stencil moved; values are the same bits either way.
 struct LpCornersA {
     LpRec r[8];
-    long long c0, c7;           // cells of corners 0 and 7 of the loaded stencil (they fix all eight)
+    unsigned int c0, c7;        // cells of corners 0 and 7 of the loaded stencil (they fix all eight)
     __device__ __forceinline__ void load(const LpCells &cells, const LpStencil &st)
     {
 #pragma unroll
@@ -153,19 +154,31 @@ __device__ __forceinline__ void lp_gather_v(const LpCells &cells, const LpStenci
     k.gather3(st, out);
 }
 
-// (bx, by, bz) from record B
+// (bx, by, bz) from record B, in two halves so that the loads can be issued ahead of other work
+struct LpCornersB {
+    LpRec r[8];
+    __device__ __forceinline__ void load(const LpCells &cells, const LpStencil &st)
+    {
+#pragma unroll
+        for (int n = 0; n < 8; ++n) r[n] = lp_ldg_rec(cells.recB + st.c[n]);
+    }
+    __device__ __forceinline__ void gather3(const LpStencil &st, double out[3]) const
+    {
+        out[0] = out[1] = out[2] = 0.0;
+#pragma unroll
+        for (int n = 0; n < 8; ++n) {
+            out[0] = lp_acc(out[0], st.w[n], r[n].a);
+            out[1] = lp_acc(out[1], st.w[n], r[n].b);
+            out[2] = lp_acc(out[2], st.w[n], r[n].c);
+        }
+    }
+};
+
 __device__ __forceinline__ void lp_gather_B(const LpCells &cells, const LpStencil &st, double out[3])
 {
-    LpRec r[8];
-#pragma unroll
-    for (int n = 0; n < 8; ++n) r[n] = lp_ldg_rec(cells.recB + st.c[n]);
-    out[0] = out[1] = out[2] = 0.0;
-#pragma unroll
-    for (int n = 0; n < 8; ++n) {
-        out[0] = lp_acc(out[0], st.w[n], r[n].a);
-        out[1] = lp_acc(out[1], st.w[n], r[n].b);
-        out[2] = lp_acc(out[2], st.w[n], r[n].c);
-    }
+    LpCornersB k;
+    k.load(cells, st);
+    k.gather3(st, out);
 }
 
 // periodic wrap into [lo, hi): x -= L*floor((x - lo)/L); a result >= hi becomes lo   (R15)

@@ -31,6 +31,7 @@ constexpr int kLpMaxCand = 24;
 struct LpLamCand {
     int n;
     int bin[kLpMaxCand];
+    double el[kLpMaxCand], er[kLpMaxCand], rde[kLpMaxCand];   // E_i, E_{i+1}, 1/dE_i of those bins
 };
 
 struct LpSpectralArgs {

@@ -42,12 +42,12 @@ __device__ __forceinline__ double lp_outflow(const double *sE, const double *sR,
 // Phase 1.  FUSED: the two push stages (same arithmetic as lp_push0/1_kernel)
 // run first on the same thread, so k1, x*, rho_old never leave registers.
 template <int NB, bool FUSED>
-__device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, const double *sE,
-                                          const double *sR, LpCoef &c, int &ns_signed)
+__device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, double px, double py, double pz,
+                                          const double *sE, const double *sR, LpCoef &c, int &ns_signed)
 {
     LpStencil st;
     LpCornersA ka;
-    double px = A.x[p], py = A.y[p], pz = A.z[p];
+    LpCornersB kb;
     double rho_old;
     double qa[4], qb[3];
     if (FUSED) {
@@ -81,7 +81,8 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
         ka.load(A.cells, st);
     }
     ka.gather4(st, qa);
-    lp_gather_B(A.cells, st, qb);
+    kb.load(A.cells, st);       // (issued after A is consumed: holding both record sets spills registers)
+    kb.gather3(st, qb);
     // gamma_g, dtau, c_r (Eq. 4), a (continuity)
     const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(qa[0], qa[0]), __dmul_rn(qa[1], qa[1])), __dmul_rn(qa[2], qa[2]));
     const double b2 = __dadd_rn(__dadd_rn(__dmul_rn(qb[0], qb[0]), __dmul_rn(qb[1], qb[1])), __dmul_rn(qb[2], qb[2]));
@@ -93,7 +94,12 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
     // lambda = max_i outflow_i: over the hull-vertex bins (see LpLamCand), or over all bins
     double lam = 0.0;
     if (A.cand.n >= 0) {
-        for (int k = 0; k < A.cand.n; ++k) lam = fmax(lam, lp_outflow(sE, sR, A.cand.bin[k], a, cr));
+        for (int k = 0; k < A.cand.n; ++k) {               // table values straight from the kernel parameters
+            const double el = A.cand.el[k], er = A.cand.er[k];
+            const double wl = -el * fma(cr, el, a);
+            const double wr = -er * fma(cr, er, a);
+            lam = fmax(lam, (fmax(wr, 0.0) - fmin(wl, 0.0)) * A.cand.rde[k]);
+        }
     } else {
         for (int i = 0; i < NB; ++i) lam = fmax(lam, lp_outflow(sE, sR, i, a, cr));
     }
@@ -272,6 +278,7 @@ __device__ __forceinline__ void lp_rows_substeps(LpRow<M, G, DIAG> (&row)[RI], i
 // Per-particle phase for one chunk of 32 particles: coefficients into the warp's shared arrays.
 template <int NB, bool FUSED>
 __device__ __forceinline__ void lp_chunk_phase1(const LpSpectralArgs &A, long long base, int lane,
+                                                double px, double py, double pz,
                                                 const double *sE, const double *sR, double2 *sAC, int *sNS)
 {
     const long long p = base + lane;
@@ -282,7 +289,7 @@ __device__ __forceinline__ void lp_chunk_phase1(const LpSpectralArgs &A, long lo
 #ifdef LP_DEBUG_SKIP_PHASE1
         c.a2 = 1.0e-3; c.cr2 = 1.0e-12; c.ns = 2; nss = 2;
 #else
-        lp_phase1<NB, FUSED>(A, p, sE, sR, c, nss);
+        lp_phase1<NB, FUSED>(A, p, px, py, pz, sE, sR, c, nss);
 #endif
         A.nsub_ws[p] = nss;
         if (A.nsub_user) A.nsub_user[p] = nss;
@@ -333,7 +340,10 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
 
     for (long long chunk = gw; chunk < nchunks; chunk += nw) {
         const long long base = chunk << 5;
-        lp_chunk_phase1<NB, FUSED>(A, base, lane, sE, sR, sAC[warp], sNS[warp]);
+        const bool have = base + lane < A.np;
+        const double px = have ? A.x[base + lane] : 0.0, py = have ? A.y[base + lane] : 0.0,
+                     pz = have ? A.z[base + lane] : 0.0;
+        lp_chunk_phase1<NB, FUSED>(A, base, lane, px, py, pz, sE, sR, sAC[warp], sNS[warp]);
         for (int j0 = 0; j0 < 32; j0 += U) {
             double buf[U][M];
 #pragma unroll
@@ -431,7 +441,7 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 
 // Tunables of the bulk mover (overridable at compile time for sweeps; defaults = measured best).
 #ifndef LP_BULK_MINB
-#define LP_BULK_MINB 2          // resident blocks per SM the register allocation is bounded for
+#define LP_BULK_MINB 1          // resident blocks per SM the register allocation is bounded for
 #endif
 #ifndef LP_BULK_SLOT_SMALL
 #define LP_BULK_SLOT_SMALL 4096 // ring slot bytes for N_b <= 64
@@ -443,22 +453,22 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #define LP_BULK_DEPTH 3         // ring slots per row warp
 #endif
 #ifndef LP_BULK_NP
-#define LP_BULK_NP 4            // particle warps per block
+#define LP_BULK_NP 8            // particle warps per block
 #endif
 #ifndef LP_BULK_NR
-#define LP_BULK_NR 4            // row warps per block
+#define LP_BULK_NR 8            // row warps per block
 #endif
 #ifndef LP_BULK_COEF_DEPTH
-#define LP_BULK_COEF_DEPTH 16   // chunks of coefficients in flight between the two kinds of warp
+#define LP_BULK_COEF_DEPTH 32   // chunks of coefficients in flight between the two kinds of warp
 #endif
 #ifndef LP_BULK_CARVEOUT
 #define LP_BULK_CARVEOUT cudaSharedmemCarveoutDefault
 #endif
 #ifndef LP_BULK_M
-#define LP_BULK_M 2             // bins per lane (at least N_b/32)
+#define LP_BULK_M 4             // bins per lane (at least N_b/32)
 #endif
 #ifndef LP_BULK_RI
-#define LP_BULK_RI 2            // rows a lane group advances together (ILP)
+#define LP_BULK_RI 1            // rows a lane group advances together (ILP)
 #endif
 #ifndef LP_BULK_TAB_REGS
 #define LP_BULK_TAB_REGS 1      // per-lane bin table in registers (1) or re-read from shared memory (0)
@@ -532,12 +542,24 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
 
     if (warp < NP) {
         // ---------------------------------------------------------------- particle warp
+        // positions are fetched one chunk ahead, so that their latency is off the dependent chain
+        auto chunk_of = [&](uint32_t t) -> uint32_t { return (blockIdx.x + t * gridDim.x) << 5; };
+        double nx = 0.0, ny = 0.0, nz = 0.0;
+        if ((uint32_t)warp < nblk && chunk_of(warp) + lane < np) {
+            const size_t p = (size_t)chunk_of(warp) + lane;
+            nx = A.x[p]; ny = A.y[p]; nz = A.z[p];
+        }
 #pragma unroll 1
         for (uint32_t t = warp; t < nblk; t += NP) {
             const uint32_t cs = t % D, use = t / D;
+            const uint32_t base = chunk_of(t);
+            const double px = nx, py = ny, pz = nz;
+            if (t + NP < nblk && chunk_of(t + NP) + lane < np) {
+                const size_t p = (size_t)chunk_of(t + NP) + lane;
+                nx = A.x[p]; ny = A.y[p]; nz = A.z[p];
+            }
             if (use >= 1) lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u);
-            const uint32_t base = (blockIdx.x + t * gridDim.x) << 5;
-            lp_chunk_phase1<NB, FUSED>(A, (long long)base, lane, sE, sR, sAC + cs * 32, sNS + cs * 32);
+            lp_chunk_phase1<NB, FUSED>(A, (long long)base, lane, px, py, pz, sE, sR, sAC + cs * 32, sNS + cs * 32);
             if (lane == 0) lp_mbar_arrive(full_u32 + 8 * cs);      // (lp_chunk_phase1 ends with __syncwarp)
         }
         return;
