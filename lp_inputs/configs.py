@@ -77,7 +77,7 @@ def workload(index: int) -> LPWorkload:
     if index == 3:
         return LPWorkload(3, WORKLOAD_NAMES[3], n=128, np=1 << 20, nbins=128, e_min=1.0, e_max=1e7,
                           periodic=(1, 1, 1), field_kind="turbulent", kmax=8, p_index=2.5,
-                          u_rad_frac=0.1, dt=0.0125, steps=50, seed=s)
+                          u_rad_frac=0.1, sort_every=50, dt=0.0125, steps=50, seed=s)
     if index == 4:
         return LPWorkload(4, WORKLOAD_NAMES[4], n=256, np=1 << 24, nbins=64, e_min=1.0, e_max=1e8,
                           periodic=(1, 1, 1), field_kind="turbulent", kmax=16, p_index=2.5,
@@ -85,5 +85,5 @@ def workload(index: int) -> LPWorkload:
     if index == 5:   # nbins is swept over 16..512 by the caller (scaled(nbins=...))
         return LPWorkload(5, WORKLOAD_NAMES[5], n=512, np=1 << 22, nbins=64, e_min=1.0, e_max=1e8,
                           periodic=(1, 1, 1), field_kind="turbulent", kmax=16, p_index=2.5,
-                          u_rad_frac=0.1, dt=0.003125, steps=10, seed=s)
+                          u_rad_frac=0.1, sort_every=10, dt=0.003125, steps=10, seed=s)
     raise ValueError("workload index must be 1..5")

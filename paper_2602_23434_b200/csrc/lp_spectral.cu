@@ -452,11 +452,22 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #ifndef LP_BULK_DEPTH
 #define LP_BULK_DEPTH 3         // ring slots per row warp
 #endif
-#ifndef LP_BULK_NP
-#define LP_BULK_NP 8            // particle warps per block
+#ifndef LP_BULK_WARPS
+#define LP_BULK_WARPS 16        // warps per block (one block per SM)
 #endif
-#ifndef LP_BULK_NR
-#define LP_BULK_NR 8            // row warps per block
+// particle warps per block by bin count (the rest are row warps): the per-particle phase costs the
+// same at every N_b, the row phase grows with N_b
+#ifndef LP_BULK_NP16
+#define LP_BULK_NP16 8
+#endif
+#ifndef LP_BULK_NP32
+#define LP_BULK_NP32 8
+#endif
+#ifndef LP_BULK_NP64
+#define LP_BULK_NP64 8
+#endif
+#ifndef LP_BULK_NP128
+#define LP_BULK_NP128 4
 #endif
 #ifndef LP_BULK_COEF_DEPTH
 #define LP_BULK_COEF_DEPTH 32   // chunks of coefficients in flight between the two kinds of warp
@@ -484,7 +495,8 @@ struct LpBulkCfg {
     static constexpr int R = SLOT_BYTES / ROW_BYTES;              // rows per slot
     static constexpr int GPC = 32 / R;                            // slots ("groups") per chunk of 32 rows
     static constexpr int S = LP_BULK_DEPTH;                       // ring depth per row warp
-    static constexpr int NP = LP_BULK_NP, NR = LP_BULK_NR;        // particle warps, row warps
+    static constexpr int NP = NB <= 16 ? LP_BULK_NP16 : NB == 32 ? LP_BULK_NP32 : NB == 64 ? LP_BULK_NP64 : LP_BULK_NP128;
+    static constexpr int NR = LP_BULK_WARPS - NP;                 // particle warps, row warps
     static constexpr int D = LP_BULK_COEF_DEPTH;                  // coefficient ring, in chunks
     static constexpr int THREADS = (NP + NR) * 32;
     static constexpr size_t SMEM_RING = (size_t)NR * S * SLOT_BYTES;

@@ -16,8 +16,8 @@ pytestmark = pytest.mark.gpu
 B = P.binding
 
 
-def small_turbulent(n=12, np_=1000 + 37, nbins=64, **kw):
-    return I.workload(3).scaled(n=n, np=np_, nbins=nbins, **kw)
+def small_turbulent(n=12, np_=1000 + 37, nbins=64, sort_every=0, **kw):
+    return I.workload(3).scaled(n=n, np=np_, nbins=nbins, sort_every=sort_every, **kw)
 
 
 def setup_pair(w, shuffle_ids=False, diag=True, jitter=True):
