@@ -132,6 +132,28 @@ def config_dict(w, n_gpus):
             "l2": "inputs larger than L2 (chi rows %.2f GB per GPU)" % (w.np * w.nbins * 8 / 1e9)}
 
 
+# ------------------------------------------------------------------------------- N > 1: replicas
+
+def rank_workload(w, rank):
+    """Every rank its own particle set (and grid): particles are independent, no exchange."""
+    return w.scaled(seed=w.seed + 7919 * rank) if rank else w
+
+
+def reduce_max(value, dist, device):
+    """Max over ranks of a device-timed duration (identity without a process group)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(world, particles_per_rank, steps, seconds_max):
+    """Whole-job particle-steps/s: the units all ranks processed over the slowest rank's time."""
+    return world * particles_per_rank * steps / seconds_max
+
+
 # ------------------------------------------------------------------------------- CPU oracle legs
 
 def oracle_state(w, fields_np, u_rad, x, y, z, pid, chi, nsel):
@@ -244,8 +266,7 @@ def run_ours(args):
     dev = torch.device("cuda", local)
 
     w = pick_workload(args)
-    if rank:
-        w = w.scaled(seed=w.seed + 7919 * rank)          # every rank its own particle set (and grid)
+    w = rank_workload(w, rank)
     dt = step_dt(w)
     fields, u_rad, x, y, z, pid, chi_host, chi_device = make_inputs(w, dev)
     lp = P.LP(P.config_from_workload(w, u_rad=u_rad, device=local))
@@ -278,11 +299,8 @@ def run_ours(args):
     spec_ms, spec_n = B.lp_timing_read(lp.ctx)
     B.lp_timing_enable(lp.ctx, 0)
     d = lp.diag()
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * w.np * args.steps / (ms * 1e-3)
+    ms = reduce_max(ms, dist, dev)
+    value = aggregate_rate(world, w.np, args.steps, ms * 1e-3)
 
     # ---- end to end through lp_step_host: pinned host buffers, H2D + D2H every step
     e2e = None
@@ -297,12 +315,9 @@ def run_ours(args):
             lp.step_host(dt, hx, hy, hz, hid, hchi)         # synchronises the stream itself
         torch.cuda.synchronize(dev)
         te = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([te], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            te = float(t.item())
+        te = reduce_max(te, dist, dev)
         nbytes = w.np * (8 * w.nbins + 32)
-        e2e = {"value": world * w.np * args.e2e_steps / te, "unit": UNIT, "h2d_bytes_per_step": nbytes,
+        e2e = {"value": aggregate_rate(world, w.np, args.e2e_steps, te), "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": args.e2e_steps,
                "api": "lp_step_host (pinned host x,y,z,id,chi in and out every step)"}
         del hx, hy, hz, hid, hchi
