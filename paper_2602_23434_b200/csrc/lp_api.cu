@@ -112,6 +112,12 @@ LpLamCand make_candidates(const std::vector<double> &E, const std::vector<double
         c.er[k] = E[v[k] + 1];
         c.rde[k] = 1.0 / dE[v[k]];          // the same value as the device table's rdE
     }
+    // On an exact log grid E_i/dE_i and E_{i+1}/dE_i do not depend on i, so the outflow rate is extremal
+    // in an end bin; the table's rounding (E to 1 ulp, dE = E_{i+1} - E_i with cancellation) perturbs those
+    // ratios by ~2^-53 E/dE.  64 times that, and never less than 1e-12.
+    double worst = 0.0;
+    for (int i = 0; i < nb; ++i) worst = std::max(worst, E[i + 1] / dE[i]);
+    c.margin = std::max(1.0e-12, 64.0 * 1.1102230246251565e-16 * worst);
     return c;
 }
 

@@ -32,6 +32,7 @@ struct LpLamCand {
     int n;
     int bin[kLpMaxCand];
     double el[kLpMaxCand], er[kLpMaxCand], rde[kLpMaxCand];   // E_i, E_{i+1}, 1/dE_i of those bins
+    double margin;      // relative bound on how far the maximum over all bins can exceed that of bins 0, N_b-1
 };
 
 struct LpSpectralArgs {

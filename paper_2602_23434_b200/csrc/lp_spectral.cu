@@ -7,14 +7,14 @@
 // (PAPER.md:96); the only cross-lane traffic per substep is one shuffle up and one shuffle down.
 //
 // Two kernels:
-//  * lp_spectral_bulk_kernel (N_b <= 128), warp-specialised: particle warps run phase 1 and hand the
+//  * lp_spectral_bulk_kernel (N_b <= 256), warp-specialised: particle warps run phase 1 and hand the
 //    coefficients through a shared-memory ring (mbarrier full/empty) to row warps, which stream the
 //    rows through private rings of shared-memory slots filled and drained by the TMA engine
 //    (cp.async.bulk + mbarrier).  Measured on B200: phase 1 is a chain of dependent gathers (latency)
 //    and phase 2 a stream (HBM); run by the same warp one after the other their times add, run by
 //    different warps they overlap.
-//  * lp_spectral_direct_kernel (N_b >= 256): rows go global -> registers -> global; these bin counts
-//    are bound by the fp64 pipe (n_sub ~ 5-10), not by HBM.
+//  * lp_spectral_direct_kernel (N_b = 512): rows go global -> registers -> global; this bin count
+//    is bound by the dependent fp64 chain of its ~10 substeps per row, not by HBM.
 // sm_100a.
 #include "lp_device.cuh"
 
@@ -91,19 +91,29 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
     const double cr = __dmul_rn(A.kappa, __dadd_rn(__dmul_rn(0.5, b2), A.u_rad));
     const double a = __ddiv_rn(-log(__ddiv_rn(qa[3], rho_old)), __dmul_rn(3.0, dtau));
 
-    // lambda = max_i outflow_i: over the hull-vertex bins (see LpLamCand), or over all bins
-    double lam = 0.0;
-    if (A.cand.n >= 0) {
-        for (int k = 0; k < A.cand.n; ++k) {               // table values straight from the kernel parameters
-            const double el = A.cand.el[k], er = A.cand.er[k];
-            const double wl = -el * fma(cr, el, a);
-            const double wr = -er * fma(cr, er, a);
-            lam = fmax(lam, (fmax(wr, 0.0) - fmin(wl, 0.0)) * A.cand.rde[k]);
+    // lambda = max_i outflow_i.  On the library's log-spaced table the maximum sits in the first or the
+    // last bin up to the rounding noise of E/dE (LpLamCand::margin, >= 1e-12), so those two bins decide n_sub
+    // unless dtau*lambda/C_E is within that margin of an integer; only then (practically never) are the other
+    // hull-vertex bins (see LpLamCand) evaluated too.  The result is the same integer either way.
+    auto cand_outflow = [&](int k) -> double {             // table values straight from the kernel parameters
+        const double el = A.cand.el[k], er = A.cand.er[k];
+        const double wl = -el * fma(cr, el, a);
+        const double wr = -er * fma(cr, er, a);
+        return (fmax(wr, 0.0) - fmin(wl, 0.0)) * A.cand.rde[k];
+    };
+    double lam = 0.0, q;
+    if (A.cand.n >= 2) {
+        lam = fmax(cand_outflow(0), cand_outflow(A.cand.n - 1));        // bins 0 and N_b - 1
+        q = __ddiv_rn(__dmul_rn(dtau, lam), A.cfl_e);
+        if (!(ceil(q * (1.0 + A.cand.margin)) == ceil(q))) {
+            for (int k = 1; k < A.cand.n - 1; ++k) lam = fmax(lam, cand_outflow(k));
+            q = __ddiv_rn(__dmul_rn(dtau, lam), A.cfl_e);
         }
     } else {
         for (int i = 0; i < NB; ++i) lam = fmax(lam, lp_outflow(sE, sR, i, a, cr));
+        q = __ddiv_rn(__dmul_rn(dtau, lam), A.cfl_e);
     }
-    const double need = ceil(__ddiv_rn(__dmul_rn(dtau, lam), A.cfl_e));
+    const double need = ceil(q);
     int n = !(need >= 1.0) ? 1 : (need > 2.0e9 ? 2000000000 : (int)need);
     const bool capped = n > A.max_substeps;
     if (capped) n = A.max_substeps;
@@ -446,8 +456,14 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #ifndef LP_BULK_SLOT_SMALL
 #define LP_BULK_SLOT_SMALL 4096 // ring slot bytes for N_b <= 64
 #endif
+#ifndef LP_BULK_MAX_NB
+#define LP_BULK_MAX_NB 256      // largest bin count the bulk kernel takes (above: direct kernel)
+#endif
 #ifndef LP_BULK_SLOT_LARGE
 #define LP_BULK_SLOT_LARGE 4096 // ring slot bytes for N_b = 128
+#endif
+#ifndef LP_BULK_SLOT_HUGE
+#define LP_BULK_SLOT_HUGE 4096  // ring slot bytes for N_b >= 256
 #endif
 #ifndef LP_BULK_DEPTH
 #define LP_BULK_DEPTH 3         // ring slots per row warp
@@ -465,6 +481,9 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #endif
 #ifndef LP_BULK_NP64
 #define LP_BULK_NP64 8
+#endif
+#ifndef LP_BULK_NP256
+#define LP_BULK_NP256 4
 #endif
 #ifndef LP_BULK_NP128
 #define LP_BULK_NP128 4
@@ -491,11 +510,11 @@ struct LpBulkCfg {
     static constexpr int G = NB / M;                              // lanes per row
     static constexpr int PPW = 32 / G;                            // rows a warp works on at once
     static constexpr int ROW_BYTES = NB * 8;
-    static constexpr int SLOT_BYTES = NB <= 64 ? LP_BULK_SLOT_SMALL : LP_BULK_SLOT_LARGE;     // one ring slot
+    static constexpr int SLOT_BYTES = NB <= 64 ? LP_BULK_SLOT_SMALL : NB <= 128 ? LP_BULK_SLOT_LARGE : LP_BULK_SLOT_HUGE;     // one ring slot
     static constexpr int R = SLOT_BYTES / ROW_BYTES;              // rows per slot
     static constexpr int GPC = 32 / R;                            // slots ("groups") per chunk of 32 rows
     static constexpr int S = LP_BULK_DEPTH;                       // ring depth per row warp
-    static constexpr int NP = NB <= 16 ? LP_BULK_NP16 : NB == 32 ? LP_BULK_NP32 : NB == 64 ? LP_BULK_NP64 : LP_BULK_NP128;
+    static constexpr int NP = NB <= 16 ? LP_BULK_NP16 : NB == 32 ? LP_BULK_NP32 : NB == 64 ? LP_BULK_NP64 : NB == 128 ? LP_BULK_NP128 : LP_BULK_NP256;
     static constexpr int NR = LP_BULK_WARPS - NP;                 // particle warps, row warps
     static constexpr int D = LP_BULK_COEF_DEPTH;                  // coefficient ring, in chunks
     static constexpr int THREADS = (NP + NR) * 32;
@@ -583,7 +602,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
     unsigned char *my_ring = sm + (size_t)rw * S * C::SLOT_BYTES;
     const uint32_t ring_u32 = lp_smem_u32(my_ring);
     const uint32_t bar_u32 = lp_smem_u32(bars + rw * S);
-    LpLaneTab<M, (LP_BULK_TAB_REGS != 0)> tab;
+    LpLaneTab<M, (LP_BULK_TAB_REGS != 0 && M <= 8)> tab;
     tab.init(sE, sR, sub);
 
     // this warp's chunks: t = rw, rw + NR, ... (nmy of them); its ring slots ("groups") are numbered
@@ -698,7 +717,7 @@ template <int NB, bool DIAG, bool FUSED>
 int launch_variant(const LpSpectralArgs &a, int sm_count, cudaStream_t s)
 {
     const long long nchunks = (a.np + 31) >> 5;
-    if constexpr (NB <= 128) {
+    if constexpr (NB <= LP_BULK_MAX_NB) {
         using C = LpBulkCfg<NB>;
         auto kernel = lp_spectral_bulk_kernel<NB, DIAG, FUSED>;
         static bool configured = false;
