@@ -318,7 +318,8 @@ def run_ours(args):
         te = reduce_max(te, dist, dev)
         nbytes = w.np * (8 * w.nbins + 32)
         e2e = {"value": aggregate_rate(world, w.np, args.e2e_steps, te), "unit": UNIT, "h2d_bytes_per_step": nbytes,
-               "d2h_bytes_per_step": nbytes, "steps": args.e2e_steps,
+               "d2h_bytes_per_step": nbytes - 8 * w.np,      # ids come back only on re-sort steps
+               "steps": args.e2e_steps,
                "api": "lp_step_host (pinned host x,y,z,id,chi in and out every step)"}
         del hx, hy, hz, hid, hchi
 

@@ -126,8 +126,11 @@ LP_API lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream);
  * spectral update (order of Table 1, without the fluid stages). */
 LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);
 
-/* The same step on HOST buffers (pinned or pageable): copies x,y,z,id,chi to the bound device
- * arrays, runs lp_step, copies them back and synchronises the stream. */
+/* The same step on HOST buffers (pinned for overlap; pageable works, serialised): copies x,y,z,id,chi
+ * to the bound device arrays, runs lp_step, copies x,y,z,chi (and id on re-sort steps) back and
+ * synchronises the stream.  With >= 65536 particles and no re-sort due, the step runs in 16 particle
+ * batches so that copy-in, kernels and copy-out overlap (particles are independent); the result is the
+ * same as lp_step's.  Work is ordered after what was enqueued on `stream` before the call. */
 LP_API lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *hz,
                        uint64_t *hid, double *hchi, void *stream);
 

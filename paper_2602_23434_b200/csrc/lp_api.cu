@@ -151,6 +151,9 @@ struct lp_ctx {
     std::vector<cudaEvent_t> ev;
     size_t ev_used = 0;
     bool timing = false;
+    // lp_step_host pipeline: copy-in and copy-out streams and their events (created on first use)
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    std::vector<cudaEvent_t> ev_pipe;
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
     LpCells cells() const { return LpCells{ at<const double4>(lay.recA), at<const double4>(lay.recB) }; }
@@ -227,7 +230,9 @@ LpPushArgs push_args(lp_ctx *c, double dt)
     return a;
 }
 
-lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cudaStream_t s)
+// p0, pcount: the particles [p0, p0 + pcount) only (pcount < 0: all)
+lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cudaStream_t s,
+                      long long p0 = 0, long long pcount = -1)
 {
     LpSpectralArgs a;
     a.g = c->geom;
@@ -244,6 +249,19 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
     a.lost_ws = c->at<double>(c->lay.lost);
     a.lost_user = c->lost_user;
     a.np = c->cfg.np;
+    if (pcount >= 0) {                  // a sub-range is the same launch on shifted arrays
+        const size_t nb = (size_t)c->cfg.nbins;
+        a.status += p0;
+        a.x += p0; a.y += p0; a.z += p0;
+        a.rho_old += p0;
+        a.chi_in += (size_t)p0 * nb;
+        a.chi_out += (size_t)p0 * nb;
+        a.nsub_ws += p0;
+        if (a.nsub_user) a.nsub_user += p0;
+        a.lost_ws += p0;
+        if (a.lost_user) a.lost_user += p0;
+        a.np = pcount;
+    }
     a.dt = dt;
     a.kappa = c->cfg.kappa;
     a.u_rad = c->cfg.u_rad;
@@ -348,6 +366,9 @@ lp_status lp_destroy(lp_ctx *ctx)
     if (!ctx) return LP_ERR_INVALID_ARG;
     if (ctx->tab) cudaFree(ctx->tab);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->ev_pipe) cudaEventDestroy(e);
+    if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
+    if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
     delete ctx;
     return LP_OK;
 }
@@ -498,21 +519,71 @@ lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *h
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t np = (size_t)ctx->cfg.np, nb = (size_t)ctx->cfg.nbins;
-    if (np) {
-        LP_CUDA(ctx, cudaMemcpyAsync(ctx->x, hx, np * 8, cudaMemcpyHostToDevice, s));
-        LP_CUDA(ctx, cudaMemcpyAsync(ctx->y, hy, np * 8, cudaMemcpyHostToDevice, s));
-        LP_CUDA(ctx, cudaMemcpyAsync(ctx->z, hz, np * 8, cudaMemcpyHostToDevice, s));
-        LP_CUDA(ctx, cudaMemcpyAsync(ctx->id, hid, np * 8, cudaMemcpyHostToDevice, s));
-        LP_CUDA(ctx, cudaMemcpyAsync(ctx->chi, hchi, np * nb * 8, cudaMemcpyHostToDevice, s));
+    const bool sort_now = ctx->cfg.sort_every > 0 && ctx->steps % ctx->cfg.sort_every == 0;
+    constexpr int kBatches = 16;
+    constexpr size_t kMinPipelined = (size_t)1 << 16;        // below this the copies are latency, not bandwidth
+    if (np < kMinPipelined || sort_now) {
+        // whole arrays in, one lp_step, whole arrays out (a re-sort needs every row on the device first)
+        if (np) {
+            LP_CUDA(ctx, cudaMemcpyAsync(ctx->x, hx, np * 8, cudaMemcpyHostToDevice, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(ctx->y, hy, np * 8, cudaMemcpyHostToDevice, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(ctx->z, hz, np * 8, cudaMemcpyHostToDevice, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(ctx->id, hid, np * 8, cudaMemcpyHostToDevice, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(ctx->chi, hchi, np * nb * 8, cudaMemcpyHostToDevice, s));
+        }
+        if ((st = lp_step(ctx, dt, stream)) != LP_OK) return st;
+        if (np) {
+            LP_CUDA(ctx, cudaMemcpyAsync(hx, ctx->x, np * 8, cudaMemcpyDeviceToHost, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(hy, ctx->y, np * 8, cudaMemcpyDeviceToHost, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(hz, ctx->z, np * 8, cudaMemcpyDeviceToHost, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(hid, ctx->id, np * 8, cudaMemcpyDeviceToHost, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(hchi, ctx->chi, np * nb * 8, cudaMemcpyDeviceToHost, s));
+        }
+        LP_CUDA(ctx, cudaStreamSynchronize(s));
+        return LP_OK;
     }
-    if ((st = lp_step(ctx, dt, stream)) != LP_OK) return st;
-    if (np) {
-        LP_CUDA(ctx, cudaMemcpyAsync(hx, ctx->x, np * 8, cudaMemcpyDeviceToHost, s));
-        LP_CUDA(ctx, cudaMemcpyAsync(hy, ctx->y, np * 8, cudaMemcpyDeviceToHost, s));
-        LP_CUDA(ctx, cudaMemcpyAsync(hz, ctx->z, np * 8, cudaMemcpyDeviceToHost, s));
-        LP_CUDA(ctx, cudaMemcpyAsync(hid, ctx->id, np * 8, cudaMemcpyDeviceToHost, s));
-        LP_CUDA(ctx, cudaMemcpyAsync(hchi, ctx->chi, np * nb * 8, cudaMemcpyDeviceToHost, s));
+
+    // Pipelined: particles are independent, so the step runs batch by batch while the rows of the next
+    // batch come in (copy-in stream) and those of the previous one go out (copy-out stream): the two
+    // PCIe directions and the kernels overlap.  Batch boundaries are multiples of 32 particles.
+    if (!ctx->s_in) {
+        LP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_in, cudaStreamNonBlocking));
+        LP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_out, cudaStreamNonBlocking));
+        for (int i = 0; i < 2 * kBatches + 2; ++i) {
+            cudaEvent_t e;
+            LP_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            ctx->ev_pipe.push_back(e);
+        }
     }
+    cudaEvent_t *ev_in = ctx->ev_pipe.data(), *ev_k = ev_in + kBatches;
+    cudaEvent_t ev_start = ctx->ev_pipe[2 * kBatches], ev_done = ctx->ev_pipe[2 * kBatches + 1];
+    const size_t per = ((np + kBatches - 1) / kBatches + 31) / 32 * 32;
+    LP_CUDA(ctx, cudaEventRecord(ev_start, s));                 // copies start after earlier work on s
+    LP_CUDA(ctx, cudaStreamWaitEvent(ctx->s_in, ev_start, 0));
+    LP_CUDA(ctx, cudaStreamWaitEvent(ctx->s_out, ev_start, 0));
+    LP_CUDA(ctx, cudaMemcpyAsync(ctx->x, hx, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    LP_CUDA(ctx, cudaMemcpyAsync(ctx->y, hy, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    LP_CUDA(ctx, cudaMemcpyAsync(ctx->z, hz, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    LP_CUDA(ctx, cudaMemcpyAsync(ctx->id, hid, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    ++ctx->steps;
+    for (int b = 0; b < kBatches; ++b) {
+        const size_t p0 = (size_t)b * per;
+        if (p0 >= np) break;
+        const size_t cnt = std::min(per, np - p0);
+        LP_CUDA(ctx, cudaMemcpyAsync(ctx->chi + p0 * nb, hchi + p0 * nb, cnt * nb * 8, cudaMemcpyHostToDevice, ctx->s_in));
+        LP_CUDA(ctx, cudaEventRecord(ev_in[b], ctx->s_in));
+        LP_CUDA(ctx, cudaStreamWaitEvent(s, ev_in[b], 0));
+        if ((st = do_spectral(ctx, dt, ctx->chi, true, s, (long long)p0, (long long)cnt)) != LP_OK) return st;
+        LP_CUDA(ctx, cudaEventRecord(ev_k[b], s));
+        LP_CUDA(ctx, cudaStreamWaitEvent(ctx->s_out, ev_k[b], 0));
+        LP_CUDA(ctx, cudaMemcpyAsync(hchi + p0 * nb, ctx->chi + p0 * nb, cnt * nb * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+    }
+    // positions are final once the last batch has run (s_out already waits for it); ids are unchanged
+    LP_CUDA(ctx, cudaMemcpyAsync(hx, ctx->x, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+    LP_CUDA(ctx, cudaMemcpyAsync(hy, ctx->y, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+    LP_CUDA(ctx, cudaMemcpyAsync(hz, ctx->z, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+    LP_CUDA(ctx, cudaEventRecord(ev_done, ctx->s_out));
+    LP_CUDA(ctx, cudaStreamWaitEvent(s, ev_done, 0));
     LP_CUDA(ctx, cudaStreamSynchronize(s));
     return LP_OK;
 }

@@ -192,16 +192,25 @@ def test_lp_step_with_resort_matches_oracle(nbins, np_):
     assert d["steps"] == 8 and d["sorts"] == 3
 
 
-def test_lp_step_host_roundtrip():
-    w = small_turbulent(np_=4000, nbins=32)
-    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+@pytest.mark.parametrize("np_,nbins,sort_every", [(4000, 32, 0), (70001, 16, 0), (66000, 64, 2)])
+def test_lp_step_host_roundtrip(np_, nbins, sort_every):
+    """lp_step on host buffers: whole-array path (small sets, re-sort steps) and the batched pipeline
+    (>= 65536 particles: copy-in, kernels and copy-out overlap) must both give the oracle's step."""
+    w = small_turbulent(np_=np_, nbins=nbins, sort_every=sort_every)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
     hx, hy, hz = (torch.from_numpy(a.copy()).pin_memory() for a in (x, y, z))
     hid = torch.from_numpy(pid.view(np.int64).copy()).pin_memory()
     hchi = torch.from_numpy(chi.copy()).pin_memory()
-    lp.step_host(w.dt, hx, hy, hz, hid, hchi)
-    x1, y1, z1, chi1, nsub, lost, st = orc.step(prm, f_np, x, y, z, w.dt, chi, nthreads=8)
-    assert np.array_equal(hx.numpy(), x1) and np.array_equal(hy.numpy(), y1)
-    assert_chi_close(hchi.numpy(), chi1)
+    for s in range(2):                                   # with sort_every = 2: a re-sort step, then a pipelined one
+        lp.step_host(w.dt, hx, hy, hz, hid, hchi)
+        if sort_every and s % sort_every == 0:
+            x, y, z, pid, chi, _, _ = oracle_sort_state(prm, x, y, z, pid, chi)
+        x, y, z, chi, nsub, lost, st = orc.step(prm, f_np, x, y, z, w.dt, chi, nthreads=8)
+    assert np.array_equal(hid.numpy().view(np.uint64), pid)
+    assert np.array_equal(hx.numpy(), x) and np.array_equal(hy.numpy(), y) and np.array_equal(hz.numpy(), z)
+    assert_chi_close(hchi.numpy(), chi)
+    assert_nsub_equal(host(lp.nsub), nsub)
+    assert lp.diag()["steps"] == 2
 
 
 # ------------------------------------------------------------------ edge cases and error paths
