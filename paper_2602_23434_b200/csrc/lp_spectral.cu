@@ -28,6 +28,7 @@ struct LpCoef {
     double a2;     // (dts/2) * a,    a = (1/3) div_mu u^mu,   dts = dtau / n_sub
     double cr2;    // (dts/2) * c_r
     int ns;        // n_sub (0 = no particle)
+    int cool;      // a + c_r E_0 >= 0: every edge velocity is <= 0 (LpRow::setup_cool)
 };
 
 // outflow rate of bin i:  (max(w_{i+1},0) - min(w_i,0)) / dE_i,   w_k = -E_k (a + c_r E_k)
@@ -121,6 +122,7 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
     c.a2 = hdts * a;
     c.cr2 = hdts * cr;
     c.ns = n;
+    c.cool = fma(c.cr2, sE[0], c.a2) >= 0.0;
     ns_signed = capped ? -n : n;
 }
 
@@ -216,6 +218,67 @@ struct LpRow {
         s0 = 0.0;
         s1 = 0.0;
     }
+    // Rows with a + c_r E_0 >= 0 ("cooling": every edge velocity w_k <= 0) have L = 0 identically, so they
+    // need neither L nor the value from the lower neighbour: U_i = -2 W_{i+1}/dE_i, D_i = 1 + 2 W_i/dE_i and
+    // chi_i <- D_i chi_i + U_i chi_{i+1}.  These are the same bits the general form gives for such a row
+    // (there W + |W| = 0 exactly and the L term adds a zero).
+    template <class Tab>
+    __device__ __forceinline__ void setup_cool(const Tab &tab, double a2, double cr2, int ns_, int sub)
+    {
+        ns = ns_;
+        const double e0 = tab.E(0);
+        double w = -e0 * fma(cr2, e0, a2);
+        w_first = w;
+        double n2 = w - fabs(w);
+#pragma unroll
+        for (int i = 0; i < M; ++i) {
+            const double e = tab.E(i + 1);
+            const double w1 = -e * fma(cr2, e, a2);
+            const double n2n = w1 - fabs(w1);
+            const double r = tab.R(i);
+            U[i] = -r * n2n;
+            D[i] = fma(r, n2, 1.0);
+            n2 = n2n;
+            w = w1;
+        }
+        w_last = w;
+        if (sub == G - 1) U[M - 1] = 0.0;
+        s0 = 0.0;
+        s1 = 0.0;
+    }
+    __device__ __forceinline__ void advance_cool()
+    {
+        const double right = __shfl_down_sync(kFull, chi[0], 1, G);
+        if (DIAG) { s0 += chi[0]; s1 += chi[M - 1]; }
+        double nx[M];
+#pragma unroll
+        for (int i = 0; i < M; ++i) {
+            const double hi = i == M - 1 ? right : chi[i + 1];
+            nx[i] = fma(U[i], hi, D[i] * chi[i]);
+        }
+#pragma unroll
+        for (int i = 0; i < M; ++i) chi[i] = nx[i];
+    }
+    __device__ __forceinline__ void step_cool(int s)
+    {
+        constexpr bool kUniform = (G == 32);
+        if (kUniform) {
+            if (s < ns) advance_cool();
+        } else {
+            const double right = __shfl_down_sync(kFull, chi[0], 1, G);
+            if (s < ns) {
+                if (DIAG) { s0 += chi[0]; s1 += chi[M - 1]; }
+                double nx[M];
+#pragma unroll
+                for (int i = 0; i < M; ++i) {
+                    const double hi = i == M - 1 ? right : chi[i + 1];
+                    nx[i] = fma(U[i], hi, D[i] * chi[i]);
+                }
+#pragma unroll
+                for (int i = 0; i < M; ++i) chi[i] = nx[i];
+            }
+        }
+    }
     // one substep, no test of ns (every lane of the warp calls)
     __device__ __forceinline__ void advance()
     {
@@ -268,7 +331,7 @@ struct LpRow {
 
 // RI independent rows advance together, so that their dependent fp64 chains and shuffles interleave
 // (a single row is a chain of ~60 cycles per substep).  nmax = largest n_sub among them (warp-wide).
-template <int RI, int M, int G, bool DIAG>
+template <bool COOL, int RI, int M, int G, bool DIAG>
 __device__ __forceinline__ void lp_rows_substeps(LpRow<M, G, DIAG> (&row)[RI], int nmin, int nmax)
 {
     // the first nmin substeps are common to every row (nmin = smallest n_sub, warp-wide): straight-line
@@ -276,12 +339,18 @@ __device__ __forceinline__ void lp_rows_substeps(LpRow<M, G, DIAG> (&row)[RI], i
 #pragma unroll 1
     for (int s = 0; s < nmin; ++s) {
 #pragma unroll
-        for (int r = 0; r < RI; ++r) row[r].advance();
+        for (int r = 0; r < RI; ++r) {
+            if (COOL) row[r].advance_cool();
+            else row[r].advance();
+        }
     }
 #pragma unroll 1
     for (int s = nmin; s < nmax; ++s) {
 #pragma unroll
-        for (int r = 0; r < RI; ++r) row[r].step(s);
+        for (int r = 0; r < RI; ++r) {
+            if (COOL) row[r].step_cool(s);
+            else row[r].step(s);
+        }
     }
 }
 
@@ -293,11 +362,11 @@ __device__ __forceinline__ void lp_chunk_phase1(const LpSpectralArgs &A, long lo
 {
     const long long p = base + lane;
     LpCoef c;
-    c.a2 = 0.0; c.cr2 = 0.0; c.ns = 0;
+    c.a2 = 0.0; c.cr2 = 0.0; c.ns = 0; c.cool = 1;
     if (p < A.np) {
         int nss;
 #ifdef LP_DEBUG_SKIP_PHASE1
-        c.a2 = 1.0e-3; c.cr2 = 1.0e-12; c.ns = 2; nss = 2;
+        c.a2 = 1.0e-3; c.cr2 = 1.0e-12; c.ns = 2; c.cool = 0; nss = 2;
 #else
         lp_phase1<NB, FUSED>(A, p, px, py, pz, sE, sR, c, nss);
 #endif
@@ -305,7 +374,7 @@ __device__ __forceinline__ void lp_chunk_phase1(const LpSpectralArgs &A, long lo
         if (A.nsub_user) A.nsub_user[p] = nss;
     }
     sAC[lane] = make_double2(c.a2, c.cr2);
-    sNS[lane] = c.ns;
+    sNS[lane] = c.cool ? -c.ns : c.ns;          // the sign carries the cooling flag to the row warps
     __syncwarp();
 }
 
@@ -371,14 +440,14 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
             for (int u = 0; u < U; ++u) {
                 const int r = j0 + u;
                 const double2 ac = sAC[warp][r];
-                const int ns = sNS[warp][r];
+                const int ns = abs(sNS[warp][r]);
 #pragma unroll
                 for (int i = 0; i < M; ++i) row[u].chi[i] = buf[u][i];
                 row[u].setup(tab, ac.x, ac.y, ns, lane);
                 nmax = max(nmax, ns);
                 nmin = min(nmin, ns);
             }
-            lp_rows_substeps<U, M, G, DIAG>(row, nmin, nmax);
+            lp_rows_substeps<false, U, M, G, DIAG>(row, nmin, nmax);
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const long long pj = base + j0 + u;
@@ -648,26 +717,38 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
 #pragma unroll 1
                 for (int j = 0; j < R; j += PPW * RI) {
                     LpRow<M, G, DIAG> row[RI];
+                    double2 ac[RI];
+                    int nsr[RI];
                     int nmax = 0, nmin = 0x7fffffff;
+                    bool cool = true;
 #pragma unroll
                     for (int r = 0; r < RI; ++r) {
                         const int rg = j + r * PPW + grp;           // row within the slot
                         const bool valid = rg < nrows;
-                        const double2 ac = my_ac[gi * R + rg];
-                        const int ns = valid ? my_ns[gi * R + rg] : 0;
+                        ac[r] = my_ac[gi * R + rg];
+                        const int nsv = valid ? my_ns[gi * R + rg] : 0;
+                        cool = cool && nsv <= 0;
+                        nsr[r] = abs(nsv);
                         const double *rp = srow + rg * NB + sub * M;
                         if (valid) lp_load_row<M>(rp, row[r].chi);
                         else {
 #pragma unroll
                             for (int i = 0; i < M; ++i) row[r].chi[i] = 0.0;
                         }
-                        row[r].setup(tab, ac.x, ac.y, ns, sub);
-                        nmax = max(nmax, ns);
-                        nmin = min(nmin, ns);
+                        nmax = max(nmax, nsr[r]);
+                        nmin = min(nmin, nsr[r]);
                     }
                     nmax = lp_group_max<G>(nmax);
                     nmin = -lp_group_max<G>(-nmin);
-                    lp_rows_substeps<RI, M, G, DIAG>(row, nmin, nmax);
+                    if (__all_sync(kFull, cool)) {                  // every row in flight is a cooling row
+#pragma unroll
+                        for (int r = 0; r < RI; ++r) row[r].setup_cool(tab, ac[r].x, ac[r].y, nsr[r], sub);
+                        lp_rows_substeps<true, RI, M, G, DIAG>(row, nmin, nmax);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < RI; ++r) row[r].setup(tab, ac[r].x, ac[r].y, nsr[r], sub);
+                        lp_rows_substeps<false, RI, M, G, DIAG>(row, nmin, nmax);
+                    }
 #pragma unroll
                     for (int r = 0; r < RI; ++r) {
                         const int rg = j + r * PPW + grp;
