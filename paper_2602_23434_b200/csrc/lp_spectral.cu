@@ -54,6 +54,11 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
     if (FUSED) {
         lp_stencil(A.g, px, py, pz, st);
         ka.load(A.cells, st);
+        // B is gathered last, at x^{n+1}, whose cells are these or their neighbours: start them on their way
+        // from DRAM to L2 now (the four x-lower corners; every prefetch is an L1 request, and eight cost more
+        // than they save)
+#pragma unroll
+        for (int n = 0; n < 8; n += 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.cells.recB + st.c[n]));
         ka.gather4(st, qa);                                 // k1 = v(x^n), rho_old = rho(x^n)
         rho_old = qa[3];
         lp_stencil(A.g, __dadd_rn(px, __dmul_rn(A.dt, qa[0])), __dadd_rn(py, __dmul_rn(A.dt, qa[1])),
