@@ -504,16 +504,34 @@ __device__ __forceinline__ void lp_mbar_wait(uint32_t bar, uint32_t parity)
 #endif
     } while (!done);
 }
-// global -> shared, completion counted in bytes on an mbarrier (TMA engine, UBLKCP in SASS)
-__device__ __forceinline__ void lp_bulk_load(uint32_t dst_smem, const void *src, uint32_t bytes, uint32_t bar)
+// L2 eviction policy for the row stream: rows are touched once per step, the grid records many times
+__device__ __forceinline__ uint64_t lp_policy_evict_first()
 {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// global -> shared, completion counted in bytes on an mbarrier (TMA engine, UBLKCP in SASS)
+__device__ __forceinline__ void lp_bulk_load(uint32_t dst_smem, const void *src, uint32_t bytes, uint32_t bar,
+                                             uint64_t pol)
+{
+#if LP_BULK_L2HINT
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(dst_smem), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+#else
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst_smem), "l"(src), "r"(bytes), "r"(bar) : "memory");
+#endif
 }
 // shared -> global, tracked by bulk async-groups
-__device__ __forceinline__ void lp_bulk_store(void *dst, uint32_t src_smem, uint32_t bytes)
+__device__ __forceinline__ void lp_bulk_store(void *dst, uint32_t src_smem, uint32_t bytes, uint64_t pol)
 {
+#if LP_BULK_L2HINT
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                 ::"l"(dst), "r"(src_smem), "r"(bytes), "l"(pol) : "memory");
+#else
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src_smem), "r"(bytes) : "memory");
+#endif
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
 template <int N> __device__ __forceinline__ void lp_bulk_wait_read()
@@ -561,6 +579,9 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #endif
 #ifndef LP_BULK_NP128
 #define LP_BULK_NP128 4
+#endif
+#ifndef LP_BULK_L2HINT
+#define LP_BULK_L2HINT 0        // 1: row loads and stores carry an L2 evict-first policy
 #endif
 #ifndef LP_BULK_COEF_DEPTH
 #define LP_BULK_COEF_DEPTH 32   // chunks of coefficients in flight between the two kinds of warp
@@ -684,6 +705,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
     const uint32_t nmy = (uint32_t)rw < nblk ? (nblk - rw + NR - 1) / NR : 0;
     const uint32_t ngroups = nmy * GPC;
 
+    const uint64_t pol = lp_policy_evict_first();
     auto chunk_base = [&](uint32_t k) -> uint32_t { return (blockIdx.x + (rw + k * NR) * gridDim.x) << 5; };
     auto issue_load = [&](uint32_t j, int slot) {        // lane 0 only
         const uint32_t row0 = chunk_base(j / GPC) + (j % GPC) * R;
@@ -691,7 +713,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
             const uint32_t left = np - row0;
             const uint32_t bytes = (left < (uint32_t)R ? left : (uint32_t)R) * C::ROW_BYTES;
             lp_mbar_expect_tx(bar_u32 + 8 * slot, bytes);
-            lp_bulk_load(ring_u32 + slot * C::SLOT_BYTES, A.chi_in + (size_t)row0 * NB, bytes, bar_u32 + 8 * slot);
+            lp_bulk_load(ring_u32 + slot * C::SLOT_BYTES, A.chi_in + (size_t)row0 * NB, bytes, bar_u32 + 8 * slot, pol);
         }
     };
     if (lane == 0) {
@@ -772,7 +794,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
                 __syncwarp();
                 if (lane == 0)
                     lp_bulk_store(A.chi_out + ((size_t)base + gi * R) * NB, ring_u32 + slot * C::SLOT_BYTES,
-                                  (uint32_t)nrows * C::ROW_BYTES);
+                                  (uint32_t)nrows * C::ROW_BYTES, pol);
             }
             // refill the slot drained in the previous iteration (its store may still be reading: wait
             // for all but the newest store group), keeping S-1 loads in flight
