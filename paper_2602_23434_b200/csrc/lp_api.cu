@@ -231,8 +231,9 @@ LpPushArgs push_args(lp_ctx *c, double dt)
 }
 
 // p0, pcount: the particles [p0, p0 + pcount) only (pcount < 0: all)
+// pos_in: [3][np] positions to read instead of the bound x, y, z (right after a re-sort), or NULL
 lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cudaStream_t s,
-                      long long p0 = 0, long long pcount = -1)
+                      long long p0 = 0, long long pcount = -1, const double *pos_in = nullptr)
 {
     LpSpectralArgs a;
     a.g = c->geom;
@@ -240,6 +241,9 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
     a.status = c->at<int32_t>(c->lay.status);
     a.cells = c->cells();
     a.x = c->x; a.y = c->y; a.z = c->z;
+    a.xin = pos_in ? pos_in : c->x;
+    a.yin = pos_in ? pos_in + c->cfg.np : c->y;
+    a.zin = pos_in ? pos_in + 2 * c->cfg.np : c->z;
     a.rho_old = c->at<double>(c->lay.rho_old);
     a.chi_in = chi_in;
     a.chi_out = c->chi;
@@ -253,6 +257,7 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
         const size_t nb = (size_t)c->cfg.nbins;
         a.status += p0;
         a.x += p0; a.y += p0; a.z += p0;
+        a.xin += p0; a.yin += p0; a.zin += p0;
         a.rho_old += p0;
         a.chi_in += (size_t)p0 * nb;
         a.chi_out += (size_t)p0 * nb;
@@ -279,9 +284,11 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
     return st;
 }
 
-// sort: permutation, then x,y,z,id through scratch and back; chi rows into chi_alt.
-// copy_chi_back = false leaves the permuted rows in chi_alt for the caller to consume.
-lp_status do_sort(lp_ctx *c, bool copy_chi_back, cudaStream_t s)
+// sort: permutation, then x, y, z, id through scratch; chi rows into chi_alt.
+// in_place = true (lp_sort): everything is copied back into the bound arrays.
+// in_place = false (lp_step): ids go back, the permuted positions stay in the x* scratch and the permuted
+// rows in chi_alt for the fused kernel to read (it writes the bound arrays), which saves four array copies.
+lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
 {
     const long long np = c->cfg.np;
     if (np == 0) return LP_OK;
@@ -298,16 +305,18 @@ lp_status do_sort(lp_ctx *c, bool copy_chi_back, cudaStream_t s)
     double *sx = c->at<double>(c->lay.xs);
     uint64_t *sid = c->at<uint64_t>(c->lay.alt_id);
     double *chi_alt = c->at<double>(c->lay.chi_alt);
-    double *pos[3] = { c->x, c->y, c->z };
+    const double *pos_src[3] = { c->x, c->y, c->z };
     for (int d = 0; d < 3; ++d)
-        if ((st = count(c, lp_launch_permute_f64(perm, pos[d], sx + (size_t)d * np, np, s), "permute launch")) != LP_OK) return st;
+        if ((st = count(c, lp_launch_permute_f64(perm, pos_src[d], sx + (size_t)d * np, np, s), "permute launch")) != LP_OK) return st;
     if ((st = count(c, lp_launch_permute_u64(perm, c->id, sid, np, s), "permute launch")) != LP_OK) return st;
     if ((st = count(c, lp_launch_permute_rows(perm, c->chi, chi_alt, np, c->cfg.nbins, s), "permute launch")) != LP_OK) return st;
-    for (int d = 0; d < 3; ++d)
-        LP_CUDA(c, cudaMemcpyAsync(pos[d], sx + (size_t)d * np, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
     LP_CUDA(c, cudaMemcpyAsync(c->id, sid, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
-    if (copy_chi_back)
+    if (in_place) {
+        double *pos[3] = { c->x, c->y, c->z };
+        for (int d = 0; d < 3; ++d)
+            LP_CUDA(c, cudaMemcpyAsync(pos[d], sx + (size_t)d * np, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
         LP_CUDA(c, cudaMemcpyAsync(c->chi, chi_alt, (size_t)np * c->cfg.nbins * 8, cudaMemcpyDeviceToDevice, s));
+    }
     c->stage0_done = false;      // k1 / x* / rho_old refer to the old order
     c->spectra_done = false;     // so do the per-particle n_sub / lost of the last update
     ++c->sorts;
@@ -498,16 +507,17 @@ lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
     if (ctx->cfg.np == 0) return LP_OK;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    const double *chi_in = ctx->chi;
+    const double *chi_in = ctx->chi, *pos_in = nullptr;
     const bool sort_now = ctx->cfg.sort_every > 0 && (ctx->steps - 1) % ctx->cfg.sort_every == 0;
     if (sort_now) {
-        // the permuted rows stay in the workspace; the spectral kernel reads them from there
-        // and writes the bound chi, which saves one copy of the whole spectrum array.
+        // the permuted rows and positions stay in the workspace; the fused kernel reads them from there
+        // and writes the bound arrays
         if ((st = do_sort(ctx, false, s)) != LP_OK) return st;
         chi_in = ctx->at<double>(ctx->lay.chi_alt);
+        pos_in = ctx->at<double>(ctx->lay.xs);
     }
     // frozen fields: both push stages run inside the spectral kernel's per-particle phase
-    return do_spectral(ctx, dt, chi_in, true, s);
+    return do_spectral(ctx, dt, chi_in, true, s, 0, -1, pos_in);
 }
 
 lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *hz, uint64_t *hid, double *hchi,

@@ -39,7 +39,8 @@ struct LpSpectralArgs {
     LpGeom g;
     LpLamCand cand;
     LpCells cells;
-    double *x, *y, *z;           // staged: x^{n+1} (read only).  fused: x^n in, x^{n+1} out
+    double *x, *y, *z;           // staged: x^{n+1} (read only).  fused: x^{n+1} out
+    const double *xin, *yin, *zin;   // positions read (== x, y, z except right after a re-sort: permuted scratch)
     const double *rho_old;       // staged: from push stage 0.  fused: unused
     int32_t *status;             // fused: outside-box flags [np]
     const double *chi_in;        // [np][nbins]  (may differ from chi_out after a re-sort)

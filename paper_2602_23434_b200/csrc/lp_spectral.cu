@@ -425,8 +425,8 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
     for (long long chunk = gw; chunk < nchunks; chunk += nw) {
         const long long base = chunk << 5;
         const bool have = base + lane < A.np;
-        const double px = have ? A.x[base + lane] : 0.0, py = have ? A.y[base + lane] : 0.0,
-                     pz = have ? A.z[base + lane] : 0.0;
+        const double px = have ? A.xin[base + lane] : 0.0, py = have ? A.yin[base + lane] : 0.0,
+                     pz = have ? A.zin[base + lane] : 0.0;
         lp_chunk_phase1<NB, FUSED>(A, base, lane, px, py, pz, sE, sR, sAC[warp], sNS[warp]);
         for (int j0 = 0; j0 < 32; j0 += U) {
             double buf[U][M];
@@ -673,7 +673,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
         double nx = 0.0, ny = 0.0, nz = 0.0;
         if ((uint32_t)warp < nblk && chunk_of(warp) + lane < np) {
             const size_t p = (size_t)chunk_of(warp) + lane;
-            nx = A.x[p]; ny = A.y[p]; nz = A.z[p];
+            nx = A.xin[p]; ny = A.yin[p]; nz = A.zin[p];
         }
 #pragma unroll 1
         for (uint32_t t = warp; t < nblk; t += NP) {
@@ -682,7 +682,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
             const double px = nx, py = ny, pz = nz;
             if (t + NP < nblk && chunk_of(t + NP) + lane < np) {
                 const size_t p = (size_t)chunk_of(t + NP) + lane;
-                nx = A.x[p]; ny = A.y[p]; nz = A.z[p];
+                nx = A.xin[p]; ny = A.yin[p]; nz = A.zin[p];
             }
             if (use >= 1) lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u);
             lp_chunk_phase1<NB, FUSED>(A, (long long)base, lane, px, py, pz, sE, sR, sAC + cs * 32, sNS + cs * 32);

@@ -94,11 +94,12 @@ def test_push_positions_bit_exact_over_steps(periodic):
 
 # ------------------------------------------------------------------ a2: sort
 
-@pytest.mark.parametrize("np_", [1, 31, 4097, 50000])
-def test_sort_order_and_permutation_bit_exact(np_):
+@pytest.mark.parametrize("np_,id_shift", [(1, 33), (31, 33), (4097, 33), (50000, 33), (5003, 62)])
+def test_sort_order_and_permutation_bit_exact(np_, id_shift):
+    """ids wider than 32 bits (35 and 64 significant bits: five and eight radix passes over the ids)."""
     w = small_turbulent(n=6, np_=np_, nbins=16)          # 216 cells: many ties per key
     lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
-    pid = pid + np.uint64(1 << 33) * (pid % np.uint64(3))        # ids wider than 32 bits
+    pid = pid + np.uint64(1 << id_shift) * (pid % np.uint64(3))
     lp.bind_particles(x, y, z, pid, chi)
     lp.sort()
     torch.cuda.synchronize()
