@@ -37,6 +37,8 @@ def parse():
     ap.add_argument("--nbins", type=int, default=0, help="override the bin count (workload 5 sweep)")
     ap.add_argument("--np", type=int, default=0, help="override the particle count (debugging only)")
     ap.add_argument("--grid", type=int, default=0, help="override the cells per axis (debugging only)")
+    ap.add_argument("--staged", action="store_true",
+                    help="time the staged calls (lp_push 0, lp_push 1, lp_spectral_update) instead of the fused lp_step")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -125,10 +127,11 @@ def step_dt(w):
     return 0.9 * w.cfl_e / lam_top
 
 
-def config_dict(w, n_gpus):
+def config_dict(w, n_gpus, staged=False):
     return {"workload": "BASELINE.json configs[%d] %s" % (w.index - 1, w.name), "grid": "%d^3" % w.n,
             "particles_per_gpu": w.np, "nbins": w.nbins, "sort_every": w.sort_every,
             "parallelism": "replicas x%d (particles independent, no collective)" % n_gpus,
+            "api": "staged lp_push(0), lp_push(1), lp_spectral_update" if staged else "fused lp_step",
             "l2": "inputs larger than L2 (chi rows %.2f GB per GPU)" % (w.np * w.nbins * 8 / 1e9)}
 
 
@@ -279,8 +282,21 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    nstep = [0]
+
+    def one_step():
+        if not args.staged:
+            lp.step(dt)
+            return
+        if w.sort_every and nstep[0] % w.sort_every == 0:
+            lp.sort()
+        nstep[0] += 1
+        lp.push(dt, 0)
+        lp.push(dt, 1)
+        lp.spectral_update(dt)
+
     for _ in range(args.warmup):
-        lp.step(dt)
+        one_step()
     barrier()
     B.lp_timing_enable(lp.ctx, args.steps)
     launches0 = lp.launch_count()
@@ -289,7 +305,7 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(args.steps):
-        lp.step(dt)
+        one_step()
     e1.record()
     torch.cuda.synchronize(dev)
     clocks = sampler.stop()
@@ -326,17 +342,29 @@ def run_ours(args):
     if rank != 0:
         return
     peak, peak_src = measured_peak()
-    alg_bytes = (16 * w.nbins + 32) * w.np                   # chi r+w, x,y,z, rho_old
+    # Algorithmic bytes of one launch of the dominant kernel:
+    #   rows: chi in and out, 16 N_b per particle;
+    #   state: fused lp_step x,y,z in and out (48); staged lp_spectral_update x,y,z and rho_old in (32);
+    #   grid: the (vx,vy,vz,rho,bx,by,bz) of every distinct cell the gathers touch, once: 56 B x
+    #         min(cells, 8 corners x particles) -- the three gathers of the fused kernel share their cells.
+    rows_bytes = 16 * w.nbins * w.np
+    state_bytes = (32 if args.staged else 48) * w.np
+    grid_bytes = 56 * min(w.n ** 3, 8 * w.np)
+    alg_bytes = rows_bytes + state_bytes + grid_bytes
     spec_avg_ms = spec_ms / max(spec_n, 1)
     achieved = alg_bytes / (spec_avg_ms * 1e-3) / 1e9 if spec_n else None
-    roofline = {"bound": "hbm", "kernel": "lp_spectral_kernel<%d>" % w.nbins, "achieved": achieved, "peak": peak,
+    kname = "lp_spectral_%s_kernel<%d,0,%d>" % ("bulk" if w.nbins <= 256 else "direct", w.nbins, 0 if args.staged else 1)
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
-                "traffic": stored_traffic(w.name, w.nbins), "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": spec_avg_ms,
+                "traffic": None if args.staged else stored_traffic(w.name, w.nbins), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes,
+                "algorithmic_bytes_split": {"rows": rows_bytes, "state": state_bytes, "grid": grid_bytes},
+                "achieved_rows_only": (rows_bytes / (spec_avg_ms * 1e-3) / 1e9) if spec_n else None,
+                "avg_launch_ms": spec_avg_ms,
                 "share_of_step": spec_ms / ms if ms else None}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world),
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, args.staged),
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
            "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],
                     "sorts_total": d["sorts"]}}
