@@ -207,9 +207,16 @@ lp_diag_kernel(const int32_t *__restrict__ nsub, const double *__restrict__ lost
     }
     double num = 0.0;
     const long long gw = (long long)blockIdx.x * kWarps + warp, nw = (long long)gridDim.x * kWarps;
-    for (long long r = gw; r < np; r += nw) {
-        const double *row = chi + r * nbins;
-        for (int i = lane; i < nbins; i += 32) num = fma(row[i], dE[i], num);
+    // four rows per trip (independent loads in flight); the sum order per lane is fixed by (gw, nw)
+    for (long long r = gw; r < np; r += 4 * nw) {
+        for (int i = lane; i < nbins; i += 32) {
+            const double w = dE[i];
+            double v[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) v[k] = (r + k * nw < np) ? chi[(r + k * nw) * nbins + i] : 0.0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) num = fma(v[k], w, num);
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -314,7 +321,7 @@ int lp_launch_max_u64(const uint64_t *v, long long np, unsigned long long *out, 
 int lp_launch_diag(const int32_t *nsub, const double *lost, const int32_t *status, const double *chi,
                    const double *tab, int nbins, long long np, double *partial, LpDiagDev *out, cudaStream_t s)
 {
-    const int blocks = 296;
+    const int blocks = 296;      // (the scratch `partial` holds 2 x 296 doubles)
     lp_diag_kernel<<<blocks, kThreads, 0, s>>>(nsub, lost, status, chi, tab, nbins, np, partial, out);
     lp_diag_final_kernel<<<1, 1, 0, s>>>(partial, blocks, out);
     return ok() ? 2 : -1;
