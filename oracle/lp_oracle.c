@@ -24,6 +24,7 @@
  *   orc_cfl_nsub         CFL-limited substep count           north_star                          R12
  *   orc_spectral_row     donor-cell upwind update of chi     PAPER.md:107 (Eq. 6)                R1,R10,R11
  *   orc_spectral_update  the three above for every particle  PAPER.md:218-231 (Particles_Spectra)
+ *   orc_shock_row/update spectrum reset at a shock crossing  PAPER.md:110-122 (Eq. 7-8)          S1-S4
  *   orc_step             one whole step with frozen fields   PAPER.md:216-233 (Table 1)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force cell search and O(N^2)
@@ -296,6 +297,52 @@ double orc_row_number(int32_t nbins, const double *dE, const double *chi)
     double s = 0.0;
     for (int i = 0; i < nbins; ++i) s = s + chi[i] * dE[i];
     return s;
+}
+
+/* ---------------------------------------------------------------- shock crossing (Eq. 7-8; NEXT-1) */
+
+/* Spectrum of a particle that crosses a shock of compression ratio r:
+ *   chi_out(e) = C * Int_{e_min}^{e} chi_in(e') (e/e')^(-q+2) de'/e'            (Eq. 7)
+ *              = C * e^(2-q) * Int_{e_min}^{e} chi_in(e') e'^(q-3) de',
+ *   q = 3r/(r-1) + q_R                                                          (Eq. 8)
+ * Readings (S1-S4): r is given per particle by the caller (the paper defines no
+ * shock finder), r <= 1 means "no shock": the row is left untouched; q_R is a caller-supplied scalar;
+ * the integral to the centre e_i of bin i is the midpoint sum over the bins below plus half of bin i,
+ *   I_i = sum_{j<i} chi_j ec_j^(q-3) dE_j + (1/2) chi_i ec_i^(q-3) dE_i,   ec = geometric bin centre;
+ * C ("a normalization that depends on the shock energy (see [19, 20])", not available here) keeps the
+ * particle's number: sum_i chi_out_i dE_i = sum_i chi_in_i dE_i.  A row whose unnormalised result sums
+ * to zero is left untouched.  Returns 1 if the row was changed. */
+int32_t orc_shock_row(int32_t nbins, const double *E, const double *dE, double r, double q_r,
+                      double *chi /*[nbins] in/out*/)
+{
+    if (!(r > 1.0)) return 0;
+    const double q = 3.0 * r / (r - 1.0) + q_r;
+    double *t = (double *)malloc((size_t)nbins * sizeof(double));
+    double below = 0.0, n_in = 0.0, n_out = 0.0;
+    for (int i = 0; i < nbins; ++i) {
+        const double ec = sqrt(E[i] * E[i + 1]);
+        const double term = chi[i] * pow(ec, q - 3.0) * dE[i];
+        const double integral = below + 0.5 * term;
+        t[i] = pow(ec, 2.0 - q) * integral;
+        below = below + term;
+        n_in = n_in + chi[i] * dE[i];
+        n_out = n_out + t[i] * dE[i];
+    }
+    int32_t changed = 0;
+    if (n_out != 0.0 && n_out == n_out) {
+        const double c = n_in / n_out;
+        for (int i = 0; i < nbins; ++i) chi[i] = c * t[i];
+        changed = 1;
+    }
+    free(t);
+    return changed;
+}
+
+/* every particle: row p with compression ratio r[p] */
+void orc_shock_update(int32_t nbins, const double *E, const double *dE, int64_t np, const double *r,
+                      double q_r, double *chi /*[np][nbins] in/out*/)
+{
+    for (int64_t p = 0; p < np; ++p) orc_shock_row(nbins, E, dE, r[p], q_r, chi + p * nbins);
 }
 
 /* ---------------------------------------------------------------- whole update / step */

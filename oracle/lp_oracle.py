@@ -154,6 +154,28 @@ def spectral_row(E, dE, a, cr, dtau, nsub, chi):
     return chi, lost.value
 
 
+def shock_row(E, dE, r, q_r, chi):
+    """Eq. 7-8 on one row; returns (new row, changed)."""
+    E, pE = _d(E); dE, pdE = _d(dE)
+    chi = np.array(chi, dtype=np.float64)
+    f = lib().orc_shock_row
+    f.restype = C.c_int32
+    ch = f(C.c_int32(dE.shape[0]), pE, pdE, C.c_double(r), C.c_double(q_r),
+           chi.ctypes.data_as(C.POINTER(C.c_double)))
+    return chi, bool(ch)
+
+
+def shock_update(E, dE, r, q_r, chi):
+    """Eq. 7-8 on every row of chi [np][nbins] with compression ratios r [np]; returns the new array."""
+    E, pE = _d(E); dE, pdE = _d(dE); r, pr = _d(r)
+    chi = np.array(chi, dtype=np.float64, order="C")
+    f = lib().orc_shock_update
+    f.restype = None
+    f(C.c_int32(dE.shape[0]), pE, pdE, C.c_int64(chi.shape[0]), pr, C.c_double(q_r),
+      chi.ctypes.data_as(C.POINTER(C.c_double)))
+    return chi
+
+
 def row_number(dE, chi):
     dE, pdE = _d(dE); chi, pchi = _d(chi)
     return float(lib().orc_row_number(C.c_int32(dE.shape[0]), pdE, pchi))
