@@ -122,6 +122,15 @@ LP_API lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream);
  * Consumes rho_old of the last lp_push(stage 0); LP_ERR_STATE if there was none. */
 LP_API lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream);
 
+/* Shock crossing (Eq. 7-8; not part of lp_step): every particle p with r[p] > 1 gets
+ *   chi_out,i = C ec_i^(2-q) [ sum_{j<i} chi_j ec_j^(q-3) dE_j + chi_i ec_i^(q-3) dE_i / 2 ],
+ *   q = 3 r[p] / (r[p] - 1) + q_r,   ec_i = sqrt(E_i E_{i+1}),
+ * with C fixed by number conservation (sum_i chi_i dE_i unchanged); rows with r[p] <= 1 or NaN, and rows
+ * whose unnormalised result sums to zero, are left untouched.  r: device array [np] of compression ratios
+ * (the paper defines no shock finder: the caller supplies them); q_r: the relativistic correction q_R of
+ * Eq. 8 as a scalar, 0 for non-relativistic shocks.  Acts on the bound chi in place. */
+LP_API lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void *stream);
+
 /* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
  * spectral update (order of Table 1, without the fluid stages). */
 LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);

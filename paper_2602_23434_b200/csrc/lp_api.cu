@@ -499,6 +499,17 @@ lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
     return do_spectral(ctx, dt, ctx->chi, false, static_cast<cudaStream_t>(stream));
 }
 
+lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    if (ctx->cfg.np == 0) return LP_OK;
+    if (!r) return fail(ctx, LP_ERR_INVALID_ARG, "r is NULL");
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    return count(ctx, lp_launch_shock(ctx->tab, r, q_r, ctx->chi, ctx->cfg.np, ctx->cfg.nbins, ctx->sm_count,
+                                      static_cast<cudaStream_t>(stream)), "lp_shock_kernel launch");
+}
+
 lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
 {
     lp_status st = need_ready(ctx, true);

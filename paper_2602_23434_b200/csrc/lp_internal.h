@@ -77,6 +77,10 @@ int lp_launch_push1(const LpPushArgs &a, cudaStream_t s);
 // fused = true: the kernel also does both push stages (a5, a6) in its per-particle phase (frozen fields)
 int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, bool fused, int sm_count, cudaStream_t s);
 
+// shock-crossing update of the flagged rows (lp_shock.cu); r [np] device, r <= 1 = untouched
+int lp_launch_shock(const double *tab, const double *r, double q_r, double *chi, long long np, int nbins,
+                    int sm_count, cudaStream_t s);
+
 // sort: fills perm[n] = source index of the n-th particle in (key, id) order.
 struct LpSortBufs {
     uint32_t *key;       // [np]

@@ -85,6 +85,11 @@ class LP:
     def spectral_update(self, dt):
         B.lp_spectral_update(self.ctx, dt, self.stream)
 
+    def shock_update(self, r, q_r=0.0):
+        """Eq. 7-8 on the rows with r[p] > 1; r: float64 CUDA tensor [np] of compression ratios."""
+        assert r.is_cuda and r.dtype == self.x.dtype and r.numel() == self.x.numel() and r.is_contiguous()
+        B.lp_shock_update(self.ctx, r.data_ptr(), q_r, self.stream)
+
     def step(self, dt):
         B.lp_step(self.ctx, dt, self.stream)
 

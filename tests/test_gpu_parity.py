@@ -172,6 +172,38 @@ def test_number_conservation_diag():
     assert d["steps"] == 1 and d["sorts"] == 0
 
 
+# ------------------------------------------------------------------ shock crossing (Eq. 7-8, NEXT-1)
+
+@pytest.mark.parametrize("nbins", [16, 32, 64, 128, 256, 512])
+def test_shock_update_matches_oracle(nbins):
+    """lp_shock_update vs the oracle row by row: flagged rows (r > 1) to 1e-10 relative, unflagged rows
+    (r <= 1, NaN) bit for bit untouched, empty bins below the lowest occupied one stay exactly zero."""
+    w = small_turbulent(np_=3000 + 37, nbins=nbins)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    rng = np.random.default_rng(nbins)
+    r = rng.uniform(1.5, 4.0, w.np)
+    r[rng.uniform(size=w.np) < 0.4] = 1.0                     # no shock
+    r[::97] = np.nan
+    r[5] = 0.3
+    chi = chi.copy()
+    chi[::7, : nbins // 4] = 0.0                              # rows with an empty low end
+    chi[11, :] = 0.0                                          # an empty row
+    lp.chi.copy_(torch.from_numpy(chi))
+    E, dE, _ = orc.bin_table(w.nbins, w.e_min, w.e_max)
+    q_r = 0.05
+    expect = orc.shock_update(E, dE, r, q_r, chi)
+    lp.shock_update(torch.from_numpy(r).cuda(), q_r)
+    torch.cuda.synchronize()
+    got = host(lp.chi)
+    untouched = ~(r > 1.0)
+    assert np.array_equal(got[untouched], chi[untouched]) and np.array_equal(got[11], chi[11])
+    assert_chi_close(got, expect)
+    assert np.array_equal(got == 0.0, expect == 0.0)
+    num_in, num_out = (chi * dE).sum(axis=1), (got * dE).sum(axis=1)
+    ok = num_in > 0
+    assert np.max(np.abs(num_out[ok] / num_in[ok] - 1)) < 1e-13                  # number conserved per row
+
+
 # ------------------------------------------------------------------ whole step, with re-sort
 
 @pytest.mark.parametrize("nbins,np_", [(64, 6000 + 3), (16, 2500), (128, 1500)])
