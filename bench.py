@@ -39,6 +39,8 @@ def parse():
     ap.add_argument("--grid", type=int, default=0, help="override the cells per axis (debugging only)")
     ap.add_argument("--staged", action="store_true",
                     help="time the staged calls (lp_push 0, lp_push 1, lp_spectral_update) instead of the fused lp_step")
+    ap.add_argument("--shock-frac", type=float, default=0.0,
+                    help="also time lp_shock_update (Eq. 7-8) with this fraction of particles flagged")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -318,6 +320,27 @@ def run_ours(args):
     ms = reduce_max(ms, dist, dev)
     value = aggregate_rate(world, w.np, args.steps, ms * 1e-3)
 
+    # ---- shock-crossing update (NEXT-1), timed alone on the resident state
+    shock = None
+    if args.shock_frac > 0:
+        rng = np.random.Generator(np.random.PCG64(w.seed + 3000))
+        r_host = np.where(rng.uniform(size=w.np) < args.shock_frac, rng.uniform(2.0, 4.0, size=w.np), 1.0)
+        r_dev = torch.from_numpy(r_host).to(dev)
+        nflag = int((r_host > 1.0).sum())
+        lp.shock_update(r_dev, 0.0)                          # warm-up
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 5
+        s0.record()
+        for _ in range(reps):
+            lp.shock_update(r_dev, 0.0)
+        s1.record()
+        torch.cuda.synchronize(dev)
+        sms = s0.elapsed_time(s1) / reps
+        sbytes = 8 * w.np + 16 * w.nbins * nflag             # r of every particle, flagged rows in and out
+        shock = {"kernel": "lp_shock_kernel<%d>" % w.nbins, "flagged": nflag, "ms": sms,
+                 "algorithmic_bytes": sbytes, "achieved_gbs": sbytes / (sms * 1e-3) / 1e9,
+                 "flagged_rows_per_s": nflag / (sms * 1e-3)}
+
     # ---- end to end through lp_step_host: pinned host buffers, H2D + D2H every step
     e2e = None
     if not args.no_e2e:
@@ -368,6 +391,10 @@ def run_ours(args):
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
            "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],
                     "sorts_total": d["sorts"]}}
+    if shock is not None:
+        peak_s, _ = measured_peak()
+        shock["frac_of_measured_peak"] = shock["achieved_gbs"] / peak_s
+        out["shock_update"] = shock
     if world == 1 and not args.no_cpu_baseline:
         fields_np = [f.cpu().numpy() for f in fields]
         out["cpu_baseline"] = cpu_baseline(w, fields_np, u_rad, x, y, z, pid, chi_host, dt, args.cpu_seconds)
