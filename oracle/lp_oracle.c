@@ -25,6 +25,7 @@
  *   orc_spectral_row     donor-cell upwind update of chi     PAPER.md:107 (Eq. 6)                R1,R10,R11
  *   orc_spectral_update  the three above for every particle  PAPER.md:218-231 (Particles_Spectra)
  *   orc_shock_row/update spectrum reset at a shock crossing  PAPER.md:110-122 (Eq. 7-8)          S1-S4
+ *   orc_compact          deletion with hole filling          PAPER.md:190-199                    C1
  *   orc_step             one whole step with frozen fields   PAPER.md:216-233 (Table 1)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force cell search and O(N^2)
@@ -343,6 +344,36 @@ void orc_shock_update(int32_t nbins, const double *E, const double *dE, int64_t 
                       double q_r, double *chi /*[np][nbins] in/out*/)
 {
     for (int64_t p = 0; p < np; ++p) orc_shock_row(nbins, E, dE, r[p], q_r, chi + p * nbins);
+}
+
+/* ---------------------------------------------------------------- deletion + hole filling (NEXT-2) */
+
+/* The paper's compaction, step by step:
+ *  1. flag and count the N_del particles to delete;  2. save the indices i_del of the flagged particles that
+ *  lie below N_p - N_del (the holes);  3. collect the indices i_f of the fillers, the particles stored at
+ *  i >= N_p - N_del that are not deleted;  4. copy every parameter of the fillers into the holes;
+ *  5. shrink to N_p - N_del.
+ * Reading (C1): the paper does not say which filler goes into which hole; here the k-th hole in
+ * ascending index order receives the k-th filler in ascending index order.  The surviving set is unique,
+ * the arrangement follows from this pairing.  Returns the new particle count. */
+int64_t orc_compact(int64_t np, const int32_t *flag, int32_t nbins,
+                    double *x, double *y, double *z, uint64_t *id, double *chi /*[np][nbins]*/)
+{
+    int64_t ndel = 0;
+    for (int64_t i = 0; i < np; ++i) if (flag[i]) ++ndel;                         /* step 1 */
+    const int64_t keep = np - ndel;
+    int64_t *holes = (int64_t *)malloc((size_t)(np > 0 ? np : 1) * sizeof(int64_t));
+    int64_t *fill = (int64_t *)malloc((size_t)(np > 0 ? np : 1) * sizeof(int64_t));
+    int64_t nh = 0, nf = 0;
+    for (int64_t i = 0; i < keep; ++i) if (flag[i]) holes[nh++] = i;              /* step 2 */
+    for (int64_t i = keep; i < np; ++i) if (!flag[i]) fill[nf++] = i;             /* step 3 */
+    for (int64_t k = 0; k < nh && k < nf; ++k) {                                  /* step 4 */
+        const int64_t d = holes[k], s = fill[k];
+        x[d] = x[s]; y[d] = y[s]; z[d] = z[s]; id[d] = id[s];
+        for (int32_t b = 0; b < nbins; ++b) chi[d * nbins + b] = chi[s * nbins + b];
+    }
+    free(holes); free(fill);
+    return keep;                                                                  /* step 5 */
 }
 
 /* ---------------------------------------------------------------- whole update / step */

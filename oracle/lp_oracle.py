@@ -176,6 +176,21 @@ def shock_update(E, dE, r, q_r, chi):
     return chi
 
 
+def compact(flag, x, y, z, pid, chi):
+    """The paper's delete-and-fill compaction; returns (x, y, z, id, chi) cut to the new count."""
+    flag = np.ascontiguousarray(flag, dtype=np.int32)
+    x = np.array(x, dtype=np.float64); y = np.array(y, dtype=np.float64); z = np.array(z, dtype=np.float64)
+    pid = np.array(pid, dtype=np.uint64)
+    chi = np.array(chi, dtype=np.float64, order="C")
+    f = lib().orc_compact
+    f.restype = C.c_int64
+    dp = C.POINTER(C.c_double)
+    keep = f(C.c_int64(x.shape[0]), flag.ctypes.data_as(C.POINTER(C.c_int32)), C.c_int32(chi.shape[1]),
+             x.ctypes.data_as(dp), y.ctypes.data_as(dp), z.ctypes.data_as(dp),
+             pid.ctypes.data_as(C.POINTER(C.c_uint64)), chi.ctypes.data_as(dp))
+    return x[:keep], y[:keep], z[:keep], pid[:keep], chi[:keep]
+
+
 def row_number(dE, chi):
     dE, pdE = _d(dE); chi, pchi = _d(chi)
     return float(lib().orc_row_number(C.c_int32(dE.shape[0]), pdE, pchi))
