@@ -131,6 +131,15 @@ LP_API lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream);
  * Eq. 8 as a scalar, 0 for non-relativistic shocks.  Acts on the bound chi in place. */
 LP_API lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void *stream);
 
+/* Deletion with hole filling (not part of lp_step): the particles with flag[p] != 0 are
+ * removed, the survivors stored at p >= N_p - N_del move into the flagged slots below N_p - N_del (k-th hole
+ * in ascending order <- k-th such survivor in ascending order), with all their parameters (x, y, z, id, chi
+ * row); the context then holds *np_new = N_p - N_del particles in the first *np_new entries of the bound
+ * arrays (the arrays and the workspace keep their size).  flag: device int32 [np], or NULL to delete the
+ * particles the last lp_push(stage 1) / lp_step marked outside the box on a non-periodic axis (outflow,
+ * Particles_Boundary); LP_ERR_STATE if there is no such marking.  Synchronises `stream`. */
+LP_API lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new /*host*/, void *stream);
+
 /* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
  * spectral update (order of Table 1, without the fluid stages). */
 LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);

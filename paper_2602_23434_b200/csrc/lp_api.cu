@@ -145,6 +145,8 @@ struct lp_ctx {
     LpLamCand cand;
     // state
     bool have_fields = false, stage0_done = false, spectra_done = false;
+    bool status_valid = false;             // the status array describes the bound particles in their current order
+    long long capacity = 0;                // particles the workspace was sized for (cfg.np shrinks in lp_compact)
     int id_bits = 0, key_bits = 0;
     long long launches = 0, steps = 0, sorts = 0;
     // optional timing of the spectral kernel (lp_timing_enable): event pairs, resolved on read
@@ -280,7 +282,11 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
         LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], s));
         c->ev_used += 2;
     }
-    if (st == LP_OK) { c->spectra_done = true; c->stage0_done = false; }
+    if (st == LP_OK) {
+        c->spectra_done = true;
+        c->stage0_done = false;
+        if (fused) c->status_valid = true;
+    }
     return st;
 }
 
@@ -319,6 +325,7 @@ lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
     }
     c->stage0_done = false;      // k1 / x* / rho_old refer to the old order
     c->spectra_done = false;     // so do the per-particle n_sub / lost of the last update
+    c->status_valid = false;
     ++c->sorts;
     return LP_OK;
 }
@@ -337,6 +344,7 @@ lp_status lp_create(const lp_config *cfg, lp_ctx **out)
     lp_ctx *c = new (std::nothrow) lp_ctx();
     if (!c) return LP_ERR_INVALID_ARG;
     c->cfg = *cfg;
+    c->capacity = cfg->np;
     c->lay = make_layout(*cfg);
     LpGeom &g = c->geom;
     g.nx = cfg->nx; g.ny = cfg->ny; g.nz = cfg->nz;
@@ -416,6 +424,7 @@ lp_status lp_bind_particles(lp_ctx *ctx, double *x, double *y, double *z, uint64
     ctx->x = x; ctx->y = y; ctx->z = z; ctx->id = id; ctx->chi = chi;
     ctx->stage0_done = false;
     ctx->spectra_done = false;
+    ctx->status_valid = false;
     ctx->id_bits = 0;
     if (ctx->cfg.np > 0) {      // number of radix passes over the ids: bit length of the largest id
         LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
@@ -486,7 +495,9 @@ lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream)
         if (st == LP_OK) ctx->stage0_done = true;
         return st;
     }
-    return count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch");
+    st = count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch");
+    if (st == LP_OK) ctx->status_valid = true;
+    return st;
 }
 
 lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
@@ -508,6 +519,34 @@ lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void *stream
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     return count(ctx, lp_launch_shock(ctx->tab, r, q_r, ctx->chi, ctx->cfg.np, ctx->cfg.nbins, ctx->sm_count,
                                       static_cast<cudaStream_t>(stream)), "lp_shock_kernel launch");
+}
+
+lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    if (!np_new) return fail(ctx, LP_ERR_INVALID_ARG, "np_new is NULL");
+    *np_new = ctx->cfg.np;
+    if (ctx->cfg.np == 0) return LP_OK;
+    if (!flag && !ctx->status_valid)
+        return fail(ctx, LP_ERR_STATE, "no flags given and no outside-box status of the bound particles (lp_push 1 / lp_step first)");
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (!flag) flag = ctx->at<int32_t>(ctx->lay.status);
+    unsigned long long *counts = ctx->at<unsigned long long>(ctx->lay.partial), h_counts[2] = { 0, 0 };
+    st = count(ctx, lp_launch_compact(flag, ctx->cfg.np, ctx->cfg.nbins, ctx->at<uint32_t>(ctx->lay.hist),
+                                      ctx->at<uint32_t>(ctx->lay.idx_a), ctx->at<uint32_t>(ctx->lay.idx_b),
+                                      ctx->at<uint32_t>(ctx->lay.key), counts, ctx->x, ctx->y, ctx->z, ctx->id,
+                                      ctx->chi, ctx->sm_count, s), "compaction kernels launch");
+    if (st != LP_OK) return st;
+    LP_CUDA(ctx, cudaMemcpyAsync(h_counts, counts, sizeof h_counts, cudaMemcpyDeviceToHost, s));
+    LP_CUDA(ctx, cudaStreamSynchronize(s));
+    ctx->cfg.np -= (long long)h_counts[0];          // the workspace keeps its size (capacity)
+    ctx->stage0_done = false;
+    ctx->spectra_done = false;
+    ctx->status_valid = false;
+    *np_new = ctx->cfg.np;
+    return LP_OK;
 }
 
 lp_status lp_step(lp_ctx *ctx, double dt, void *stream)

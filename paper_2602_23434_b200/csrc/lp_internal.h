@@ -81,6 +81,12 @@ int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, bool fused
 int lp_launch_shock(const double *tab, const double *r, double q_r, double *chi, long long np, int nbins,
                     int sm_count, cudaStream_t s);
 
+// deletion with hole filling (lp_compact.cu); counts = 2 x u64 on the device: N_del, number of holes
+size_t lp_compact_block_elems(long long np);
+int lp_launch_compact(const int32_t *flag, long long np, int nbins, uint32_t *blk, uint32_t *rank, uint32_t *hole,
+                      uint32_t *filler, unsigned long long *counts, double *x, double *y, double *z, uint64_t *id,
+                      double *chi, int sm_count, cudaStream_t s);
+
 // sort: fills perm[n] = source index of the n-th particle in (key, id) order.
 struct LpSortBufs {
     uint32_t *key;       // [np]

@@ -90,6 +90,14 @@ class LP:
         assert r.is_cuda and r.dtype == self.x.dtype and r.numel() == self.x.numel() and r.is_contiguous()
         B.lp_shock_update(self.ctx, r.data_ptr(), q_r, self.stream)
 
+    def compact(self, flag=None):
+        """Delete the flagged particles (int32 CUDA tensor [np], nonzero = delete; None = those outside the
+        box after the last push) and fill the holes from the tail; returns the new particle count.  The
+        tensors keep their size: the first `count` entries are the particles."""
+        if flag is not None:
+            assert flag.is_cuda and flag.dtype == torch.int32 and flag.is_contiguous()
+        return B.lp_compact(self.ctx, flag.data_ptr() if flag is not None else None, self.stream)
+
     def step(self, dt):
         B.lp_step(self.ctx, dt, self.stream)
 

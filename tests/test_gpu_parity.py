@@ -204,6 +204,47 @@ def test_shock_update_matches_oracle(nbins):
     assert np.max(np.abs(num_out[ok] / num_in[ok] - 1)) < 1e-13                  # number conserved per row
 
 
+# ------------------------------------------------------------------ deletion + hole filling (NEXT-2)
+
+@pytest.mark.parametrize("np_,frac", [(1, 1.0), (33, 0.5), (5000 + 7, 0.05), (70001, 0.3), (4097, 0.0), (4097, 1.0)])
+def test_compact_matches_oracle_bit_exact(np_, frac):
+    """lp_compact vs the paper's five steps in the oracle: the same particles in the same slots, every
+    parameter bit for bit; the context then steps the shortened set like the oracle does."""
+    w = small_turbulent(np_=np_, nbins=32)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
+    rng = np.random.default_rng(np_)
+    flag = (rng.uniform(size=np_) < frac).astype(np.int32)
+    n_new = lp.compact(torch.from_numpy(flag).cuda())
+    x, y, z, pid, chi = orc.compact(flag, x, y, z, pid, chi)
+    assert n_new == x.shape[0] == np_ - int(flag.sum()) and lp.diag()["np"] == n_new
+    assert np.array_equal(host(lp.id)[:n_new].view(np.uint64), pid)
+    assert np.array_equal(host(lp.x)[:n_new], x) and np.array_equal(host(lp.y)[:n_new], y)
+    assert np.array_equal(host(lp.z)[:n_new], z) and np.array_equal(host(lp.chi)[:n_new], chi)
+    if n_new:
+        lp.step(w.dt)
+        x, y, z, chi, nsub, lost, st = orc.step(prm, f_np, x, y, z, w.dt, chi, nthreads=8)
+        assert np.array_equal(host(lp.x)[:n_new], x)
+        assert_nsub_equal(host(lp.nsub)[:n_new], nsub)
+        assert_chi_close(host(lp.chi)[:n_new], chi)
+
+
+def test_compact_outflow_deletes_what_left_the_box():
+    """Open (zero-gradient) box: after a step some particles are outside; lp_compact without flags deletes
+    exactly those (Particles_Boundary) and a second call without a new push is refused."""
+    w = small_turbulent(np_=6000, nbins=16).scaled(periodic=(0, 0, 0), dt=0.2)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    lp.step(w.dt)
+    x, y, z, chi, nsub, lost, st = orc.step(prm, f_np, x, y, z, w.dt, chi, nthreads=8)
+    assert (st != 0).sum() > 10
+    n_new = lp.compact()
+    x, y, z, pid, chi = orc.compact((st != 0).astype(np.int32), x, y, z, pid, chi)
+    assert n_new == x.shape[0]
+    assert np.array_equal(host(lp.id)[:n_new].view(np.uint64), pid) and np.array_equal(host(lp.x)[:n_new], x)
+    assert_chi_close(host(lp.chi)[:n_new], chi)            # (rows went through one update: 1e-10, not bits)
+    with pytest.raises(P.binding.LPError):
+        lp.compact()
+
+
 # ------------------------------------------------------------------ whole step, with re-sort
 
 @pytest.mark.parametrize("nbins,np_", [(64, 6000 + 3), (16, 2500), (128, 1500)])
