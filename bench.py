@@ -41,6 +41,8 @@ def parse():
                     help="time the staged calls (lp_push 0, lp_push 1, lp_spectral_update) instead of the fused lp_step")
     ap.add_argument("--shock-frac", type=float, default=0.0,
                     help="also time lp_shock_update (Eq. 7-8) with this fraction of particles flagged")
+    ap.add_argument("--compact-frac", type=float, default=0.0,
+                    help="at the very end, time one lp_compact (PAPER.md:190-199) deleting this fraction of particles")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -362,6 +364,25 @@ def run_ours(args):
                "api": "lp_step_host (pinned host x,y,z,id,chi in and out every step)"}
         del hx, hy, hz, hid, hchi
 
+    # ---- deletion with hole filling (NEXT-2): one call at the end (it shrinks the particle set)
+    compact = None
+    if args.compact_frac > 0:
+        rng = np.random.Generator(np.random.PCG64(w.seed + 4000))
+        flag = torch.from_numpy((rng.uniform(size=w.np) < args.compact_frac).astype(np.int32)).to(dev)
+        ndel = int(flag.sum().item())
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        c0.record()
+        n_new = lp.compact(flag)
+        c1.record()
+        torch.cuda.synchronize(dev)
+        cms = c0.elapsed_time(c1)
+        holes = int(flag[: w.np - ndel].sum().item())
+        # flags read by the count and the rank pass, ranks written and read, moved particles in and out
+        cbytes = w.np * (4 + 4 + 4 + 4 + 4) + holes * 2 * (32 + 8 * w.nbins)
+        compact = {"deleted": ndel, "moved": holes, "np_new": n_new, "ms": cms, "algorithmic_bytes": cbytes,
+                   "achieved_gbs": cbytes / (cms * 1e-3) / 1e9}
+
     if rank != 0:
         return
     peak, peak_src = measured_peak()
@@ -391,6 +412,8 @@ def run_ours(args):
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
            "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],
                     "sorts_total": d["sorts"]}}
+    if compact is not None:
+        out["compact"] = compact
     if shock is not None:
         peak_s, _ = measured_peak()
         shock["frac_of_measured_peak"] = shock["achieved_gbs"] / peak_s
