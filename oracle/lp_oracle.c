@@ -26,6 +26,7 @@
  *   orc_spectral_update  the three above for every particle  PAPER.md:218-231 (Particles_Spectra)
  *   orc_shock_row/update spectrum reset at a shock crossing  PAPER.md:110-122 (Eq. 7-8)          S1-S4
  *   orc_compact          deletion with hole filling          PAPER.md:190-199                    C1
+ *   orc_push_rk3_stage   three-stage third-order pusher      PAPER.md:245, 258-260               K1
  *   orc_step             one whole step with frozen fields   PAPER.md:216-233 (Table 1)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force cell search and O(N^2)
@@ -220,6 +221,46 @@ void orc_push_stage1(const orc_params *g, const double *const *fields7, int64_t 
             pos[d][p] = xn;
         }
         if (status) status[p] = st;
+    }
+}
+
+/* Third-order pusher (NEXT-4; PAPER.md:245, 258-260 show a "third order Runge-Kutta" next to the second
+ * order one without naming the variant).  Reading K1: the three-stage Shu-Osher (SSP) scheme
+ * that PLUTO's RK3 time stepping uses, one call per stage so that the caller can advance the fields in
+ * between, as for the two-stage pusher:
+ *   stage 0:  x0 = x^n (kept);  rho_old = rho(x^n);  x1 = x0 + dt v(x0)
+ *   stage 1:  x2 = (3/4) x0 + (1/4) (x1 + dt v(x1))
+ *   stage 2:  x^{n+1} = (x0 + 2 (x2 + dt v(x2))) / 3;  periodic wrap / outside flag as orc_push_stage1.
+ * x, y, z hold the current stage position on entry and the next one on return; intermediate positions
+ * are not wrapped (the gather wraps indices). */
+void orc_push_rk3_stage(const orc_params *g, const double *const *fields7, int64_t np, int32_t stage,
+                        double *x, double *y, double *z, double *x0 /*[3][np]*/, double dt,
+                        double *rho_old /*[np], stage 0*/, int32_t *status /*[np] or NULL, stage 2*/)
+{
+    const double *q[4] = { fields7[0], fields7[1], fields7[2], fields7[6] };
+    double *pos[3] = { x, y, z };
+    for (int64_t p = 0; p < np; ++p) {
+        double o[4];
+        int32_t st = 0;
+        gather_point(g, 4, q, x[p], y[p], z[p], o);
+        for (int d = 0; d < 3; ++d) {
+            const double cur = pos[d][p];
+            const double adv = cur + dt * o[d];
+            double xn;
+            if (stage == 0) {
+                x0[(int64_t)d * np + p] = cur;
+                xn = adv;
+            } else if (stage == 1) {
+                xn = 0.75 * x0[(int64_t)d * np + p] + 0.25 * adv;
+            } else {
+                xn = (x0[(int64_t)d * np + p] + 2.0 * adv) / 3.0;
+                if (g->periodic[d]) xn = wrap_pos(xn, g->xlo[d], g->xhi[d]);
+                else if (xn < g->xlo[d] || xn >= g->xhi[d]) st |= (1 << d);
+            }
+            pos[d][p] = xn;
+        }
+        if (stage == 0 && rho_old) rho_old[p] = o[3];
+        if (stage == 2 && status) status[p] = st;
     }
 }
 

@@ -126,6 +126,27 @@ def push_stage1(prm, fields7, x, y, z, xs, k1, dt, nthreads=1):
     return x, y, z, status
 
 
+def push_rk3(prm, fields_by_stage, x, y, z, dt):
+    """One third-order step; fields_by_stage: the seven fields to use at stages 0, 1, 2 (or one set for all).
+    Returns (x, y, z, rho_old, status, stage positions [(x1,y1,z1), (x2,y2,z2)])."""
+    if not isinstance(fields_by_stage[0], (list, tuple)):
+        fields_by_stage = [fields_by_stage] * 3
+    x = np.array(x, dtype=np.float64); y = np.array(y, dtype=np.float64); z = np.array(z, dtype=np.float64)
+    n = x.shape[0]
+    x0 = np.empty((3, n)); rho_old = np.empty(n); status = np.zeros(n, dtype=np.int32)
+    dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+    f = lib().orc_push_rk3_stage
+    f.restype = None
+    mids = []
+    for stage in range(3):
+        keep, fa = _fields(fields_by_stage[stage])
+        f(C.byref(prm), fa, C.c_int64(n), C.c_int32(stage), dp(x), dp(y), dp(z), dp(x0), C.c_double(dt),
+          dp(rho_old), status.ctypes.data_as(C.POINTER(C.c_int32)))
+        if stage < 2:
+            mids.append((x.copy(), y.copy(), z.copy()))
+    return x, y, z, rho_old, status, mids
+
+
 def coefficients(prm, dt, v, B, rho_new, rho_old):
     a = C.c_double(); cr = C.c_double(); dtau = C.c_double()
     v3 = (C.c_double * 3)(*[float(t) for t in v]); b3 = (C.c_double * 3)(*[float(t) for t in B])
