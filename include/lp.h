@@ -117,6 +117,15 @@ LP_API lp_status lp_sort(lp_ctx *ctx, void *stream);
  * stage 1 without a preceding stage 0 returns LP_ERR_STATE. */
 LP_API lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream);
 
+/* Third-order pusher, an alternative to lp_push (the paper does not name the
+ * variant: the three-stage Shu-Osher scheme is taken), one call per stage, fields may be re-set in between:
+ *   stage 0: x0 = x^n (kept in the workspace), rho_old = rho(x^n), x <- x0 + dt v(x0)
+ *   stage 1: x <- (3/4) x0 + (1/4) (x + dt v(x))
+ *   stage 2: x <- (x0 + 2 (x + dt v(x))) / 3, periodic wrap / outside flag.
+ * The bound x, y, z hold the stage positions in between.  Stages out of order return LP_ERR_STATE.
+ * lp_spectral_update may follow stage 2 (it uses the rho_old of stage 0). */
+LP_API lp_status lp_push_rk3(lp_ctx *ctx, double dt, int stage, void *stream);
+
 /* Spectral update at the current positions with the current fields:
  * coefficients, CFL substep count, n_sub donor-cell upwind substeps of Eq. 6 per particle.
  * Consumes rho_old of the last lp_push(stage 0); LP_ERR_STATE if there was none. */

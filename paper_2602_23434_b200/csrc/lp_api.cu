@@ -145,6 +145,8 @@ struct lp_ctx {
     LpLamCand cand;
     // state
     bool have_fields = false, stage0_done = false, spectra_done = false;
+    int push_kind = 0;                     // which pusher ran stage 0: 1 two-stage (k1, x* kept), 2 three-stage (x0 kept)
+    int rk3_next = 0;                      // next stage lp_push_rk3 expects
     bool status_valid = false;             // the status array describes the bound particles in their current order
     long long capacity = 0;                // particles the workspace was sized for (cfg.np shrinks in lp_compact)
     int id_bits = 0, key_bits = 0;
@@ -284,7 +286,7 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
     }
     if (st == LP_OK) {
         c->spectra_done = true;
-        c->stage0_done = false;
+        c->stage0_done = false; c->rk3_next = 0;
         if (fused) c->status_valid = true;
     }
     return st;
@@ -323,7 +325,7 @@ lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
             LP_CUDA(c, cudaMemcpyAsync(pos[d], sx + (size_t)d * np, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
         LP_CUDA(c, cudaMemcpyAsync(c->chi, chi_alt, (size_t)np * c->cfg.nbins * 8, cudaMemcpyDeviceToDevice, s));
     }
-    c->stage0_done = false;      // k1 / x* / rho_old refer to the old order
+    c->stage0_done = false; c->rk3_next = 0;      // k1 / x* / rho_old refer to the old order
     c->spectra_done = false;     // so do the per-particle n_sub / lost of the last update
     c->status_valid = false;
     ++c->sorts;
@@ -410,7 +412,7 @@ lp_status lp_bind_workspace(lp_ctx *ctx, void *workspace, size_t bytes)
     if (bytes < ctx->lay.total) return fail(ctx, LP_ERR_WORKSPACE, "workspace smaller than lp_workspace_bytes");
     ctx->ws = static_cast<unsigned char *>(workspace);
     ctx->have_fields = false;
-    ctx->stage0_done = false;
+    ctx->stage0_done = false; ctx->rk3_next = 0;
     ctx->spectra_done = false;
     return LP_OK;
 }
@@ -422,7 +424,7 @@ lp_status lp_bind_particles(lp_ctx *ctx, double *x, double *y, double *z, uint64
     if (ctx->cfg.np > 0 && (!x || !y || !z || !id || !chi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL particle array");
     if (reinterpret_cast<uintptr_t>(chi) % 16) return fail(ctx, LP_ERR_INVALID_ARG, "chi not 16-byte aligned");
     ctx->x = x; ctx->y = y; ctx->z = z; ctx->id = id; ctx->chi = chi;
-    ctx->stage0_done = false;
+    ctx->stage0_done = false; ctx->rk3_next = 0;
     ctx->spectra_done = false;
     ctx->status_valid = false;
     ctx->id_bits = 0;
@@ -485,19 +487,38 @@ lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream)
     lp_status st = need_ready(ctx, true);
     if (st != LP_OK) return st;
     if (stage != 0 && stage != 1) return fail(ctx, LP_ERR_INVALID_ARG, "stage must be 0 or 1");
-    if (stage == 1 && !ctx->stage0_done) return fail(ctx, LP_ERR_STATE, "lp_push stage 1 without stage 0");
+    if (stage == 1 && !(ctx->stage0_done && ctx->push_kind == 1)) return fail(ctx, LP_ERR_STATE, "lp_push stage 1 without stage 0");
     if (ctx->cfg.np == 0) { ctx->stage0_done = true; return LP_OK; }
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     LpPushArgs a = push_args(ctx, dt);
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     if (stage == 0) {
         st = count(ctx, lp_launch_push0(a, s), "lp_push0_kernel launch");
-        if (st == LP_OK) ctx->stage0_done = true;
+        if (st == LP_OK) { ctx->stage0_done = true; ctx->push_kind = 1; ctx->rk3_next = 0; }
         return st;
     }
     st = count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch");
     if (st == LP_OK) ctx->status_valid = true;
     return st;
+}
+
+lp_status lp_push_rk3(lp_ctx *ctx, double dt, int stage, void *stream)
+{
+    lp_status st = need_ready(ctx, true);
+    if (st != LP_OK) return st;
+    if (stage < 0 || stage > 2) return fail(ctx, LP_ERR_INVALID_ARG, "stage must be 0, 1 or 2");
+    if (stage != 0 && !(ctx->push_kind == 2 && ctx->rk3_next == stage))
+        return fail(ctx, LP_ERR_STATE, "lp_push_rk3 stages must run in the order 0, 1, 2");
+    if (ctx->cfg.np > 0) {
+        LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+        LpPushArgs a = push_args(ctx, dt);
+        st = count(ctx, lp_launch_push_rk3(a, stage, static_cast<cudaStream_t>(stream)), "lp_push_rk3_kernel launch");
+        if (st != LP_OK) return st;
+    }
+    if (stage == 0) { ctx->stage0_done = true; ctx->push_kind = 2; ctx->status_valid = false; }
+    if (stage == 2) ctx->status_valid = true;
+    ctx->rk3_next = stage == 2 ? 0 : stage + 1;
+    return LP_OK;
 }
 
 lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
@@ -542,7 +563,7 @@ lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *st
     LP_CUDA(ctx, cudaMemcpyAsync(h_counts, counts, sizeof h_counts, cudaMemcpyDeviceToHost, s));
     LP_CUDA(ctx, cudaStreamSynchronize(s));
     ctx->cfg.np -= (long long)h_counts[0];          // the workspace keeps its size (capacity)
-    ctx->stage0_done = false;
+    ctx->stage0_done = false; ctx->rk3_next = 0;
     ctx->spectra_done = false;
     ctx->status_valid = false;
     *np_new = ctx->cfg.np;

@@ -74,6 +74,7 @@ int lp_launch_interpolate(const LpGeom &g, const LpCells &c, const double *x, co
                           const double *z, long long np, double *out7, uint32_t *key, cudaStream_t s);
 int lp_launch_push0(const LpPushArgs &a, cudaStream_t s);
 int lp_launch_push1(const LpPushArgs &a, cudaStream_t s);
+int lp_launch_push_rk3(const LpPushArgs &a, int stage, cudaStream_t s);     // stage 0, 1, 2 (x0 kept in a.xs)
 // fused = true: the kernel also does both push stages (a5, a6) in its per-particle phase (frozen fields)
 int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, bool fused, int sm_count, cudaStream_t s);
 

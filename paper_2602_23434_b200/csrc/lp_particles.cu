@@ -98,7 +98,53 @@ __global__ void __launch_bounds__(kThreads) lp_push1_kernel(LpPushArgs A)
     A.status[p] = stt;
 }
 
+// Three-stage third-order pusher (reading K1 of DESIGN.md), one launch per stage:
+//   0: x0 = x^n kept in the x* scratch, rho_old = rho(x^n), x <- x0 + dt v(x0)
+//   1: x <- (3/4) x0 + (1/4) (x + dt v(x))
+//   2: x <- (x0 + 2 (x + dt v(x))) / 3, periodic wrap / outside flag
+template <int STAGE>
+__global__ void __launch_bounds__(kThreads) lp_push_rk3_kernel(LpPushArgs A)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= A.np) return;
+    const long long np = A.np;
+    double *pos[3] = { A.x, A.y, A.z };
+    const double cur[3] = { A.x[p], A.y[p], A.z[p] };
+    LpStencil st;
+    lp_stencil(A.g, cur[0], cur[1], cur[2], st);
+    double q[4];
+    lp_gather_A(A.cells, st, q);
+    int stt = 0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double adv = __dadd_rn(cur[d], __dmul_rn(A.dt, q[d]));
+        double xn;
+        if (STAGE == 0) {
+            A.xs[(long long)d * np + p] = cur[d];
+            xn = adv;
+        } else if (STAGE == 1) {
+            xn = __dadd_rn(__dmul_rn(0.75, A.xs[(long long)d * np + p]), __dmul_rn(0.25, adv));
+        } else {
+            xn = __ddiv_rn(__dadd_rn(A.xs[(long long)d * np + p], __dmul_rn(2.0, adv)), 3.0);
+            if (A.g.per[d]) xn = lp_wrap_pos(xn, A.g.xlo[d], A.g.xhi[d], A.g.len[d]);
+            else if (xn < A.g.xlo[d] || xn >= A.g.xhi[d]) stt |= (1 << d);
+        }
+        pos[d][p] = xn;
+    }
+    if (STAGE == 0) A.rho_old[p] = q[3];
+    if (STAGE == 2) A.status[p] = stt;
+}
+
 }  // namespace
+
+int lp_launch_push_rk3(const LpPushArgs &a, int stage, cudaStream_t s)
+{
+    const int blocks = blocks_for(a.np, kThreads);
+    if (stage == 0) lp_push_rk3_kernel<0><<<blocks, kThreads, 0, s>>>(a);
+    else if (stage == 1) lp_push_rk3_kernel<1><<<blocks, kThreads, 0, s>>>(a);
+    else lp_push_rk3_kernel<2><<<blocks, kThreads, 0, s>>>(a);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
 
 int lp_launch_repack(const double *const f[7], double4 *recA, double4 *recB, long long ncell, cudaStream_t s)
 {

@@ -82,6 +82,9 @@ class LP:
     def push(self, dt, stage):
         B.lp_push(self.ctx, dt, stage, self.stream)
 
+    def push_rk3(self, dt, stage):
+        B.lp_push_rk3(self.ctx, dt, stage, self.stream)
+
     def spectral_update(self, dt):
         B.lp_spectral_update(self.ctx, dt, self.stream)
 

@@ -172,6 +172,36 @@ def test_number_conservation_diag():
     assert d["steps"] == 1 and d["sorts"] == 0
 
 
+# ------------------------------------------------------------------ third-order pusher (NEXT-4)
+
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 1, 0)])
+def test_push_rk3_bit_exact_and_spectral_update_follows(periodic):
+    """lp_push_rk3 stage by stage vs the oracle (positions of every stage bit for bit, outside flags),
+    fields changed between the stages, then lp_spectral_update with the rho_old of stage 0."""
+    w = small_turbulent(np_=4000 + 5, nbins=32).scaled(periodic=periodic, dt=0.05)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    fields_b = I.make_fields(w.scaled(seed=w.seed + 1), device="cpu")          # "advanced" fields for stages 1, 2
+    fb_np = fields_to_numpy(fields_b)
+    for step in range(3):
+        xe, ye, ze, rho_old, st, mids = orc.push_rk3(prm, [f_np, fb_np, fb_np], x, y, z, w.dt)
+        lp.set_fields([f.cuda() for f in I.make_fields(w, device="cpu")])
+        lp.push_rk3(w.dt, 0)
+        assert np.array_equal(host(lp.x), mids[0][0]) and np.array_equal(host(lp.z), mids[0][2])
+        lp.set_fields([f.cuda() for f in fields_b])
+        lp.push_rk3(w.dt, 1)
+        assert np.array_equal(host(lp.x), mids[1][0]) and np.array_equal(host(lp.y), mids[1][1])
+        lp.push_rk3(w.dt, 2)
+        assert np.array_equal(host(lp.x), xe) and np.array_equal(host(lp.y), ye) and np.array_equal(host(lp.z), ze)
+        lp.spectral_update(w.dt)
+        chi, nsub, lost = orc.spectral_update(prm, fb_np, xe, ye, ze, rho_old, w.dt, chi, nthreads=8)
+        assert_nsub_equal(host(lp.nsub), nsub)
+        assert_chi_close(host(lp.chi), chi)
+        assert lp.diag()["n_outside"] == int((st != 0).sum())
+        x, y, z = xe, ye, ze
+    with pytest.raises(P.binding.LPError):
+        lp.push_rk3(w.dt, 2)                               # stages out of order
+
+
 # ------------------------------------------------------------------ shock crossing (Eq. 7-8, NEXT-1)
 
 @pytest.mark.parametrize("nbins", [16, 32, 64, 128, 256, 512])
