@@ -43,6 +43,8 @@ def parse():
                     help="also time lp_shock_update (Eq. 7-8) with this fraction of particles flagged")
     ap.add_argument("--compact-frac", type=float, default=0.0,
                     help="at the very end, time one lp_compact (PAPER.md:190-199) deleting this fraction of particles")
+    ap.add_argument("--pusher", default="rk2", choices=["rk2", "rk3"],
+                    help="with --staged: the two-stage pusher (lp_push) or the three-stage one (lp_push_rk3)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -135,7 +137,7 @@ def config_dict(w, n_gpus, staged=False):
     return {"workload": "BASELINE.json configs[%d] %s" % (w.index - 1, w.name), "grid": "%d^3" % w.n,
             "particles_per_gpu": w.np, "nbins": w.nbins, "sort_every": w.sort_every,
             "parallelism": "replicas x%d (particles independent, no collective)" % n_gpus,
-            "api": "staged lp_push(0), lp_push(1), lp_spectral_update" if staged else "fused lp_step",
+            "api": ("staged %s, lp_spectral_update" % staged) if staged else "fused lp_step",
             "l2": "inputs larger than L2 (chi rows %.2f GB per GPU)" % (w.np * w.nbins * 8 / 1e9)}
 
 
@@ -295,8 +297,12 @@ def run_ours(args):
         if w.sort_every and nstep[0] % w.sort_every == 0:
             lp.sort()
         nstep[0] += 1
-        lp.push(dt, 0)
-        lp.push(dt, 1)
+        if args.pusher == "rk3":
+            for stage in range(3):
+                lp.push_rk3(dt, stage)
+        else:
+            lp.push(dt, 0)
+            lp.push(dt, 1)
         lp.spectral_update(dt)
 
     for _ in range(args.warmup):
@@ -408,7 +414,7 @@ def run_ours(args):
                 "share_of_step": spec_ms / ms if ms else None}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, args.staged),
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, ("lp_push_rk3(0..2)" if args.pusher == "rk3" else "lp_push(0), lp_push(1)") if args.staged else False),
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
            "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],
                     "sorts_total": d["sorts"]}}
