@@ -13,8 +13,8 @@
 //    (cp.async.bulk + mbarrier).  Measured on B200: phase 1 is a chain of dependent gathers (latency)
 //    and phase 2 a stream (HBM); run by the same warp one after the other their times add, run by
 //    different warps they overlap.
-//  * lp_spectral_direct_kernel (N_b = 512): rows go global -> registers -> global; this bin count
-//    is bound by the dependent fp64 chain of its ~10 substeps per row, not by HBM.
+//  * lp_spectral_direct_kernel (N_b = 512, 16 bins per lane): every warp does both phases; rows move with
+//    coalesced accesses through a transposing staging buffer, one row fetched ahead.
 // sm_100a.
 #include "lp_device.cuh"
 
@@ -158,25 +158,47 @@ __device__ __forceinline__ void lp_store_row(double *__restrict__ dst, const dou
 }
 
 // Per-lane slice of the bin table: edges E[sub*M .. sub*M+M] and 1/dE of the lane's M bins, held in
-// registers (IN_REGS) or re-read from shared memory at each use (large M).
+// registers (IN_REGS) or re-read from shared memory at each use (large M).  In shared memory the slices
+// are stored lane-interleaved (entry i of lane `sub` at [i*32 + sub]): a straight copy of the table would
+// put the lanes' slices M*8 bytes apart, i.e. all in the same banks (measured at M = 16: the kernel was
+// bound by these 32-way conflicts, l1tex at 94 %).
 template <int M, bool IN_REGS>
 struct LpLaneTab {
     double rE[IN_REGS ? M + 1 : 1], rR[IN_REGS ? M : 1];
     const double *pE, *pR;
+    // sE, sR: the plain tables (IN_REGS) or the lane-interleaved ones (lp_fill_interleaved)
     __device__ __forceinline__ void init(const double *sE, const double *sR, int sub)
     {
-        pE = sE + sub * M;
-        pR = sR + sub * M;
         if (IN_REGS) {
 #pragma unroll
-            for (int i = 0; i <= M; ++i) rE[i] = pE[i];
+            for (int i = 0; i <= M; ++i) rE[i] = sE[sub * M + i];
 #pragma unroll
-            for (int i = 0; i < M; ++i) rR[i] = pR[i];
+            for (int i = 0; i < M; ++i) rR[i] = sR[sub * M + i];
+            pE = pR = nullptr;
+        } else {
+            pE = sE + sub;
+            pR = sR + sub;
         }
     }
-    __device__ __forceinline__ double E(int i) const { return IN_REGS ? rE[i] : pE[i]; }
-    __device__ __forceinline__ double R(int i) const { return IN_REGS ? rR[i] : pR[i]; }
+    __device__ __forceinline__ double E(int i) const { return IN_REGS ? rE[i] : pE[i * 32]; }
+    __device__ __forceinline__ double R(int i) const { return IN_REGS ? rR[i] : pR[i * 32]; }
 };
+
+// lane-interleaved copies of the bin table for LpLaneTab<M, false>: tE[(M+1)*32], tR[M*32]
+template <int M>
+__device__ __forceinline__ void lp_fill_interleaved(const double *tab, int nb, double *tE, double *tR, int tid, int nthreads)
+{
+    for (int k = tid; k < (M + 1) * 32; k += nthreads) {
+        const int i = k >> 5, lane = k & 31;
+        const int e = lane * M + i;
+        tE[k] = e <= nb ? tab[e] : 0.0;
+    }
+    for (int k = tid; k < M * 32; k += nthreads) {
+        const int i = k >> 5, lane = k & 31;
+        const int b = lane * M + i;
+        tR[k] = b < nb ? tab[(nb + 1) + nb + b] : 0.0;
+    }
+}
 
 // Phase 2 for one row held as M bins per lane over G lanes (32/G rows per warp at once).
 // Donor-cell upwind:
@@ -392,9 +414,56 @@ __device__ __forceinline__ int lp_group_max(int n)
     return n;
 }
 
+// Row <-> lane slices through a per-warp staging buffer, for M >= 8 bins per lane.  A lane's slice is M*8
+// bytes of the row, so loading it directly makes every 16-byte load instruction of the warp touch 32
+// different 128-byte lines (measured at M = 16: ~500 L1 wavefronts per row, the kernel's bound after the
+// table fix).  Instead the warp moves the row with fully coalesced 16-byte accesses and transposes in shared
+// memory; slices are padded by 16 bytes so that both sides are free of bank conflicts.
+template <int M>
+struct LpStage {
+    static constexpr int kSliceBytes = M * 8 + 16;                 // padded slice of one lane
+    static constexpr int kBytes = 32 * kSliceBytes;
+    // 16-byte unit e of the row (0 .. 2M*... ) lives at:
+    static __device__ __forceinline__ int unit_offset(int e) { return (e / (M / 2)) * kSliceBytes + (e % (M / 2)) * 16; }
+
+    // the row's coalesced 16-byte pieces into registers (issued early: a row ahead of its use)
+    static __device__ __forceinline__ void fetch(const double *__restrict__ grow, int lane, double2 (&t)[M / 2])
+    {
+#pragma unroll
+        for (int k = 0; k < M / 2; ++k) t[k] = *reinterpret_cast<const double2 *>(grow + 2 * (k * 32 + lane));
+    }
+    // fetched pieces -> this lane's slice
+    static __device__ __forceinline__ void place(const double2 (&t)[M / 2], unsigned char *stage, int lane, double (&v)[M])
+    {
+#pragma unroll
+        for (int k = 0; k < M / 2; ++k) *reinterpret_cast<double2 *>(stage + unit_offset(k * 32 + lane)) = t[k];
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < M / 2; ++j) {
+            const double2 u = *reinterpret_cast<const double2 *>(stage + lane * kSliceBytes + j * 16);
+            v[2 * j] = u.x;
+            v[2 * j + 1] = u.y;
+        }
+        __syncwarp();
+    }
+    static __device__ __forceinline__ void store(double *__restrict__ grow, unsigned char *stage, int lane,
+                                                 const double (&v)[M])
+    {
+#pragma unroll
+        for (int j = 0; j < M / 2; ++j)
+            *reinterpret_cast<double2 *>(stage + lane * kSliceBytes + j * 16) = make_double2(v[2 * j], v[2 * j + 1]);
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < M / 2; ++k)
+            *reinterpret_cast<double2 *>(grow + 2 * (k * 32 + lane)) =
+                *reinterpret_cast<const double2 *>(stage + unit_offset(k * 32 + lane));
+        __syncwarp();
+    }
+};
+
 // ------------------------------------------------------------------ direct mover (N_b >= 256)
 
-constexpr int kDirectThreads = 256;
+constexpr int kDirectThreads = 128;
 constexpr int kDirectWarps = kDirectThreads / 32;
 
 template <int NB, bool DIAG, bool FUSED>
@@ -415,8 +484,19 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
     __syncthreads();
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    LpLaneTab<M, (M <= 4)> tab;
-    tab.init(sE, sR, lane);
+    constexpr bool kTabRegs = (M <= 4);
+    constexpr bool kStaged = (M >= 8);           // rows through the transposing staging buffer
+    static_assert(!kStaged || U == 1, "the staged path keeps one row ahead");
+    __shared__ __align__(16) unsigned char sStage[kDirectWarps][kStaged ? LpStage<M>::kBytes : 16];
+    __shared__ double sET[kTabRegs ? 1 : (M + 1) * 32];
+    __shared__ double sRT[kTabRegs ? 1 : M * 32];
+    if (!kTabRegs) {
+        lp_fill_interleaved<M>(A.tab, NB, sET, sRT, threadIdx.x, kDirectThreads);
+        __syncthreads();
+    }
+    LpLaneTab<M, kTabRegs> tab;
+    if (kTabRegs) tab.init(sE, sR, lane);
+    else tab.init(sET, sRT, lane);
 
     const long long nchunks = (A.np + 31) >> 5;
     const long long gw = (long long)blockIdx.x * kDirectWarps + warp;
@@ -427,14 +507,24 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
         const bool have = base + lane < A.np;
         const double px = have ? A.xin[base + lane] : 0.0, py = have ? A.yin[base + lane] : 0.0,
                      pz = have ? A.zin[base + lane] : 0.0;
+        double2 ahead[kStaged ? M / 2 : 1];                 // (staged, U == 1) the next row, fetched a row ahead
+        if constexpr (kStaged) {
+            if (base < A.np) LpStage<M>::fetch(A.chi_in + base * NB, lane, ahead);      // flies during phase 1
+        }
         lp_chunk_phase1<NB, FUSED>(A, base, lane, px, py, pz, sE, sR, sAC[warp], sNS[warp]);
         for (int j0 = 0; j0 < 32; j0 += U) {
             double buf[U][M];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const long long pj = base + j0 + u;
-                if (pj < A.np) lp_load_row<M>(A.chi_in + pj * NB + lane * M, buf[u]);
-                else {
+                if (pj < A.np) {
+                    if constexpr (kStaged) {
+                        LpStage<M>::place(ahead, sStage[warp], lane, buf[u]);
+                        if (j0 + 1 < 32 && pj + 1 < A.np) LpStage<M>::fetch(A.chi_in + (pj + 1) * NB, lane, ahead);
+                    } else {
+                        lp_load_row<M>(A.chi_in + pj * NB + lane * M, buf[u]);
+                    }
+                } else {
 #pragma unroll
                     for (int i = 0; i < M; ++i) buf[u][i] = 0.0;
                 }
@@ -458,7 +548,8 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
                 const long long pj = base + j0 + u;
                 const double lost = DIAG ? row[u].lost(lane) : 0.0;
                 if (pj < A.np) {
-                    lp_store_row<M>(A.chi_out + pj * NB + lane * M, row[u].chi);
+                    if constexpr (kStaged) LpStage<M>::store(A.chi_out + pj * NB, sStage[warp], lane, row[u].chi);
+                    else lp_store_row<M>(A.chi_out + pj * NB + lane * M, row[u].chi);
                     if (DIAG && lane == 0) {
                         A.lost_ws[pj] = lost;
                         if (A.lost_user) A.lost_user[pj] = lost;
@@ -595,9 +686,6 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #ifndef LP_BULK_RI
 #define LP_BULK_RI 1            // rows a lane group advances together (ILP)
 #endif
-#ifndef LP_BULK_TAB_REGS
-#define LP_BULK_TAB_REGS 1      // per-lane bin table in registers (1) or re-read from shared memory (0)
-#endif
 
 template <int NB>
 struct LpBulkCfg {
@@ -697,7 +785,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
     unsigned char *my_ring = sm + (size_t)rw * S * C::SLOT_BYTES;
     const uint32_t ring_u32 = lp_smem_u32(my_ring);
     const uint32_t bar_u32 = lp_smem_u32(bars + rw * S);
-    LpLaneTab<M, (LP_BULK_TAB_REGS != 0 && M <= 8)> tab;
+    LpLaneTab<M, true> tab;             // (from shared memory it measured 13 % slower)
     tab.init(sE, sR, sub);
 
     // this warp's chunks: t = rw, rw + NR, ... (nmy of them); its ring slots ("groups") are numbered
