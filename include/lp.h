@@ -149,6 +149,15 @@ LP_API lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void 
  * Particles_Boundary); LP_ERR_STATE if there is no such marking.  Synchronises `stream`. */
 LP_API lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new /*host*/, void *stream);
 
+/* Particle count within the capacity given to lp_create (config.np at creation): particles are injected by
+ * writing them behind the current ones in the bound arrays and raising the count; lp_compact lowers it.
+ * The paper sizes its containers in chunks of L = 2^e particles so that growth rarely reallocates
+ * (Listing 1: N_c = (N >> e) + (N % L == 0 ? 0 : 1); e = 18 in Listing 3):
+ * lp_chunked_capacity returns N_c * L, the capacity to create the context and the arrays with.
+ * Per-particle results of earlier calls (n_sub, lost, push stages) are invalidated by lp_set_count. */
+LP_API lp_status lp_chunked_capacity(int64_t n, int32_t e, int64_t *capacity /*host*/);
+LP_API lp_status lp_set_count(lp_ctx *ctx, int64_t np_new);
+
 /* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
  * spectral update (order of Table 1, without the fluid stages). */
 LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);

@@ -17,7 +17,7 @@ _STATUS_NAMES = {0: "LP_OK", -1: "LP_ERR_INVALID_ARG", -2: "LP_ERR_STATE", -3: "
 EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp_bind_workspace",
            "lp_bind_particles", "lp_bind_diag", "lp_set_fields", "lp_interpolate", "lp_sort", "lp_push",
            "lp_spectral_update", "lp_step", "lp_step_host", "lp_get_diag", "lp_launch_count", "lp_get_bins",
-           "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3")
+           "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3", "lp_chunked_capacity", "lp_set_count")
 
 
 class LPError(RuntimeError):
@@ -77,6 +77,8 @@ def load():
     lib.lp_shock_update.argtypes = [vp, vp, C.c_double, vp]
     lib.lp_compact.argtypes = [vp, vp, C.POINTER(C.c_int64), vp]
     lib.lp_push_rk3.argtypes = [vp, C.c_double, C.c_int, vp]
+    lib.lp_chunked_capacity.argtypes = [C.c_int64, C.c_int32, C.POINTER(C.c_int64)]
+    lib.lp_set_count.argtypes = [vp, C.c_int64]
     lib.lp_step_host.argtypes = [vp, C.c_double, dp, dp, dp, dp, dp, vp]
     lib.lp_get_diag.argtypes = [vp, C.POINTER(lp_diag), vp]
     lib.lp_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
@@ -172,6 +174,18 @@ def lp_spectral_update(ctx, dt, stream=None):
 
 def lp_shock_update(ctx, r_ptr, q_r, stream=None):
     _check(ctx, load().lp_shock_update(ctx, r_ptr, float(q_r), stream))
+
+
+def lp_chunked_capacity(n, e=18):
+    cap = C.c_int64()
+    st = load().lp_chunked_capacity(int(n), int(e), C.byref(cap))
+    if st != LP_OK:
+        raise LPError(st)
+    return int(cap.value)
+
+
+def lp_set_count(ctx, n):
+    _check(ctx, load().lp_set_count(ctx, int(n)))
 
 
 def lp_push_rk3(ctx, dt, stage, stream=None):

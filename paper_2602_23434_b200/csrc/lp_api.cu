@@ -570,6 +570,27 @@ lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *st
     return LP_OK;
 }
 
+lp_status lp_chunked_capacity(int64_t n, int32_t e, int64_t *capacity)
+{
+    if (!capacity || n < 0 || e < 0 || e > 40) return LP_ERR_INVALID_ARG;
+    const int64_t len = (int64_t)1 << e;
+    const int64_t nc = (n >> e) + (n % len == 0 ? 0 : 1);          // Listing 1
+    *capacity = nc << e;
+    return LP_OK;
+}
+
+lp_status lp_set_count(lp_ctx *ctx, int64_t np_new)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (np_new < 0 || np_new > ctx->capacity) return fail(ctx, LP_ERR_INVALID_ARG, "count outside [0, capacity of lp_create]");
+    if (np_new > 0 && ctx->ws && !ctx->x) return fail(ctx, LP_ERR_STATE, "no particles bound (lp_bind_particles)");
+    ctx->cfg.np = np_new;
+    ctx->stage0_done = false; ctx->rk3_next = 0;
+    ctx->spectra_done = false;
+    ctx->status_valid = false;
+    return LP_OK;
+}
+
 lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
 {
     lp_status st = need_ready(ctx, true);

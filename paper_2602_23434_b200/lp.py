@@ -93,6 +93,10 @@ class LP:
         assert r.is_cuda and r.dtype == self.x.dtype and r.numel() == self.x.numel() and r.is_contiguous()
         B.lp_shock_update(self.ctx, r.data_ptr(), q_r, self.stream)
 
+    def set_count(self, n):
+        """Use the first n particles of the bound arrays (n <= the capacity the context was created with)."""
+        B.lp_set_count(self.ctx, n)
+
     def compact(self, flag=None):
         """Delete the flagged particles (int32 CUDA tensor [np], nonzero = delete; None = those outside the
         box after the last push) and fill the holes from the tail; returns the new particle count.  The

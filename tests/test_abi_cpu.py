@@ -20,7 +20,7 @@ def declared_symbols():
 def test_library_exports_every_declared_symbol():
     lib = B.load()
     names = declared_symbols()
-    assert len(names) == 23 and set(names) == set(B.EXPORTS)
+    assert len(names) == 25 and set(names) == set(B.EXPORTS)
     for n in names:
         assert getattr(lib, n) is not None
 
@@ -136,3 +136,25 @@ def test_cfl_candidate_bins_carry_the_maximum(nbins, e_min, e_max):
         lam_all = out.max()
         lam_cand = out[cand].max()
         assert lam_all <= lam_cand * (1 + 1e-15), (a, cr, int(out.argmax()), cand)
+
+
+@pytest.mark.parametrize("n,e,cap", [(0, 18, 0), (1, 18, 262144), (262144, 18, 262144), (262145, 18, 524288),
+                                     (16777216, 18, 16777216), (1000, 4, 1008), (1024, 4, 1024)])
+def test_chunked_capacity_is_listing_1(n, e, cap):
+    """Listing 1: N_c = (N >> e) + (N % L == 0 ? 0 : 1) chunks of L = 2^e."""
+    assert B.lp_chunked_capacity(n, e) == cap
+    assert cap % (1 << e) == 0 and cap >= n and cap - n < (1 << e)
+
+
+def test_set_count_stays_within_capacity():
+    lib = B.load()
+    c = cfg()
+    ctx = C.c_void_p()
+    st = lib.lp_create(C.byref(c), C.byref(ctx))
+    assert ctx and st in (B.LP_OK, B.LP_ERR_CUDA)
+    try:
+        assert lib.lp_set_count(ctx, C.c_int64(c.np + 1)) == B.LP_ERR_INVALID_ARG
+        assert lib.lp_set_count(ctx, C.c_int64(-1)) == B.LP_ERR_INVALID_ARG
+        assert lib.lp_set_count(ctx, C.c_int64(0)) == B.LP_OK
+    finally:
+        lib.lp_destroy(ctx)

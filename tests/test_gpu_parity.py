@@ -275,6 +275,30 @@ def test_compact_outflow_deletes_what_left_the_box():
         lp.compact()
 
 
+def test_injection_within_capacity():
+    """Particles are injected by writing them behind the current ones and raising the count
+    (lp_set_count): a step on the first 3000, then on all 5000."""
+    w = small_turbulent(np_=5000, nbins=32)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+    n0 = 3000
+    lp.set_count(n0)
+    lp.step(w.dt)
+    xa, ya, za, chia, nsub, lost, st = orc.step(prm, f_np, x[:n0], y[:n0], z[:n0], w.dt, chi[:n0], nthreads=8)
+    assert lp.diag()["np"] == n0
+    assert np.array_equal(host(lp.x)[:n0], xa) and np.array_equal(host(lp.x)[n0:], x[n0:])      # the tail is untouched
+    assert np.array_equal(host(lp.chi)[n0:], chi[n0:])
+    lp.set_count(w.np)
+    lp.step(w.dt)
+    x2 = np.concatenate([xa, x[n0:]]); y2 = np.concatenate([ya, y[n0:]]); z2 = np.concatenate([za, z[n0:]])
+    chi2 = np.concatenate([chia, chi[n0:]])
+    xb, yb, zb, chib, nsub, lost, st = orc.step(prm, f_np, x2, y2, z2, w.dt, chi2, nthreads=8)
+    assert np.array_equal(host(lp.x), xb) and np.array_equal(host(lp.z), zb)
+    assert_nsub_equal(host(lp.nsub), nsub)
+    assert_chi_close(host(lp.chi), chib)
+    with pytest.raises(P.binding.LPError):
+        lp.set_count(w.np + 1)
+
+
 # ------------------------------------------------------------------ whole step, with re-sort
 
 @pytest.mark.parametrize("nbins,np_", [(64, 6000 + 3), (16, 2500), (128, 1500)])
