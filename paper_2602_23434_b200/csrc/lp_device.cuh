@@ -8,8 +8,6 @@
 #include <cuda_runtime.h>
 #include "lp_internal.h"
 
-__device__ __forceinline__ double2 ldg2(const double *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
-
 // floor-mod for an index far outside the grid (kept out of line: the integer division is long)
 static __device__ __noinline__ int lp_wrap_far(int i, int n)
 {

@@ -633,6 +633,9 @@ __device__ __forceinline__ void lp_bulk_wait_all() { asm volatile("cp.async.bulk
 __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // Tunables of the bulk mover (overridable at compile time for sweeps; defaults = measured best).
+// LP_DEBUG_SKIP_PHASE1 / LP_DEBUG_SKIP_ROWS (never defined in the product build) time one kind of warp alone:
+// the first replaces the per-particle phase by constants (results are then meaningless), the second skips
+// the row stream.  profiles/r01_spectral_full.md quotes the timings they gave.
 #ifndef LP_BULK_MINB
 #define LP_BULK_MINB 1          // resident blocks per SM the register allocation is bounded for
 #endif
