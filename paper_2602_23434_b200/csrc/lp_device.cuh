@@ -86,10 +86,15 @@ __device__ __forceinline__ double lp_acc(double acc, double w, double q) { retur
 // the L1 request count of the gather (the per-particle phase is bound by L1 requests, one per lane
 // and divergent address, not by bytes).
 struct LpRec { double a, b, c, d; };
+// The load carries an L2 evict-last policy: a cell's record is needed again by the particles of the
+// neighbouring rows and planes, long after the row stream (evict-first, lp_spectral.cu) has passed.
 __device__ __forceinline__ LpRec lp_ldg_rec(const double4 *p)
 {
     LpRec r;
-    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.a), "=d"(r.b), "=d"(r.c), "=d"(r.d) : "l"(p));
+    unsigned long long pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm("ld.global.nc.L2::cache_hint.v4.f64 {%0,%1,%2,%3}, [%4], %5;"
+        : "=d"(r.a), "=d"(r.b), "=d"(r.c), "=d"(r.d) : "l"(p), "l"(pol));
     return r;
 }
 
