@@ -922,14 +922,20 @@ int launch_variant(const LpSpectralArgs &a, int sm_count, cudaStream_t s)
     if constexpr (NB <= LP_BULK_MAX_NB) {
         using C = LpBulkCfg<NB>;
         auto kernel = lp_spectral_bulk_kernel<NB, DIAG, FUSED>;
-        static bool configured = false;
-        if (!configured) {
+        // function attributes are per device: set them once on each device this kernel is launched on
+        static bool configured[64] = {};
+        static int blocks_per_sm[64] = {};
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+        const int slot = dev & 63;
+        if (!configured[slot]) {
             if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_TOTAL) != cudaSuccess) return -1;
             if (cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, LP_BULK_CARVEOUT) != cudaSuccess) return -1;
-            configured = true;
+            blocks_per_sm[slot] = lp_blocks_per_sm(kernel, C::THREADS, C::SMEM_TOTAL);
+            configured[slot] = true;
         }
         const long long want = nchunks;                      // a block takes whole chunks
-        const long long cap = (long long)sm_count * lp_blocks_per_sm(kernel, C::THREADS, C::SMEM_TOTAL);
+        const long long cap = (long long)sm_count * blocks_per_sm[slot];
         int blocks = (int)(want < cap ? want : cap);
         if (blocks < 1) blocks = 1;
         kernel<<<blocks, C::THREADS, C::SMEM_TOTAL, s>>>(a);
