@@ -37,6 +37,7 @@ def parse():
     ap.add_argument("--nbins", type=int, default=0, help="override the bin count (workload 5 sweep)")
     ap.add_argument("--np", type=int, default=0, help="override the particle count (debugging only)")
     ap.add_argument("--grid", type=int, default=0, help="override the cells per axis (debugging only)")
+    ap.add_argument("--sort-every", type=int, default=-1, help="override the workload's re-sort period (0 = never)")
     ap.add_argument("--staged", action="store_true",
                     help="time the staged calls (lp_push 0, lp_push 1, lp_spectral_update) instead of the fused lp_step")
     ap.add_argument("--shock-frac", type=float, default=0.0,
@@ -121,6 +122,8 @@ def pick_workload(args):
         kw["np"] = args.np
     if args.grid:
         kw["n"] = args.grid
+    if args.sort_every >= 0:
+        kw["sort_every"] = args.sort_every
     return w.scaled(**kw) if kw else w
 
 
