@@ -20,6 +20,8 @@
  *    The library allocates only small tables itself; bulk scratch is the caller's workspace.
  *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls only enqueue
  *    work on it and return; lp_get_diag and the *_host call are the ones that synchronise.
+ *  - A context is not thread-safe: one host thread at a time per context (several contexts, on one or
+ *    several devices, may be used concurrently).
  *  - Every function returns an lp_status; nothing aborts, throws or prints.
  *    lp_last_error gives a human-readable detail for the last failure on that context.
  */
