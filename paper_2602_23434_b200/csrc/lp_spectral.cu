@@ -461,7 +461,7 @@ struct LpStage {
     }
 };
 
-// ------------------------------------------------------------------ direct mover (N_b >= 256)
+// ------------------------------------------------------------------ direct mover (N_b = 512)
 
 constexpr int kDirectThreads = 128;
 constexpr int kDirectWarps = kDirectThreads / 32;
@@ -561,7 +561,7 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
     }
 }
 
-// ------------------------------------------------------------------ TMA bulk mover (N_b <= 128)
+// ------------------------------------------------------------------ TMA bulk mover (N_b <= 256)
 
 __device__ __forceinline__ uint32_t lp_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -590,9 +590,6 @@ __device__ __forceinline__ void lp_mbar_wait(uint32_t bar, uint32_t parity)
                      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
                      "selp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(done) : "r"(bar), "r"(parity), "r"((uint32_t)LP_MBAR_SUSPEND_NS) : "memory");
-#ifdef LP_MBAR_SLEEP_NS
-        if (!done) __nanosleep(LP_MBAR_SLEEP_NS);
-#endif
     } while (!done);
 }
 // L2 eviction policy for the row stream: rows are touched once per step, the grid records many times
