@@ -530,19 +530,31 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
                 }
             }
             LpRow<M, G, DIAG> row[U];
+            double2 ac[U];
+            int nsr[U];
             int nmax = 0, nmin = 0x7fffffff;
+            bool cool = true;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int r = j0 + u;
-                const double2 ac = sAC[warp][r];
-                const int ns = abs(sNS[warp][r]);
+                ac[u] = sAC[warp][r];
+                const int nsv = sNS[warp][r];              // (warp-uniform: every lane reads the same entries)
+                cool = cool && nsv <= 0;
+                nsr[u] = abs(nsv);
 #pragma unroll
                 for (int i = 0; i < M; ++i) row[u].chi[i] = buf[u][i];
-                row[u].setup(tab, ac.x, ac.y, ns, lane);
-                nmax = max(nmax, ns);
-                nmin = min(nmin, ns);
+                nmax = max(nmax, nsr[u]);
+                nmin = min(nmin, nsr[u]);
             }
-            lp_rows_substeps<false, U, M, G, DIAG>(row, nmin, nmax);
+            if (cool) {                                     // every row in flight is a cooling row
+#pragma unroll
+                for (int u = 0; u < U; ++u) row[u].setup_cool(tab, ac[u].x, ac[u].y, nsr[u], lane);
+                lp_rows_substeps<true, U, M, G, DIAG>(row, nmin, nmax);
+            } else {
+#pragma unroll
+                for (int u = 0; u < U; ++u) row[u].setup(tab, ac[u].x, ac[u].y, nsr[u], lane);
+                lp_rows_substeps<false, U, M, G, DIAG>(row, nmin, nmax);
+            }
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const long long pj = base + j0 + u;
