@@ -306,6 +306,7 @@ lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
     b.idx_b = c->at<uint32_t>(c->lay.idx_b);
     b.hist = c->at<uint32_t>(c->lay.hist);
     b.hist_elems = c->lay.hist_elems;
+    b.digit = c->at<uint8_t>(c->lay.lost);          // the per-particle `lost` buffer is dead across a re-sort
     uint32_t *perm = nullptr;
     lp_status st = count(c, lp_launch_sort_perm(c->geom, c->x, c->y, c->z, c->id, np, c->id_bits, c->key_bits, b, &perm, s),
                          "sort kernels launch");

@@ -95,6 +95,7 @@ struct LpSortBufs {
     uint32_t *idx_b;     // [np]
     uint32_t *hist;      // [256 * nblocks]
     size_t hist_elems;
+    uint8_t *digit;      // [np] digit of every element of the current pass (hist kernel -> scatter kernel)
 };
 size_t lp_sort_hist_elems(long long np);
 int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const double *z,

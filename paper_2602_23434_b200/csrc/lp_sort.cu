@@ -34,7 +34,7 @@ __device__ __forceinline__ uint32_t lp_digit(const uint32_t *idx_in, const uint6
 __global__ void __launch_bounds__(kThreads)
 lp_radix_hist_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__restrict__ id,
                      const uint32_t *__restrict__ key, long long np, int use_key, int shift,
-                     uint32_t *__restrict__ hist, int nblocks)
+                     uint32_t *__restrict__ hist, int nblocks, uint8_t *__restrict__ digit)
 {
     __shared__ uint32_t sh[256];
     sh[threadIdx.x] = 0;
@@ -44,7 +44,9 @@ lp_radix_hist_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__rest
         long long e = t0 + r * kThreads + threadIdx.x;
         if (e < np) {
             uint32_t src;
-            atomicAdd(&sh[lp_digit(idx_in, id, key, e, use_key, shift, src)], 1u);
+            const uint32_t d = lp_digit(idx_in, id, key, e, use_key, shift, src);
+            digit[e] = (uint8_t)d;              // kept for the scatter pass: one gather through the permutation, not two
+            atomicAdd(&sh[d], 1u);
         }
     }
     __syncthreads();
@@ -88,7 +90,7 @@ __global__ void __launch_bounds__(kThreads)
 lp_radix_scatter_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__restrict__ id,
                         const uint32_t *__restrict__ key, long long np, int use_key, int shift,
                         const uint32_t *__restrict__ hist, const uint32_t *__restrict__ totals, int nblocks,
-                        uint32_t *__restrict__ idx_out)
+                        uint32_t *__restrict__ idx_out, const uint8_t *__restrict__ digit)
 {
     __shared__ uint32_t base[256];
     __shared__ uint32_t wcount[kWarps][256];
@@ -116,7 +118,10 @@ lp_radix_scatter_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__r
         const long long e = t0 + r * kThreads + t;
         const bool valid = e < np;
         uint32_t src = 0, d = 256u + lane;          // invalid lanes get distinct pseudo-digits
-        if (valid) d = lp_digit(idx_in, id, key, e, use_key, shift, src);
+        if (valid) {
+            src = idx_in ? idx_in[e] : (uint32_t)e;
+            d = digit[e];                        // written by lp_radix_hist_kernel of this pass
+        }
         const unsigned same = __match_any_sync(kFull, d);
         const int rank = __popc(same & ((1u << lane) - 1u));
         if (valid && rank == 0) wcount[warp][d] = __popc(same);
@@ -274,10 +279,11 @@ int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const
     for (int pass = 0; pass < (total > 0 ? total : 1); ++pass) {
         const int use_key = pass >= id_passes ? 1 : 0;
         const int shift = 8 * (use_key ? pass - id_passes : pass);
-        lp_radix_hist_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, nblocks);
+        lp_radix_hist_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, nblocks, b.digit);
         uint32_t *totals = b.hist + (size_t)256 * nblocks;
         lp_scan_rows_kernel<<<256, kThreads, 0, s>>>(b.hist, nblocks, totals);
-        lp_radix_scatter_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, totals, nblocks, bufs[cur]);
+        lp_radix_scatter_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, totals, nblocks, bufs[cur],
+                                                             b.digit);
         launches += 3;
         in = bufs[cur];
         cur ^= 1;
