@@ -143,7 +143,7 @@ lp_permute_f64_kernel(const uint32_t *__restrict__ perm, const double *__restric
                       double *__restrict__ dst, long long np)
 {
     long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p < np) dst[p] = src[perm[p]];
+    if (p < np) __stcs(dst + p, src[perm[p]]);
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -151,7 +151,7 @@ lp_permute_u64_kernel(const uint32_t *__restrict__ perm, const uint64_t *__restr
                       uint64_t *__restrict__ dst, long long np)
 {
     long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p < np) dst[p] = src[perm[p]];
+    if (p < np) __stcs(dst + p, src[perm[p]]);
 }
 
 // one warp (or half warp for 16 bins) moves one row of nbins doubles with 16-byte accesses
@@ -170,7 +170,7 @@ lp_permute_rows_kernel(const uint32_t *__restrict__ perm, const double *__restri
         if (r >= np) continue;
         const double2 *s = reinterpret_cast<const double2 *>(src + (long long)perm[r] * nbins);
         double2 *d = reinterpret_cast<double2 *>(dst + r * nbins);
-        for (int i = sub; i < nbins / 2; i += lanes) d[i] = s[i];
+        for (int i = sub; i < nbins / 2; i += lanes) __stcs(d + i, __ldcs(s + i));      // touched once: streaming
     }
 }
 
