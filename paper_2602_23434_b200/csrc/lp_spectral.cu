@@ -77,8 +77,8 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
             pos[d] = xn;
         }
         px = pos[0]; py = pos[1]; pz = pos[2];
-        A.x[p] = px; A.y[p] = py; A.z[p] = pz;
-        A.status[p] = stt;
+        __stcs(A.x + p, px); __stcs(A.y + p, py); __stcs(A.z + p, pz);
+        __stcs(A.status + p, stt);
         lp_stencil(A.g, px, py, pz, st);
         ka.update(A.cells, st);
     } else {
@@ -397,8 +397,8 @@ __device__ __forceinline__ void lp_chunk_phase1(const LpSpectralArgs &A, long lo
 #else
         lp_phase1<NB, FUSED>(A, p, px, py, pz, sE, sR, c, nss);
 #endif
-        A.nsub_ws[p] = nss;
-        if (A.nsub_user) A.nsub_user[p] = nss;
+        __stcs(A.nsub_ws + p, nss);
+        if (A.nsub_user) __stcs(A.nsub_user + p, nss);
     }
     sAC[lane] = make_double2(c.a2, c.cr2);
     sNS[lane] = c.cool ? -c.ns : c.ns;          // the sign carries the cooling flag to the row warps
@@ -775,7 +775,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
         double nx = 0.0, ny = 0.0, nz = 0.0;
         if ((uint32_t)warp < nblk && chunk_of(warp) + lane < np) {
             const size_t p = (size_t)chunk_of(warp) + lane;
-            nx = A.xin[p]; ny = A.yin[p]; nz = A.zin[p];
+            nx = __ldcs(A.xin + p); ny = __ldcs(A.yin + p); nz = __ldcs(A.zin + p);   // touched once: streaming
         }
 #pragma unroll 1
         for (uint32_t t = warp; t < nblk; t += NP) {
@@ -784,7 +784,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
             const double px = nx, py = ny, pz = nz;
             if (t + NP < nblk && chunk_of(t + NP) + lane < np) {
                 const size_t p = (size_t)chunk_of(t + NP) + lane;
-                nx = A.xin[p]; ny = A.yin[p]; nz = A.zin[p];
+                nx = __ldcs(A.xin + p); ny = __ldcs(A.yin + p); nz = __ldcs(A.zin + p);   // touched once: streaming
             }
             if (use >= 1) lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u);
             lp_chunk_phase1<NB, FUSED>(A, (long long)base, lane, px, py, pz, sE, sR, sAC + cs * 32, sNS + cs * 32);
