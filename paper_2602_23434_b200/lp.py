@@ -96,6 +96,7 @@ class LP:
     def set_count(self, n):
         """Use the first n particles of the bound arrays (n <= the capacity the context was created with)."""
         B.lp_set_count(self.ctx, n)
+        self.cfg.np = n            # (the binding's copy of the count sizes the outputs of interpolate)
 
     def compact(self, flag=None):
         """Delete the flagged particles (int32 CUDA tensor [np], nonzero = delete; None = those outside the
@@ -103,7 +104,9 @@ class LP:
         tensors keep their size: the first `count` entries are the particles."""
         if flag is not None:
             assert flag.is_cuda and flag.dtype == torch.int32 and flag.is_contiguous()
-        return B.lp_compact(self.ctx, flag.data_ptr() if flag is not None else None, self.stream)
+        n = B.lp_compact(self.ctx, flag.data_ptr() if flag is not None else None, self.stream)
+        self.cfg.np = n
+        return n
 
     def step(self, dt):
         B.lp_step(self.ctx, dt, self.stream)
