@@ -392,3 +392,31 @@ def test_state_errors():
     lp.push(0.1, 0); lp.push(0.1, 1); lp.spectral_update(0.1)      # and the good order works
     torch.cuda.synchronize()
     assert lp.launch_count() >= 4
+
+
+# ------------------------------------------------------------------ seeded random configurations
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_small_configurations(seed):
+    """Ragged sizes against the ring / chunk / batch boundaries of the kernels: random particle counts, bin
+    counts, boundary kinds and re-sort periods; three fused steps, everything compared as in the other tests."""
+    rng = np.random.default_rng(1000 + seed)
+    np_ = int(rng.choice([1, 2, 31, 32, 33, 63, 65, 255, 257, 1023, 1025, 4095, 4129, int(rng.integers(1, 9000))]))
+    nbins = int(rng.choice([16, 32, 64, 128, 256, 512]))
+    periodic = tuple(int(v) for v in rng.integers(0, 2, 3))
+    sort_every = int(rng.choice([0, 1, 2]))
+    w = small_turbulent(n=int(rng.choice([4, 7, 12])), np_=np_, nbins=nbins, sort_every=sort_every).scaled(
+        periodic=periodic, dt=float(rng.choice([0.01, 0.05])))
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
+    for s in range(3):
+        lp.step(w.dt)
+        if sort_every and s % sort_every == 0:
+            x, y, z, pid, chi, _, _ = oracle_sort_state(prm, x, y, z, pid, chi)
+        x, y, z, chi, nsub, lost, st = orc.step(prm, f_np, x, y, z, w.dt, chi, nthreads=8)
+    torch.cuda.synchronize()
+    assert np.array_equal(host(lp.id).view(np.uint64), pid)
+    assert np.array_equal(host(lp.x), x) and np.array_equal(host(lp.y), y) and np.array_equal(host(lp.z), z)
+    assert_nsub_equal(host(lp.nsub), nsub)
+    assert_chi_close(host(lp.chi), chi)
+    d = lp.diag()
+    assert d["n_outside"] == int((st != 0).sum()) and d["np"] == np_
