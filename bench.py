@@ -413,6 +413,7 @@ def run_ours(args):
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "algorithmic_bytes_split": {"rows": rows_bytes, "state": state_bytes, "grid": grid_bytes},
                 "achieved_rows_only": (rows_bytes / (spec_avg_ms * 1e-3) / 1e9) if spec_n else None,
+                "frac_rows_only": (rows_bytes / (spec_avg_ms * 1e-3) / 1e9 / peak) if spec_n else None,
                 "avg_launch_ms": spec_avg_ms,
                 "share_of_step": spec_ms / ms if ms else None}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
