@@ -50,6 +50,10 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--repeats", type=int, default=5,
+                    help="timed passes of --steps in all (SURVEY.md 8(d): median of 5); `value` is the first one")
+    ap.add_argument("--no-parity", action="store_true", help="skip the oracle check of the timed state")
+    ap.add_argument("--parity-sample", type=int, default=2048)
     return ap.parse_args()
 
 
@@ -61,11 +65,12 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def stored_traffic(wname, nbins):
-    """dram bytes per spectral launch from the committed ncu --set full summary, or None."""
+def stored_traffic(wname, nbins, staged=False):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    ncu --set full captures (profiles/spectral_traffic.md names the command of every entry), or None."""
     p = os.path.join(ROOT, "profiles", "spectral_traffic.json")
     try:
-        return json.load(open(p)).get("%s/nb%d" % (wname, nbins))
+        return json.load(open(p)).get("%s/nb%d%s" % (wname, nbins, "/staged" if staged else ""))
     except Exception:
         return None
 
@@ -190,6 +195,8 @@ def oracle_steps(orc, prm, fields_np, st, dt, nsteps, sort_every, step0, threads
 
 
 def cpu_baseline(w, fields_np, u_rad, x, y, z, pid, chi_host_fn, dt, seconds):
+    """The oracle as it stands on the host cores, on bounded samples of the workload: the whole
+    step on all cores (the headline `value`), the whole step on one thread, and the spectral update alone."""
     threads = os.cpu_count() or 1
     ncal = min(w.np, 32768)
     orc, prm, st = oracle_state(w, fields_np, u_rad, x, y, z, pid, chi_host_fn(ncal), ncal)
@@ -199,9 +206,59 @@ def cpu_baseline(w, fields_np, u_rad, x, y, z, pid, chi_host_fn, dt, seconds):
     nsel = int(min(w.np, max(ncal, rate * seconds / nsteps)))
     orc, prm, st = oracle_state(w, fields_np, u_rad, x, y, z, pid, chi_host_fn(nsel), nsel)
     t = oracle_steps(orc, prm, fields_np, st, dt, nsteps, w.sort_every, 0, threads)
-    return {"value": nsel * nsteps / t, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": "first %d particles of the workload, %d steps (one sort), %.1f s, full %d^3 fields"
-                      % (nsel, nsteps, t, w.n)}
+    out = {"value": nsel * nsteps / t, "unit": UNIT, "cores": threads, "kind": "oracle",
+           "sample": "first %d particles of the workload, %d steps (one sort), %.1f s, full %d^3 fields"
+                     % (nsel, nsteps, t, w.n)}
+    # one thread: a third of the time budget
+    n1 = int(min(w.np, max(4096, rate / threads * seconds / 3)))
+    orc, prm, st = oracle_state(w, fields_np, u_rad, x, y, z, pid, chi_host_fn(n1), n1)
+    t1 = oracle_steps(orc, prm, fields_np, st, dt, 1, 0, 1, 1)
+    out["single_thread"] = {"value": n1 / t1, "unit": UNIT, "cores": 1,
+                            "sample": "first %d particles, 1 step, %.1f s" % (n1, t1)}
+    # Particles_Spectra alone (orc_spectral_update: gather, coefficients, n_sub, substeps), all cores
+    import numpy as np
+    ns = int(min(w.np, max(ncal, rate * seconds / 3)))
+    xs_, ys_, zs_ = (a[:ns] for a in (x, y, z))
+    t0 = time.perf_counter()
+    orc.spectral_update(prm, fields_np, xs_, ys_, zs_, np.ones(ns), dt, chi_host_fn(ns), nthreads=threads)
+    ts = time.perf_counter() - t0
+    out["spectral_update_only"] = {"value": ns / ts, "unit": "particle-updates/s", "cores": threads,
+                                   "sample": "first %d particles, 1 call of orc_spectral_update (rho_old = 1), %.1f s"
+                                             % (ns, ts)}
+    return out
+
+
+def parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_rows_fn, dt, nsteps, nsample, dev):
+    """The timed state against the oracle: a seeded sample of particles is replayed on the CPU for the
+    `nsteps` steps the GPU state has taken and compared by id (positions bit for bit, spectra relative).
+    fields_for_step(k) -> (fields at t^n, fields at t^{n+1}) as numpy, the same object twice when frozen."""
+    import numpy as np
+    import torch
+    from oracle import lp_oracle as orc
+    prm = orc.make_params(w.n, w.n, w.n, w.xlo, w.xhi, w.periodic, w.nbins, w.e_min, w.e_max,
+                          kappa=w.kappa, u_rad=u_rad, cfl_e=w.cfl_e, max_substeps=w.max_substeps)
+    sel = np.sort(np.random.default_rng(4321).choice(w.np, size=min(nsample, w.np), replace=False))
+    sx, sy, sz, sid, schi = x[sel].copy(), y[sel].copy(), z[sel].copy(), pid[sel].copy(), chi_rows_fn(sel)
+    nt = os.cpu_count() or 1
+    for k in range(nsteps):
+        f0, f1 = fields_for_step(k)
+        if f0 is f1:
+            sx, sy, sz, schi, nsub, lost, status = orc.step(prm, f0, sx, sy, sz, dt, schi, nthreads=nt)
+        else:
+            k1, rho_old, xs = orc.push_stage0(prm, f0, sx, sy, sz, dt, nthreads=nt)
+            sx, sy, sz, status = orc.push_stage1(prm, f1, sx, sy, sz, xs, k1, dt, nthreads=nt)
+            schi, nsub, lost = orc.spectral_update(prm, f1, sx, sy, sz, rho_old, dt, schi, nthreads=nt)
+    cx, cy, cz, cid, cchi = lp.current()
+    where = torch.empty(w.np, dtype=torch.int64, device=dev)
+    where[cid.view(torch.int64)] = torch.arange(w.np, dtype=torch.int64, device=dev)     # ids are 0 .. np-1
+    loc = where[torch.from_numpy(sid.astype(np.int64)).to(dev)]
+    gx, gy, gz = (t[loc].cpu().numpy() for t in (cx, cy, cz))
+    gchi = cchi[loc].cpu().numpy()
+    rel = np.abs(gchi - schi) / np.maximum(np.abs(schi), 1e-290)
+    return {"particles": int(sel.size), "steps": int(nsteps), "max_rel": float(rel.max()),
+            "positions_bit_exact": bool(np.array_equal(gx, sx) and np.array_equal(gy, sy) and np.array_equal(gz, sz)),
+            "tolerance": 1e-10, "ok": bool(rel.max() <= 1e-10 and np.array_equal(gx, sx)),
+            "against": "oracle/lp_oracle.c replaying the same steps on the sample (matched by id)"}
 
 
 # ------------------------------------------------------------------------------- inputs
@@ -223,6 +280,7 @@ def make_inputs(w, device):
     def chi_device():
         return (torch.from_numpy(amp).to(device)[:, None] * torch.from_numpy(row).to(device)[None, :]).contiguous()
 
+    chi_host.rows = lambda sel: amp[sel, None] * row[None, :]
     return fields, u_rad, x, y, z, pid, chi_host, chi_device
 
 
@@ -280,11 +338,21 @@ def run_ours(args):
     w = pick_workload(args)
     w = rank_workload(w, rank)
     dt = step_dt(w)
+    staged = args.staged or w.field_kind == "homologous"       # workload 2 re-sets its fields between the stages
+    args.staged = staged
     fields, u_rad, x, y, z, pid, chi_host, chi_device = make_inputs(w, dev)
     lp = P.LP(P.config_from_workload(w, u_rad=u_rad, device=local))
     lp.set_fields(fields)
     lp.bind_particles(x, y, z, pid, chi_device())
     B = P.binding
+    total_steps = args.warmup + args.steps * max(1, args.repeats)
+    field_at = None
+    if w.field_kind == "homologous":
+        # time-dependent fields (reading R18): the sets for every step boundary are made before the timed
+        # region, lp_set_fields (the repack kernel) runs inside it, as in the paper's step
+        import lp_inputs as I
+        field_sets = [I.make_fields(w, t=k * dt, device=dev) for k in range(total_steps + 1)]
+        field_at = lambda k: field_sets[k]
 
     def barrier():
         if dist is not None:
@@ -294,42 +362,75 @@ def run_ours(args):
     nstep = [0]
 
     def one_step():
-        if not args.staged:
+        k = nstep[0]
+        nstep[0] += 1
+        if not staged:
             lp.step(dt)
             return
-        if w.sort_every and nstep[0] % w.sort_every == 0:
+        if w.sort_every and k % w.sort_every == 0:
             lp.sort()
-        nstep[0] += 1
+        if field_at is not None:
+            lp.set_fields(field_at(k))
         if args.pusher == "rk3":
             for stage in range(3):
+                if stage == 1 and field_at is not None:
+                    lp.set_fields(field_at(k + 1))
                 lp.push_rk3(dt, stage)
         else:
             lp.push(dt, 0)
+            if field_at is not None:
+                lp.set_fields(field_at(k + 1))
             lp.push(dt, 1)
         lp.spectral_update(dt)
+
+    def timed_pass():
+        B.lp_timing_enable(lp.ctx, args.steps)
+        l0 = lp.launch_count()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        t0.record()
+        for _ in range(args.steps):
+            one_step()
+        t1.record()
+        torch.cuda.synchronize(dev)
+        barrier()
+        sp_ms, sp_n = B.lp_timing_read(lp.ctx)
+        return reduce_max(t0.elapsed_time(t1), dist, dev), lp.launch_count() - l0, sp_ms, sp_n
 
     for _ in range(args.warmup):
         one_step()
     barrier()
-    B.lp_timing_enable(lp.ctx, args.steps)
-    launches0 = lp.launch_count()
     sampler = ClockSampler(local)
     sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        one_step()
-    e1.record()
-    torch.cuda.synchronize(dev)
+    ms, launches, spec_ms, spec_n = timed_pass()           # the K steps `value` is quoted on
     clocks = sampler.stop()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches = lp.launch_count() - launches0
-    spec_ms, spec_n = B.lp_timing_read(lp.ctx)
-    B.lp_timing_enable(lp.ctx, 0)
     d = lp.diag()
-    ms = reduce_max(ms, dist, dev)
     value = aggregate_rate(world, w.np, args.steps, ms * 1e-3)
+
+    # ---- the timed state against the oracle (rank 0 of a single-GPU run; the oracle is test infrastructure)
+    parity = None
+    fields_np = None
+    if world == 1 and not args.no_parity and args.pusher == "rk2":
+        fields_np = [f.cpu().numpy() for f in fields]
+        if field_at is None:
+            fields_for_step = lambda k: (fields_np, fields_np)
+        else:
+            fields_for_step = lambda k: tuple([f.cpu().numpy() for f in field_at(k + j)] for j in (0, 1))
+        parity = parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_host.rows, dt, nstep[0],
+                              args.parity_sample, dev)
+
+    # ---- further passes of the same K steps: median of all (SURVEY.md 8(d) "median of 5 repeats")
+    passes = [(ms, spec_ms, spec_n)]
+    for _ in range(max(1, args.repeats) - 1):
+        m, _, sm_, sn_ = timed_pass()
+        passes.append((m, sm_, sn_))
+    B.lp_timing_enable(lp.ctx, 0)
+    med = sorted(passes)[len(passes) // 2]
+    repeats = {"passes": len(passes), "steps_per_pass": args.steps,
+               "ms_per_step": [p_[0] / args.steps for p_ in passes],
+               "median_ms_per_step": med[0] / args.steps,
+               "median_value": aggregate_rate(world, w.np, args.steps, med[0] * 1e-3),
+               "dominant_kernel_ms": [p_[1] / max(p_[2], 1) for p_ in passes]}
 
     # ---- shock-crossing update (NEXT-1), timed alone on the resident state
     shock = None
@@ -401,25 +502,49 @@ def run_ours(args):
     #   grid: the (vx,vy,vz,rho,bx,by,bz) of every distinct cell the gathers touch, once: 56 B x
     #         min(cells, 8 corners x particles) -- the three gathers of the fused kernel share their cells.
     rows_bytes = 16 * w.nbins * w.np
-    state_bytes = (32 if args.staged else 48) * w.np
+    state_bytes = (32 if staged else 48) * w.np
     grid_bytes = 56 * min(w.n ** 3, 8 * w.np)
     alg_bytes = rows_bytes + state_bytes + grid_bytes
     spec_avg_ms = spec_ms / max(spec_n, 1)
     achieved = alg_bytes / (spec_avg_ms * 1e-3) / 1e9 if spec_n else None
-    kname = "lp_spectral_%s_kernel<%d,0,%d>" % ("bulk" if w.nbins <= 256 else "direct", w.nbins, 0 if args.staged else 1)
+    kname = "lp_spectral_%s_kernel<%d,0,%d>" % ("bulk" if w.nbins <= 256 else "direct", w.nbins, 0 if staged else 1)
+    # The secondary bound ("report both fractions"): fp64 arithmetic.  Algorithmic flops of a row:
+    # per bin and substep the donor-cell update is 3 multiply-adds (6 flop), plus 12 flop per bin once for the
+    # edge velocities and the update coefficients; the substep total is the kernel's own count (lp_get_diag).
+    # Peak: the device's fp64 FMA rate measured now by the library (lp_measure_fp64_peak, independent DFMA chains).
+    alu = None
+    try:
+        alu_peak = B.lp_measure_fp64_peak(local)
+        flops = 6.0 * w.nbins * d["sum_substeps"] + 12.0 * w.nbins * w.np
+        alu_ach = flops / (spec_avg_ms * 1e-3) / 1e12 if spec_n else None
+        alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s (fp64)",
+               "frac": (alu_ach / alu_peak) if alu_ach else None,
+               "peak_source": "measured now: lp_measure_fp64_peak (8 DFMA chains/thread, 512 threads x 4 blocks/SM, best of 3)",
+               "algorithmic_flops_per_launch": flops,
+               "flop_per_byte": flops / alg_bytes}
+    except Exception as e:          # noqa: BLE001 -- the line is still valid without the secondary bound
+        alu = {"error": str(e)}
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
-                "traffic": None if args.staged else stored_traffic(w.name, w.nbins), "peak_source": peak_src,
+                "traffic": stored_traffic(w.name, w.nbins, staged), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "algorithmic_bytes_split": {"rows": rows_bytes, "state": state_bytes, "grid": grid_bytes},
                 "achieved_rows_only": (rows_bytes / (spec_avg_ms * 1e-3) / 1e9) if spec_n else None,
                 "frac_rows_only": (rows_bytes / (spec_avg_ms * 1e-3) / 1e9 / peak) if spec_n else None,
                 "avg_launch_ms": spec_avg_ms,
-                "share_of_step": spec_ms / ms if ms else None}
+                "share_of_step": spec_ms / ms if ms else None,
+                "whole_step_frac": alg_bytes / (ms / args.steps * 1e-3) / 1e9 / peak,
+                "alu": alu}
+    api = False
+    if staged:
+        api = "lp_push_rk3(0..2)" if args.pusher == "rk3" else "lp_push(0), lp_push(1)"
+        if field_at is not None:
+            api = "lp_set_fields(t^n), lp_push(0), lp_set_fields(t^n+1), lp_push(1)"
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, ("lp_push_rk3(0..2)" if args.pusher == "rk3" else "lp_push(0), lp_push(1)") if args.staged else False),
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, api),
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+           "parity_checked": parity, "repeats": repeats,
            "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],
                     "sorts_total": d["sorts"]}}
     if compact is not None:
@@ -429,7 +554,8 @@ def run_ours(args):
         shock["frac_of_measured_peak"] = shock["achieved_gbs"] / peak_s
         out["shock_update"] = shock
     if world == 1 and not args.no_cpu_baseline:
-        fields_np = [f.cpu().numpy() for f in fields]
+        if fields_np is None:
+            fields_np = [f.cpu().numpy() for f in fields]
         out["cpu_baseline"] = cpu_baseline(w, fields_np, u_rad, x, y, z, pid, chi_host, dt, args.cpu_seconds)
     print(json.dumps(out), flush=True)
     if dist is not None:

@@ -21,7 +21,8 @@
  *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls only enqueue
  *    work on it and return; lp_get_diag and the *_host call are the ones that synchronise.
  *  - A context is not thread-safe: one host thread at a time per context (several contexts, on one or
- *    several devices, may be used concurrently).
+ *    several devices, may be used concurrently from different threads: a context shares no mutable state
+ *    with another).
  *  - Every function returns an lp_status; nothing aborts, throws or prints.
  *    lp_last_error gives a human-readable detail for the last failure on that context.
  */
@@ -93,7 +94,10 @@ LP_API lp_status lp_workspace_bytes(const lp_config *cfg, size_t *out_bytes /*ho
 LP_API lp_status lp_bind_workspace(lp_ctx *ctx, void *workspace, size_t bytes);
 
 /* Particle state, advanced in place: positions x,y,z [np], ids [np] (unique), chi [np][nbins]
- * (16-byte aligned).  What a particle carries: PAPER.md:598-613 (Listing 3). */
+ * (16-byte aligned).  What a particle carries: PAPER.md:598-613 (Listing 3).  Enqueues nothing: the width
+ * of the ids (the number of radix passes a sort makes over them) is measured by the first sort that
+ * follows a bind, a raised count or a host copy of the ids -- on that sort's stream, which it synchronises
+ * once for it. */
 LP_API lp_status lp_bind_particles(lp_ctx *ctx, double *x, double *y, double *z, uint64_t *id, double *chi);
 
 /* Optional per-particle outputs of the spectral update: n_sub [np] (negative = capped) and
@@ -111,7 +115,8 @@ LP_API lp_status lp_set_fields(lp_ctx *ctx, const double *vx, const double *vy, 
  * vx,vy,vz,bx,by,bz,rho (or NULL) and the containing-cell key (k*ny+j)*nx+i [np] (or NULL). */
 LP_API lp_status lp_interpolate(lp_ctx *ctx, double *out7, uint32_t *cell_key, void *stream);
 
-/* Reorder all particle arrays ascending by (cell key, id); bound arrays hold the result. */
+/* Reorder all particle arrays ascending by (cell key, id); bound arrays hold the result.  Asynchronous,
+ * except for the first sort after the ids may have changed (see lp_bind_particles). */
 LP_API lp_status lp_sort(lp_ctx *ctx, void *stream);
 
 /* stage 0: k1 = v(x^n), rho_old = rho(x^n), x* = x^n + dt k1 (kept in the workspace).
@@ -130,7 +135,8 @@ LP_API lp_status lp_push_rk3(lp_ctx *ctx, double dt, int stage, void *stream);
 
 /* Spectral update at the current positions with the current fields:
  * coefficients, CFL substep count, n_sub donor-cell upwind substeps of Eq. 6 per particle.
- * Consumes rho_old of the last lp_push(stage 0); LP_ERR_STATE if there was none. */
+ * Consumes rho_old of the last stage 0 and needs the push finished (lp_push stage 1 or lp_push_rk3 stage 2
+ * since that stage 0), so that the bound positions are x^{n+1}; LP_ERR_STATE otherwise. */
 LP_API lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream);
 
 /* Shock crossing (Eq. 7-8; not part of lp_step): every particle p with r[p] > 1 gets
@@ -184,6 +190,12 @@ LP_API lp_status lp_launch_count(const lp_ctx *ctx, int64_t *out /*host*/);
  * number of launches recorded, and re-arms the records.  n = 0 disables. */
 LP_API lp_status lp_timing_enable(lp_ctx *ctx, int max_records);
 LP_API lp_status lp_timing_read(lp_ctx *ctx, double *spectral_ms_sum /*host*/, int32_t *n_records /*host*/);
+
+/* fp64 FMA rate of `device` in TFLOP/s (2 flop per DFMA), measured with a kernel of independent dependent-FMA
+ * chains (8 per thread, 512 threads x 4 blocks per SM, best of three): the denominator of the arithmetic
+ * roofline bench.py prints beside the HBM one for the bin counts whose rows take many substeps.  Needs no
+ * context; allocates and frees 8 B per thread; synchronises the device. */
+LP_API lp_status lp_measure_fp64_peak(int device, double *tflops /*host*/);
 
 /* Copy the library's bin table to host arrays: edges [nbins+1], widths [nbins] (either may be NULL). */
 LP_API lp_status lp_get_bins(const lp_ctx *ctx, double *edges /*host*/, double *widths /*host*/);

@@ -17,7 +17,8 @@ _STATUS_NAMES = {0: "LP_OK", -1: "LP_ERR_INVALID_ARG", -2: "LP_ERR_STATE", -3: "
 EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp_bind_workspace",
            "lp_bind_particles", "lp_bind_diag", "lp_set_fields", "lp_interpolate", "lp_sort", "lp_push",
            "lp_spectral_update", "lp_step", "lp_step_host", "lp_get_diag", "lp_launch_count", "lp_get_bins",
-           "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3", "lp_chunked_capacity", "lp_set_count")
+           "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3", "lp_chunked_capacity", "lp_set_count",
+           "lp_measure_fp64_peak")
 
 
 class LPError(RuntimeError):
@@ -86,6 +87,7 @@ def load():
     lib.lp_timing_enable.argtypes = [vp, C.c_int]
     lib.lp_get_cfl_bins.argtypes = [vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.lp_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
+    lib.lp_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
     for name in EXPORTS:
         if name != "lp_last_error":
             getattr(lib, name).restype = C.c_int
@@ -232,6 +234,14 @@ def lp_timing_read(ctx):
     ms = C.c_double(); n = C.c_int32()
     _check(ctx, load().lp_timing_read(ctx, C.byref(ms), C.byref(n)))
     return ms.value, n.value
+
+
+def lp_measure_fp64_peak(device=0):
+    out = C.c_double()
+    st = load().lp_measure_fp64_peak(int(device), C.byref(out))
+    if st != LP_OK:
+        raise LPError(st)
+    return out.value
 
 
 def lp_get_bins(ctx, nbins):

@@ -148,6 +148,9 @@ struct lp_ctx {
     int push_kind = 0;                     // which pusher ran stage 0: 1 two-stage (k1, x* kept), 2 three-stage (x0 kept)
     int rk3_next = 0;                      // next stage lp_push_rk3 expects
     bool status_valid = false;             // the status array describes the bound particles in their current order
+    bool push_done = false;                // a pusher ran to its last stage since stage 0 (x^{n+1} is in place)
+    bool id_bits_stale = true;             // ids may have changed since id_bits was measured (bind, injection, host copy)
+    int spectral_blocks[4] = { 0, 0, 0, 0 };   // resident blocks per SM of the spectral kernel variants [diag][fused], 0 = not set up
     long long capacity = 0;                // particles the workspace was sized for (cfg.np shrinks in lp_compact)
     int id_bits = 0, key_bits = 0;
     long long launches = 0, steps = 0, sorts = 0;
@@ -278,7 +281,8 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
     a.max_substeps = c->cfg.max_substeps;
     const bool rec = c->timing && c->ev_used + 2 <= c->ev.size();
     if (rec) LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used], s));
-    lp_status st = count(c, lp_launch_spectral(a, c->cfg.nbins, c->lost_user != nullptr, fused, c->sm_count, s),
+    lp_status st = count(c, lp_launch_spectral(a, c->cfg.nbins, c->lost_user != nullptr, fused, c->sm_count,
+                                                    c->spectral_blocks, s),
                          "lp_spectral_kernel launch");
     if (rec) {
         LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], s));
@@ -286,7 +290,7 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
     }
     if (st == LP_OK) {
         c->spectra_done = true;
-        c->stage0_done = false; c->rk3_next = 0;
+        c->stage0_done = false; c->rk3_next = 0; c->push_done = false;
         if (fused) c->status_valid = true;
     }
     return st;
@@ -308,7 +312,20 @@ lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
     b.hist_elems = c->lay.hist_elems;
     b.digit = c->at<uint8_t>(c->lay.lost);          // the per-particle `lost` buffer is dead across a re-sort
     uint32_t *perm = nullptr;
-    lp_status st = count(c, lp_launch_sort_perm(c->geom, c->x, c->y, c->z, c->id, np, c->id_bits, c->key_bits, b, &perm, s),
+    lp_status st;
+    if (c->id_bits_stale) {
+        // number of radix passes over the ids = bit length of the largest id among the current particles.
+        // Measured on the caller's stream, once after every event that can change the ids (bind, raised
+        // count, host copy); this is the one place a sort synchronises.
+        unsigned long long *d = c->at<unsigned long long>(c->lay.maxid), h = 0;
+        LP_CUDA(c, cudaMemsetAsync(d, 0, 8, s));
+        if ((st = count(c, lp_launch_max_u64(c->id, np, d, s), "lp_max_u64_kernel launch")) != LP_OK) return st;
+        LP_CUDA(c, cudaMemcpyAsync(&h, d, 8, cudaMemcpyDeviceToHost, s));
+        LP_CUDA(c, cudaStreamSynchronize(s));
+        c->id_bits = bit_length(h);
+        c->id_bits_stale = false;
+    }
+    st = count(c, lp_launch_sort_perm(c->geom, c->x, c->y, c->z, c->id, np, c->id_bits, c->key_bits, b, &perm, s),
                          "sort kernels launch");
     if (st != LP_OK) return st;
     double *sx = c->at<double>(c->lay.xs);
@@ -326,7 +343,7 @@ lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
             LP_CUDA(c, cudaMemcpyAsync(pos[d], sx + (size_t)d * np, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
         LP_CUDA(c, cudaMemcpyAsync(c->chi, chi_alt, (size_t)np * c->cfg.nbins * 8, cudaMemcpyDeviceToDevice, s));
     }
-    c->stage0_done = false; c->rk3_next = 0;      // k1 / x* / rho_old refer to the old order
+    c->stage0_done = false; c->rk3_next = 0; c->push_done = false;      // k1 / x* / rho_old refer to the old order
     c->spectra_done = false;     // so do the per-particle n_sub / lost of the last update
     c->status_valid = false;
     ++c->sorts;
@@ -413,8 +430,9 @@ lp_status lp_bind_workspace(lp_ctx *ctx, void *workspace, size_t bytes)
     if (bytes < ctx->lay.total) return fail(ctx, LP_ERR_WORKSPACE, "workspace smaller than lp_workspace_bytes");
     ctx->ws = static_cast<unsigned char *>(workspace);
     ctx->have_fields = false;
-    ctx->stage0_done = false; ctx->rk3_next = 0;
+    ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
     ctx->spectra_done = false;
+    ctx->status_valid = false;
     return LP_OK;
 }
 
@@ -425,19 +443,11 @@ lp_status lp_bind_particles(lp_ctx *ctx, double *x, double *y, double *z, uint64
     if (ctx->cfg.np > 0 && (!x || !y || !z || !id || !chi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL particle array");
     if (reinterpret_cast<uintptr_t>(chi) % 16) return fail(ctx, LP_ERR_INVALID_ARG, "chi not 16-byte aligned");
     ctx->x = x; ctx->y = y; ctx->z = z; ctx->id = id; ctx->chi = chi;
-    ctx->stage0_done = false; ctx->rk3_next = 0;
+    ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
     ctx->spectra_done = false;
     ctx->status_valid = false;
     ctx->id_bits = 0;
-    if (ctx->cfg.np > 0) {      // number of radix passes over the ids: bit length of the largest id
-        LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-        unsigned long long *d = ctx->at<unsigned long long>(ctx->lay.maxid), h = 0;
-        LP_CUDA(ctx, cudaMemset(d, 0, 8));
-        lp_status st = count(ctx, lp_launch_max_u64(id, ctx->cfg.np, d, 0), "lp_max_u64_kernel launch");
-        if (st != LP_OK) return st;
-        LP_CUDA(ctx, cudaMemcpy(&h, d, 8, cudaMemcpyDeviceToHost));
-        ctx->id_bits = bit_length(h);
-    }
+    ctx->id_bits_stale = true;          // measured on the caller's stream by the next sort
     return LP_OK;
 }
 
@@ -489,17 +499,17 @@ lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream)
     if (st != LP_OK) return st;
     if (stage != 0 && stage != 1) return fail(ctx, LP_ERR_INVALID_ARG, "stage must be 0 or 1");
     if (stage == 1 && !(ctx->stage0_done && ctx->push_kind == 1)) return fail(ctx, LP_ERR_STATE, "lp_push stage 1 without stage 0");
-    if (ctx->cfg.np == 0) { ctx->stage0_done = true; return LP_OK; }
+    if (ctx->cfg.np == 0) { ctx->stage0_done = true; ctx->push_kind = 1; ctx->push_done = stage == 1; return LP_OK; }
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     LpPushArgs a = push_args(ctx, dt);
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     if (stage == 0) {
         st = count(ctx, lp_launch_push0(a, s), "lp_push0_kernel launch");
-        if (st == LP_OK) { ctx->stage0_done = true; ctx->push_kind = 1; ctx->rk3_next = 0; }
+        if (st == LP_OK) { ctx->stage0_done = true; ctx->push_kind = 1; ctx->rk3_next = 0; ctx->push_done = false; }
         return st;
     }
     st = count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch");
-    if (st == LP_OK) ctx->status_valid = true;
+    if (st == LP_OK) { ctx->status_valid = true; ctx->push_done = true; }
     return st;
 }
 
@@ -516,8 +526,8 @@ lp_status lp_push_rk3(lp_ctx *ctx, double dt, int stage, void *stream)
         st = count(ctx, lp_launch_push_rk3(a, stage, static_cast<cudaStream_t>(stream)), "lp_push_rk3_kernel launch");
         if (st != LP_OK) return st;
     }
-    if (stage == 0) { ctx->stage0_done = true; ctx->push_kind = 2; ctx->status_valid = false; }
-    if (stage == 2) ctx->status_valid = true;
+    if (stage == 0) { ctx->stage0_done = true; ctx->push_kind = 2; ctx->status_valid = false; ctx->push_done = false; }
+    if (stage == 2) { ctx->status_valid = true; ctx->push_done = true; }
     ctx->rk3_next = stage == 2 ? 0 : stage + 1;
     return LP_OK;
 }
@@ -527,6 +537,8 @@ lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
     lp_status st = need_ready(ctx, true);
     if (st != LP_OK) return st;
     if (!ctx->stage0_done) return fail(ctx, LP_ERR_STATE, "lp_spectral_update needs rho_old of lp_push stage 0");
+    if (!ctx->push_done)
+        return fail(ctx, LP_ERR_STATE, "lp_spectral_update needs the push finished (lp_push stage 1 / lp_push_rk3 stage 2)");
     if (ctx->cfg.np == 0) return LP_OK;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     return do_spectral(ctx, dt, ctx->chi, false, static_cast<cudaStream_t>(stream));
@@ -564,7 +576,7 @@ lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *st
     LP_CUDA(ctx, cudaMemcpyAsync(h_counts, counts, sizeof h_counts, cudaMemcpyDeviceToHost, s));
     LP_CUDA(ctx, cudaStreamSynchronize(s));
     ctx->cfg.np -= (long long)h_counts[0];          // the workspace keeps its size (capacity)
-    ctx->stage0_done = false; ctx->rk3_next = 0;
+    ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
     ctx->spectra_done = false;
     ctx->status_valid = false;
     *np_new = ctx->cfg.np;
@@ -585,8 +597,9 @@ lp_status lp_set_count(lp_ctx *ctx, int64_t np_new)
     if (!ctx) return LP_ERR_INVALID_ARG;
     if (np_new < 0 || np_new > ctx->capacity) return fail(ctx, LP_ERR_INVALID_ARG, "count outside [0, capacity of lp_create]");
     if (np_new > 0 && ctx->ws && !ctx->x) return fail(ctx, LP_ERR_STATE, "no particles bound (lp_bind_particles)");
+    if (np_new > ctx->cfg.np) ctx->id_bits_stale = true;      // injected particles bring their own ids
     ctx->cfg.np = np_new;
-    ctx->stage0_done = false; ctx->rk3_next = 0;
+    ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
     ctx->spectra_done = false;
     ctx->status_valid = false;
     return LP_OK;
@@ -633,6 +646,7 @@ lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *h
             LP_CUDA(ctx, cudaMemcpyAsync(ctx->z, hz, np * 8, cudaMemcpyHostToDevice, s));
             LP_CUDA(ctx, cudaMemcpyAsync(ctx->id, hid, np * 8, cudaMemcpyHostToDevice, s));
             LP_CUDA(ctx, cudaMemcpyAsync(ctx->chi, hchi, np * nb * 8, cudaMemcpyHostToDevice, s));
+            ctx->id_bits_stale = true;                  // the host may hand in other ids than last time
         }
         if ((st = lp_step(ctx, dt, stream)) != LP_OK) return st;
         if (np) {
@@ -710,7 +724,7 @@ lp_status lp_get_diag(lp_ctx *ctx, lp_diag *out, void *stream)
     if (!have) LP_CUDA(ctx, cudaMemsetAsync(ctx->at<int32_t>(ctx->lay.nsub), 0, (size_t)ctx->cfg.np * 4, s));
     st = count(ctx, lp_launch_diag(ctx->at<int32_t>(ctx->lay.nsub),
                                    (have && ctx->lost_user) ? ctx->at<double>(ctx->lay.lost) : nullptr,
-                                   have ? ctx->at<int32_t>(ctx->lay.status) : nullptr, ctx->chi, ctx->tab,
+                                   ctx->status_valid ? ctx->at<int32_t>(ctx->lay.status) : nullptr, ctx->chi, ctx->tab,
                                    ctx->cfg.nbins, ctx->cfg.np, ctx->at<double>(ctx->lay.partial), d, s),
                "lp_diag_kernel launch");
     if (st != LP_OK) return st;

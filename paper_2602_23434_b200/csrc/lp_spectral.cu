@@ -924,34 +924,31 @@ template <class K> int lp_blocks_per_sm(K kernel, int threads, size_t smem)
     return per_sm < 1 ? 1 : per_sm;
 }
 
+// blocks_cache: the context's slot for this variant (0 = not set up yet).  Function attributes are per
+// device and a context lives on one device, so the set-up runs once per context and variant; a context
+// is used by one host thread at a time (lp.h), and cudaFuncSetAttribute itself is thread-safe.
 template <int NB, bool DIAG, bool FUSED>
-int launch_variant(const LpSpectralArgs &a, int sm_count, cudaStream_t s)
+int launch_variant(const LpSpectralArgs &a, int sm_count, int *blocks_cache, cudaStream_t s)
 {
     const long long nchunks = (a.np + 31) >> 5;
     if constexpr (NB <= LP_BULK_MAX_NB) {
         using C = LpBulkCfg<NB>;
         auto kernel = lp_spectral_bulk_kernel<NB, DIAG, FUSED>;
-        // function attributes are per device: set them once on each device this kernel is launched on
-        static bool configured[64] = {};
-        static int blocks_per_sm[64] = {};
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return -1;
-        const int slot = dev & 63;
-        if (!configured[slot]) {
+        if (*blocks_cache == 0) {
             if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_TOTAL) != cudaSuccess) return -1;
             if (cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, LP_BULK_CARVEOUT) != cudaSuccess) return -1;
-            blocks_per_sm[slot] = lp_blocks_per_sm(kernel, C::THREADS, C::SMEM_TOTAL);
-            configured[slot] = true;
+            *blocks_cache = lp_blocks_per_sm(kernel, C::THREADS, C::SMEM_TOTAL);
         }
         const long long want = nchunks;                      // a block takes whole chunks
-        const long long cap = (long long)sm_count * blocks_per_sm[slot];
+        const long long cap = (long long)sm_count * *blocks_cache;
         int blocks = (int)(want < cap ? want : cap);
         if (blocks < 1) blocks = 1;
         kernel<<<blocks, C::THREADS, C::SMEM_TOTAL, s>>>(a);
     } else {
         auto kernel = lp_spectral_direct_kernel<NB, DIAG, FUSED>;
+        if (*blocks_cache == 0) *blocks_cache = lp_blocks_per_sm(kernel, kDirectThreads, 0);
         const long long want = (nchunks + kDirectWarps - 1) / kDirectWarps;
-        const long long cap = (long long)sm_count * lp_blocks_per_sm(kernel, kDirectThreads, 0);
+        const long long cap = (long long)sm_count * *blocks_cache;
         int blocks = (int)(want < cap ? want : cap);
         if (blocks < 1) blocks = 1;
         kernel<<<blocks, kDirectThreads, 0, s>>>(a);
@@ -960,23 +957,25 @@ int launch_variant(const LpSpectralArgs &a, int sm_count, cudaStream_t s)
 }
 
 template <int NB>
-int launch_nb(const LpSpectralArgs &a, bool diag, bool fused, int sm_count, cudaStream_t s)
+int launch_nb(const LpSpectralArgs &a, bool diag, bool fused, int sm_count, int *blocks_cache, cudaStream_t s)
 {
-    if (diag) return fused ? launch_variant<NB, true, true>(a, sm_count, s) : launch_variant<NB, true, false>(a, sm_count, s);
-    return fused ? launch_variant<NB, false, true>(a, sm_count, s) : launch_variant<NB, false, false>(a, sm_count, s);
+    int *slot = blocks_cache + (diag ? 2 : 0) + (fused ? 1 : 0);
+    if (diag) return fused ? launch_variant<NB, true, true>(a, sm_count, slot, s) : launch_variant<NB, true, false>(a, sm_count, slot, s);
+    return fused ? launch_variant<NB, false, true>(a, sm_count, slot, s) : launch_variant<NB, false, false>(a, sm_count, slot, s);
 }
 
 }  // namespace
 
-int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, bool fused, int sm_count, cudaStream_t s)
+int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, bool fused, int sm_count, int *blocks_cache,
+                       cudaStream_t s)
 {
     switch (nbins) {
-    case 16:  return launch_nb<16>(a, diag, fused, sm_count, s);
-    case 32:  return launch_nb<32>(a, diag, fused, sm_count, s);
-    case 64:  return launch_nb<64>(a, diag, fused, sm_count, s);
-    case 128: return launch_nb<128>(a, diag, fused, sm_count, s);
-    case 256: return launch_nb<256>(a, diag, fused, sm_count, s);
-    case 512: return launch_nb<512>(a, diag, fused, sm_count, s);
+    case 16:  return launch_nb<16>(a, diag, fused, sm_count, blocks_cache, s);
+    case 32:  return launch_nb<32>(a, diag, fused, sm_count, blocks_cache, s);
+    case 64:  return launch_nb<64>(a, diag, fused, sm_count, blocks_cache, s);
+    case 128: return launch_nb<128>(a, diag, fused, sm_count, blocks_cache, s);
+    case 256: return launch_nb<256>(a, diag, fused, sm_count, blocks_cache, s);
+    case 512: return launch_nb<512>(a, diag, fused, sm_count, blocks_cache, s);
     default:  return -1;
     }
 }

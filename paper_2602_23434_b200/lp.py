@@ -76,6 +76,10 @@ class LP:
                          key.data_ptr() if want_key else None, self.stream)
         return out7, key
 
+    def current(self):
+        """The tensors that hold the particle state now: (x, y, z, id, chi)."""
+        return self.x, self.y, self.z, self.id, self.chi
+
     def sort(self):
         B.lp_sort(self.ctx, self.stream)
 

@@ -23,7 +23,8 @@ def test_bench_line_has_the_contract_keys():
     d = run_bench("--workload", "1", "--steps", "5", "--warmup", "3", "--e2e-steps", "2", "--cpu-seconds", "1",
                   "--shock-frac", "0.5", "--compact-frac", "0.25")
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
-              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline",
+              "parity_checked", "repeats"):
         assert k in d, k
     assert d["n_gpus"] == 1 and d["steps"] == 5 and d["warmup"] == 3 and d["dtype"] == "f64"
     assert d["vs_baseline"] is None and d["scaling"] == "weak" and d["data"] == "synthetic"
@@ -31,12 +32,27 @@ def test_bench_line_has_the_contract_keys():
     r = d["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["peak"] > 1000 and r["achieved"] > 0
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and "traffic" in r
+    a = r["alu"]
+    assert a["bound"] == "alu" and a["peak"] > 1.0 and a["achieved"] > 0 and abs(a["frac"] - a["achieved"] / a["peak"]) < 1e-12
+    pc = d["parity_checked"]
+    assert pc["ok"] and pc["positions_bit_exact"] and pc["max_rel"] <= 1e-10 and pc["steps"] == 8 and pc["particles"] == 1024
+    rp = d["repeats"]
+    assert rp["passes"] == 5 and len(rp["ms_per_step"]) == 5 and rp["median_ms_per_step"] > 0
     e = d["e2e"]
     assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
     assert d["shock_update"]["flagged"] > 0 and d["compact"]["np_new"] == 1024 - d["compact"]["deleted"]
+    c1, cs = c["single_thread"], c["spectral_update_only"]
+    assert c1["cores"] == 1 and c1["value"] > 0 and cs["value"] > 0
+
+
+@pytest.mark.gpu
+def test_bench_workload2_staged_with_time_dependent_fields():
+    """configs[1]: the staged calls with the fields re-set between the stages, parity-checked in the line."""
+    d = run_bench("--workload", "2", "--steps", "4", "--warmup", "3", "--repeats", "2", "--no-e2e", "--cpu-seconds", "1")
+    assert "lp_set_fields" in d["config"]["api"] and d["parity_checked"]["ok"] and d["parity_checked"]["steps"] == 7
 
 
 @pytest.mark.gpu

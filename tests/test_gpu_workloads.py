@@ -105,8 +105,10 @@ def cached_fields(w, dev):
     return _FIELD_CACHE[k]
 
 
-def run_sampled(w, steps, nsample=2048, check_sort=True):
-    """Run `steps` lp_step on the GPU at full size and the oracle on a sample; compare by id."""
+def run_sampled(w, steps, nsample=2048, check_sort=True, diag="full"):
+    """Run `steps` lp_step on the GPU at full size and the oracle on a sample; compare by id.
+    diag = "nsub": only n_sub is bound, so the DIAG=false kernel instantiations run -- the ones bench.py
+    times (it binds no `lost` output); the number-conservation property needs `lost` and is then skipped."""
     dev = "cuda"
     fields, f_np = cached_fields(w, dev)
     u_rad = u_rad_of(w, fields)
@@ -118,7 +120,7 @@ def run_sampled(w, steps, nsample=2048, check_sort=True):
     lp = P.LP(P.config_from_workload(w, u_rad=u_rad))
     lp.set_fields(fields)
     lp.bind_particles(x, y, z, pid, chi_dev)
-    lp.bind_diag()
+    lp.bind_diag(nsub=True, lost=(diag == "full"))
     n0 = lp.diag()["number"]
     # oracle sample (ids chosen by a seeded draw)
     srng = np.random.default_rng(12345)
@@ -130,7 +132,8 @@ def run_sampled(w, steps, nsample=2048, check_sort=True):
     for s in range(steps):
         lp.step(w.dt)
         sx, sy, sz, schi, snsub, slost, st = orc.step(prm, f_np, sx, sy, sz, w.dt, schi, nthreads=8)
-        lost_total += lp.diag()["lost"]
+        if diag == "full":
+            lost_total += lp.diag()["lost"]
     torch.cuda.synchronize()
     gid = host(lp.id).view(np.uint64)
     # properties at full size
@@ -139,7 +142,8 @@ def run_sampled(w, steps, nsample=2048, check_sort=True):
     for a in (gx, gy, gz):
         assert (a >= -1.0).all() and (a < 1.0).all()
     d = lp.diag()
-    assert abs((d["number"] + lost_total) / n0 - 1) < 1e-11
+    if diag == "full":
+        assert abs((d["number"] + lost_total) / n0 - 1) < 1e-11
     assert d["n_capped"] == 0 and d["n_outside"] == 0
     if check_sort and w.sort_every:
         assert d["sorts"] == (steps + w.sort_every - 1) // w.sort_every
@@ -159,13 +163,15 @@ def test_workload3_turbulent_sampled():
     assert d["max_substeps"] >= 1
 
 
-def test_workload4_large_sampled_with_resort():
-    """16.7M particles, 256^3, 64 bins, sort_every = 10: 11 steps so that two sorts happen; after the
-    second sort + one step the order is still (key, id) ascending up to the drift of that step, so
-    the order property is checked right after an explicit lp_sort."""
-    w = I.workload(4)
-    lp, d, nsub = run_sampled(w, steps=11, nsample=4096)
-    assert d["sorts"] == 2
+def test_workload3_full_length_bench_kernels():
+    """All 50 steps of BASELINE.json configs[2] in the kernels bench.py times (no `lost` output bound)."""
+    w = I.workload(3)
+    assert w.steps == 50
+    lp, d, nsub = run_sampled(w, steps=w.steps, diag="nsub")
+    assert d["steps"] == 50
+
+
+def check_sorted_after_explicit_sort(lp):
     lp.sort()
     _, key = lp.interpolate(want_fields=False)
     key = host(key).view(np.uint32).astype(np.int64)
@@ -176,9 +182,37 @@ def test_workload4_large_sampled_with_resort():
     assert (np.diff(gid.astype(np.int64))[same] > 0).all()
 
 
+def test_workload4_large_sampled_with_resort():
+    """16.7M particles, 256^3, 64 bins, sort_every = 10: 11 steps so that two sorts happen; after the
+    second sort + one step the order is still (key, id) ascending up to the drift of that step, so
+    the order property is checked right after an explicit lp_sort."""
+    w = I.workload(4)
+    lp, d, nsub = run_sampled(w, steps=11, nsample=4096)
+    assert d["sorts"] == 2
+    check_sorted_after_explicit_sort(lp)
+
+
+def test_workload4_full_length_bench_kernels():
+    """All 20 steps of BASELINE.json configs[3] (two re-sorts) in the kernels bench.py times."""
+    w = I.workload(4)
+    assert w.steps == 20
+    lp, d, nsub = run_sampled(w, steps=w.steps, nsample=4096, diag="nsub")
+    assert d["sorts"] == 2 and d["steps"] == 20
+    check_sorted_after_explicit_sort(lp)
+
+
 @pytest.mark.parametrize("nbins", [16, 32, 64, 128, 256, 512])
 def test_workload5_bin_sweep_sampled(nbins):
     w = I.workload(5).scaled(nbins=nbins)
     lp, d, nsub = run_sampled(w, steps=2, nsample=1024)
     expected_typical = {16: 1, 32: 1, 64: 1, 128: 2, 256: 5, 512: 10}[nbins]
     assert 0.4 * expected_typical <= np.median(np.abs(nsub)) <= 2.5 * expected_typical
+
+
+@pytest.mark.parametrize("nbins", [16, 32, 64, 128, 256, 512])
+def test_workload5_full_length_bench_kernels(nbins):
+    """All 10 steps of BASELINE.json configs[4] at every bin count, in the kernels bench.py times."""
+    w = I.workload(5).scaled(nbins=nbins)
+    assert w.steps == 10
+    lp, d, nsub = run_sampled(w, steps=w.steps, nsample=1024, diag="nsub")
+    assert d["steps"] == 10 and d["sorts"] == 1
