@@ -52,6 +52,9 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--repeats", type=int, default=5,
                     help="timed passes of --steps in all (SURVEY.md 8(d): median of 5); `value` is the first one")
+    ap.add_argument("--no-pingpong", action="store_true",
+                    help="keep the state in the bound arrays across re-sorts (permute pass + copies) instead of "
+                         "lp_set_pingpong (re-sort folded into the fused kernel)")
     ap.add_argument("--no-parity", action="store_true", help="skip the oracle check of the timed state")
     ap.add_argument("--parity-sample", type=int, default=2048)
     return ap.parse_args()
@@ -141,11 +144,12 @@ def step_dt(w):
     return 0.9 * w.cfl_e / lam_top
 
 
-def config_dict(w, n_gpus, staged=False):
+def config_dict(w, n_gpus, staged=False, pingpong=False):
     return {"workload": "BASELINE.json configs[%d] %s" % (w.index - 1, w.name), "grid": "%d^3" % w.n,
             "particles_per_gpu": w.np, "nbins": w.nbins, "sort_every": w.sort_every,
             "parallelism": "replicas x%d (particles independent, no collective)" % n_gpus,
             "api": ("staged %s, lp_spectral_update" % staged) if staged else "fused lp_step",
+            "resort": "ping-pong buffers (lp_set_pingpong)" if pingpong else "bound arrays (permute + copy back)",
             "l2": "inputs larger than L2 (chi rows %.2f GB per GPU)" % (w.np * w.nbins * 8 / 1e9)}
 
 
@@ -344,6 +348,7 @@ def run_ours(args):
     lp = P.LP(P.config_from_workload(w, u_rad=u_rad, device=local))
     lp.set_fields(fields)
     lp.bind_particles(x, y, z, pid, chi_device())
+    lp.set_pingpong(not args.no_pingpong)
     B = P.binding
     total_steps = args.warmup + args.steps * max(1, args.repeats)
     field_at = None
@@ -421,16 +426,20 @@ def run_ours(args):
 
     # ---- further passes of the same K steps: median of all (SURVEY.md 8(d) "median of 5 repeats")
     passes = [(ms, spec_ms, spec_n)]
+    sampler2 = ClockSampler(local)
+    sampler2.start()
     for _ in range(max(1, args.repeats) - 1):
         m, _, sm_, sn_ = timed_pass()
         passes.append((m, sm_, sn_))
+    clocks2 = sampler2.stop()
     B.lp_timing_enable(lp.ctx, 0)
     med = sorted(passes)[len(passes) // 2]
     repeats = {"passes": len(passes), "steps_per_pass": args.steps,
                "ms_per_step": [p_[0] / args.steps for p_ in passes],
                "median_ms_per_step": med[0] / args.steps,
                "median_value": aggregate_rate(world, w.np, args.steps, med[0] * 1e-3),
-               "dominant_kernel_ms": [p_[1] / max(p_[2], 1) for p_ in passes]}
+               "dominant_kernel_ms": [p_[1] / max(p_[2], 1) for p_ in passes],
+               "clocks_after_first_pass": clocks2}
 
     # ---- shock-crossing update (NEXT-1), timed alone on the resident state
     shock = None
@@ -542,7 +551,7 @@ def run_ours(args):
             api = "lp_set_fields(t^n), lp_push(0), lp_set_fields(t^n+1), lp_push(1)"
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, api),
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, api, not args.no_pingpong),
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
            "parity_checked": parity, "repeats": repeats,
            "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],

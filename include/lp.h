@@ -170,6 +170,22 @@ LP_API lp_status lp_set_count(lp_ctx *ctx, int64_t np_new);
  * spectral update (order of Table 1, without the fluid stages). */
 LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);
 
+/* Ping-pong particle buffers (off by default).  A re-sort cannot run in place: every array is read through
+ * the permutation and written in the new order.  By default the library permutes into the workspace and the
+ * bound arrays hold the state again when the call returns (one extra pass over every row per sort).  With
+ * ping-pong enabled the workspace twins of the bound arrays (same sizes, inside the caller's workspace)
+ * become a second home of the state: lp_sort permutes from the current home into the other one, and on a
+ * sort step lp_step folds the permutation into the fused kernel (it reads rows, positions and ids through
+ * the permutation and writes the other home), so a re-sort costs the permutation itself and nothing else.
+ * The price: after a sort the state may live in the workspace -- lp_current_particles says where, and every
+ * call of this library follows it (injection through lp_set_count writes behind the current particles of
+ * the CURRENT arrays).  Disabling copies the state back into the bound arrays on `stream` if it is not there. */
+LP_API lp_status lp_set_pingpong(lp_ctx *ctx, int enable, void *stream);
+/* Device pointers of the arrays that hold the particle state now (any may be NULL): the bound arrays, or with
+ * ping-pong their workspace twins.  Valid until the next sort. */
+LP_API lp_status lp_current_particles(const lp_ctx *ctx, double **x, double **y, double **z, uint64_t **id,
+                                      double **chi);
+
 /* The same step on HOST buffers (pinned for overlap; pageable works, serialised): copies x,y,z,id,chi
  * to the bound device arrays, runs lp_step, copies x,y,z,chi (and id on re-sort steps) back and
  * synchronises the stream.  With >= 65536 particles and no re-sort due, the step runs in 16 particle

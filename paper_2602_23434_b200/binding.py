@@ -18,7 +18,7 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_bind_particles", "lp_bind_diag", "lp_set_fields", "lp_interpolate", "lp_sort", "lp_push",
            "lp_spectral_update", "lp_step", "lp_step_host", "lp_get_diag", "lp_launch_count", "lp_get_bins",
            "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3", "lp_chunked_capacity", "lp_set_count",
-           "lp_measure_fp64_peak")
+           "lp_measure_fp64_peak", "lp_set_pingpong", "lp_current_particles")
 
 
 class LPError(RuntimeError):
@@ -88,6 +88,8 @@ def load():
     lib.lp_get_cfl_bins.argtypes = [vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.lp_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
     lib.lp_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    lib.lp_set_pingpong.argtypes = [vp, C.c_int, vp]
+    lib.lp_current_particles.argtypes = [vp] + [C.POINTER(C.c_void_p)] * 5
     for name in EXPORTS:
         if name != "lp_last_error":
             getattr(lib, name).restype = C.c_int
@@ -198,6 +200,17 @@ def lp_compact(ctx, flag_ptr, stream=None):
     n = C.c_int64()
     _check(ctx, load().lp_compact(ctx, flag_ptr, C.byref(n), stream))
     return int(n.value)
+
+
+def lp_set_pingpong(ctx, enable, stream=None):
+    _check(ctx, load().lp_set_pingpong(ctx, int(bool(enable)), stream))
+
+
+def lp_current_particles(ctx):
+    """Device addresses (ints) of x, y, z, id, chi as they are now."""
+    p = [C.c_void_p() for _ in range(5)]
+    _check(ctx, load().lp_current_particles(ctx, *[C.byref(q) for q in p]))
+    return tuple(q.value or 0 for q in p)
 
 
 def lp_step(ctx, dt, stream=None):

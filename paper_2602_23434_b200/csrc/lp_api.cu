@@ -17,7 +17,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t recA, recB, k1, xs, rho_old, nsub, lost, status, key, idx_a, idx_b, hist, alt_id, chi_alt,
+    size_t recA, recB, k1, xs, rho_old, nsub, lost, status, key, idx_a, idx_b, hist, alt_id, pos_alt, chi_alt,
         partial, diag, maxid, total;
     size_t hist_elems;
 };
@@ -43,6 +43,7 @@ Layout make_layout(const lp_config &c)
     L.hist_elems = lp_sort_hist_elems(c.np);
     L.hist = take(L.hist_elems * 4);
     L.alt_id = take(np * 8);
+    L.pos_alt = take(np * 24);
     L.chi_alt = take(np * (size_t)c.nbins * 8);
     L.partial = take(2 * 296 * 8);
     L.diag = take(sizeof(LpDiagDev));
@@ -162,8 +163,23 @@ struct lp_ctx {
     cudaStream_t s_in = nullptr, s_out = nullptr;
     std::vector<cudaEvent_t> ev_pipe;
 
+    // Two sets of particle arrays: 0 = the caller's bound arrays, 1 = their twins in the workspace (pos_alt,
+    // alt_id, chi_alt; stride = capacity).  Without ping-pong (default) the state is always in set 0.  With it
+    // (lp_set_pingpong) a re-sort reads one set through the permutation and writes the other, and `cur` flips.
+    bool pingpong = false;
+    int cur = 0;
+
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
     LpCells cells() const { return LpCells{ at<const double4>(lay.recA), at<const double4>(lay.recB) }; }
+    struct Set { double *x, *y, *z; uint64_t *id; double *chi; };
+    Set set(int which) const
+    {
+        if (which == 0) return Set{ x, y, z, id, chi };
+        double *p = at<double>(lay.pos_alt);
+        return Set{ p, p + capacity, p + 2 * capacity, at<uint64_t>(lay.alt_id), at<double>(lay.chi_alt) };
+    }
+    Set now() const { return set(cur); }
+    Set other() const { return set(cur ^ 1); }
 };
 
 namespace {
@@ -227,7 +243,8 @@ LpPushArgs push_args(lp_ctx *c, double dt)
     LpPushArgs a;
     a.g = c->geom;
     a.cells = c->cells();
-    a.x = c->x; a.y = c->y; a.z = c->z;
+    const lp_ctx::Set n = c->now();
+    a.x = n.x; a.y = n.y; a.z = n.z;
     a.k1 = c->at<double>(c->lay.k1);
     a.xs = c->at<double>(c->lay.xs);
     a.rho_old = c->at<double>(c->lay.rho_old);
@@ -237,23 +254,36 @@ LpPushArgs push_args(lp_ctx *c, double dt)
     return a;
 }
 
+// Where one launch of the spectral kernel reads and writes the particle arrays.
+struct SpectralIO {
+    const double *xin, *yin, *zin, *chi_in;
+    double *x, *y, *z, *chi_out;
+    const uint32_t *perm;              // re-sort folded into the fused step, or NULL
+    const uint64_t *id_in;
+    uint64_t *id_out;
+};
+
+SpectralIO io_in_place(const lp_ctx *c)
+{
+    const lp_ctx::Set n = c->now();
+    return SpectralIO{ n.x, n.y, n.z, n.chi, n.x, n.y, n.z, n.chi, nullptr, nullptr, nullptr };
+}
+
 // p0, pcount: the particles [p0, p0 + pcount) only (pcount < 0: all)
-// pos_in: [3][np] positions to read instead of the bound x, y, z (right after a re-sort), or NULL
-lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cudaStream_t s,
-                      long long p0 = 0, long long pcount = -1, const double *pos_in = nullptr)
+lp_status do_spectral(lp_ctx *c, double dt, const SpectralIO &io, bool fused, cudaStream_t s,
+                      long long p0 = 0, long long pcount = -1)
 {
     LpSpectralArgs a;
     a.g = c->geom;
     a.cand = c->cand;
     a.status = c->at<int32_t>(c->lay.status);
     a.cells = c->cells();
-    a.x = c->x; a.y = c->y; a.z = c->z;
-    a.xin = pos_in ? pos_in : c->x;
-    a.yin = pos_in ? pos_in + c->cfg.np : c->y;
-    a.zin = pos_in ? pos_in + 2 * c->cfg.np : c->z;
+    a.x = io.x; a.y = io.y; a.z = io.z;
+    a.xin = io.xin; a.yin = io.yin; a.zin = io.zin;
+    a.perm = io.perm; a.id_in = io.id_in; a.id_out = io.id_out;
     a.rho_old = c->at<double>(c->lay.rho_old);
-    a.chi_in = chi_in;
-    a.chi_out = c->chi;
+    a.chi_in = io.chi_in;
+    a.chi_out = io.chi_out;
     a.tab = c->tab;
     a.nsub_ws = c->at<int32_t>(c->lay.nsub);
     a.nsub_user = c->nsub_user;
@@ -296,14 +326,11 @@ lp_status do_spectral(lp_ctx *c, double dt, const double *chi_in, bool fused, cu
     return st;
 }
 
-// sort: permutation, then x, y, z, id through scratch; chi rows into chi_alt.
-// in_place = true (lp_sort): everything is copied back into the bound arrays.
-// in_place = false (lp_step): ids go back, the permuted positions stay in the x* scratch and the permuted
-// rows in chi_alt for the fused kernel to read (it writes the bound arrays), which saves four array copies.
-lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
+// The permutation into (cell key, id) order of the current particles: perm[n] = index now of the n-th.
+lp_status sort_permutation(lp_ctx *c, uint32_t **perm, cudaStream_t s)
 {
     const long long np = c->cfg.np;
-    if (np == 0) return LP_OK;
+    const lp_ctx::Set n = c->now();
     LpSortBufs b;
     b.key = c->at<uint32_t>(c->lay.key);
     b.idx_a = c->at<uint32_t>(c->lay.idx_a);
@@ -311,7 +338,6 @@ lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
     b.hist = c->at<uint32_t>(c->lay.hist);
     b.hist_elems = c->lay.hist_elems;
     b.digit = c->at<uint8_t>(c->lay.lost);          // the per-particle `lost` buffer is dead across a re-sort
-    uint32_t *perm = nullptr;
     lp_status st;
     if (c->id_bits_stale) {
         // number of radix passes over the ids = bit length of the largest id among the current particles.
@@ -319,34 +345,62 @@ lp_status do_sort(lp_ctx *c, bool in_place, cudaStream_t s)
         // count, host copy); this is the one place a sort synchronises.
         unsigned long long *d = c->at<unsigned long long>(c->lay.maxid), h = 0;
         LP_CUDA(c, cudaMemsetAsync(d, 0, 8, s));
-        if ((st = count(c, lp_launch_max_u64(c->id, np, d, s), "lp_max_u64_kernel launch")) != LP_OK) return st;
+        if ((st = count(c, lp_launch_max_u64(n.id, np, d, s), "lp_max_u64_kernel launch")) != LP_OK) return st;
         LP_CUDA(c, cudaMemcpyAsync(&h, d, 8, cudaMemcpyDeviceToHost, s));
         LP_CUDA(c, cudaStreamSynchronize(s));
         c->id_bits = bit_length(h);
         c->id_bits_stale = false;
     }
-    st = count(c, lp_launch_sort_perm(c->geom, c->x, c->y, c->z, c->id, np, c->id_bits, c->key_bits, b, &perm, s),
-                         "sort kernels launch");
-    if (st != LP_OK) return st;
-    double *sx = c->at<double>(c->lay.xs);
-    uint64_t *sid = c->at<uint64_t>(c->lay.alt_id);
-    double *chi_alt = c->at<double>(c->lay.chi_alt);
-    const double *pos_src[3] = { c->x, c->y, c->z };
-    for (int d = 0; d < 3; ++d)
-        if ((st = count(c, lp_launch_permute_f64(perm, pos_src[d], sx + (size_t)d * np, np, s), "permute launch")) != LP_OK) return st;
-    if ((st = count(c, lp_launch_permute_u64(perm, c->id, sid, np, s), "permute launch")) != LP_OK) return st;
-    if ((st = count(c, lp_launch_permute_rows(perm, c->chi, chi_alt, np, c->cfg.nbins, s), "permute launch")) != LP_OK) return st;
-    LP_CUDA(c, cudaMemcpyAsync(c->id, sid, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
-    if (in_place) {
-        double *pos[3] = { c->x, c->y, c->z };
-        for (int d = 0; d < 3; ++d)
-            LP_CUDA(c, cudaMemcpyAsync(pos[d], sx + (size_t)d * np, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
-        LP_CUDA(c, cudaMemcpyAsync(c->chi, chi_alt, (size_t)np * c->cfg.nbins * 8, cudaMemcpyDeviceToDevice, s));
-    }
+    return count(c, lp_launch_sort_perm(c->geom, n.x, n.y, n.z, n.id, np, c->id_bits, c->key_bits, b, perm, s),
+                 "sort kernels launch");
+}
+
+void sort_invalidates(lp_ctx *c)
+{
     c->stage0_done = false; c->rk3_next = 0; c->push_done = false;      // k1 / x* / rho_old refer to the old order
     c->spectra_done = false;     // so do the per-particle n_sub / lost of the last update
     c->status_valid = false;
     ++c->sorts;
+}
+
+// Apply the permutation with the permute kernels.
+//  * ping-pong: current set -> other set, which becomes the current one (no copy back).
+//  * otherwise through scratch (x* buffer, alt_id, chi_alt).  in_place = true (lp_sort): everything is copied
+//    back into the bound arrays.  in_place = false (lp_step without ping-pong): the ids go back, the permuted
+//    positions stay in the x* scratch and the permuted rows in chi_alt for the fused kernel to read (it writes
+//    the bound arrays), which saves four array copies; *io describes that launch.
+lp_status do_sort(lp_ctx *c, bool in_place, SpectralIO *io, cudaStream_t s)
+{
+    const long long np = c->cfg.np;
+    if (np == 0) return LP_OK;
+    uint32_t *perm = nullptr;
+    lp_status st = sort_permutation(c, &perm, s);
+    if (st != LP_OK) return st;
+    const lp_ctx::Set n = c->now();
+    lp_ctx::Set o = c->other();
+    if (!c->pingpong) {
+        double *sx = c->at<double>(c->lay.xs);
+        o = lp_ctx::Set{ sx, sx + np, sx + 2 * np, c->at<uint64_t>(c->lay.alt_id), c->at<double>(c->lay.chi_alt) };
+    }
+    const double *pos_src[3] = { n.x, n.y, n.z };
+    double *pos_dst[3] = { o.x, o.y, o.z };
+    for (int d = 0; d < 3; ++d)
+        if ((st = count(c, lp_launch_permute_f64(perm, pos_src[d], pos_dst[d], np, s), "permute launch")) != LP_OK) return st;
+    if ((st = count(c, lp_launch_permute_u64(perm, n.id, o.id, np, s), "permute launch")) != LP_OK) return st;
+    if ((st = count(c, lp_launch_permute_rows(perm, n.chi, o.chi, np, c->cfg.nbins, s), "permute launch")) != LP_OK) return st;
+    if (c->pingpong) {
+        c->cur ^= 1;
+    } else {
+        LP_CUDA(c, cudaMemcpyAsync(n.id, o.id, (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
+        if (in_place) {
+            for (int d = 0; d < 3; ++d)
+                LP_CUDA(c, cudaMemcpyAsync(const_cast<double *>(pos_src[d]), pos_dst[d], (size_t)np * 8, cudaMemcpyDeviceToDevice, s));
+            LP_CUDA(c, cudaMemcpyAsync(n.chi, o.chi, (size_t)np * c->cfg.nbins * 8, cudaMemcpyDeviceToDevice, s));
+        } else if (io) {
+            *io = SpectralIO{ o.x, o.y, o.z, o.chi, n.x, n.y, n.z, n.chi, nullptr, nullptr, nullptr };
+        }
+    }
+    sort_invalidates(c);
     return LP_OK;
 }
 
@@ -443,6 +497,7 @@ lp_status lp_bind_particles(lp_ctx *ctx, double *x, double *y, double *z, uint64
     if (ctx->cfg.np > 0 && (!x || !y || !z || !id || !chi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL particle array");
     if (reinterpret_cast<uintptr_t>(chi) % 16) return fail(ctx, LP_ERR_INVALID_ARG, "chi not 16-byte aligned");
     ctx->x = x; ctx->y = y; ctx->z = z; ctx->id = id; ctx->chi = chi;
+    ctx->cur = 0;                       // the state is what the caller just bound
     ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
     ctx->spectra_done = false;
     ctx->status_valid = false;
@@ -481,7 +536,8 @@ lp_status lp_interpolate(lp_ctx *ctx, double *out7, uint32_t *cell_key, void *st
     if (!out7 && !cell_key) return LP_OK;
     if (ctx->cfg.np == 0) return LP_OK;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    return count(ctx, lp_launch_interpolate(ctx->geom, ctx->cells(), ctx->x, ctx->y, ctx->z, ctx->cfg.np, out7, cell_key,
+    const lp_ctx::Set n = ctx->now();
+    return count(ctx, lp_launch_interpolate(ctx->geom, ctx->cells(), n.x, n.y, n.z, ctx->cfg.np, out7, cell_key,
                                             static_cast<cudaStream_t>(stream)), "lp_interpolate_kernel launch");
 }
 
@@ -490,7 +546,7 @@ lp_status lp_sort(lp_ctx *ctx, void *stream)
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    return do_sort(ctx, true, static_cast<cudaStream_t>(stream));
+    return do_sort(ctx, true, nullptr, static_cast<cudaStream_t>(stream));
 }
 
 lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream)
@@ -541,7 +597,7 @@ lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
         return fail(ctx, LP_ERR_STATE, "lp_spectral_update needs the push finished (lp_push stage 1 / lp_push_rk3 stage 2)");
     if (ctx->cfg.np == 0) return LP_OK;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    return do_spectral(ctx, dt, ctx->chi, false, static_cast<cudaStream_t>(stream));
+    return do_spectral(ctx, dt, io_in_place(ctx), false, static_cast<cudaStream_t>(stream));
 }
 
 lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void *stream)
@@ -551,7 +607,7 @@ lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void *stream
     if (ctx->cfg.np == 0) return LP_OK;
     if (!r) return fail(ctx, LP_ERR_INVALID_ARG, "r is NULL");
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    return count(ctx, lp_launch_shock(ctx->tab, r, q_r, ctx->chi, ctx->cfg.np, ctx->cfg.nbins, ctx->sm_count,
+    return count(ctx, lp_launch_shock(ctx->tab, r, q_r, ctx->now().chi, ctx->cfg.np, ctx->cfg.nbins, ctx->sm_count,
                                       static_cast<cudaStream_t>(stream)), "lp_shock_kernel launch");
 }
 
@@ -570,8 +626,8 @@ lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *st
     unsigned long long *counts = ctx->at<unsigned long long>(ctx->lay.partial), h_counts[2] = { 0, 0 };
     st = count(ctx, lp_launch_compact(flag, ctx->cfg.np, ctx->cfg.nbins, ctx->at<uint32_t>(ctx->lay.hist),
                                       ctx->at<uint32_t>(ctx->lay.idx_a), ctx->at<uint32_t>(ctx->lay.idx_b),
-                                      ctx->at<uint32_t>(ctx->lay.key), counts, ctx->x, ctx->y, ctx->z, ctx->id,
-                                      ctx->chi, ctx->sm_count, s), "compaction kernels launch");
+                                      ctx->at<uint32_t>(ctx->lay.key), counts, ctx->now().x, ctx->now().y, ctx->now().z,
+                                      ctx->now().id, ctx->now().chi, ctx->sm_count, s), "compaction kernels launch");
     if (st != LP_OK) return st;
     LP_CUDA(ctx, cudaMemcpyAsync(h_counts, counts, sizeof h_counts, cudaMemcpyDeviceToHost, s));
     LP_CUDA(ctx, cudaStreamSynchronize(s));
@@ -605,6 +661,39 @@ lp_status lp_set_count(lp_ctx *ctx, int64_t np_new)
     return LP_OK;
 }
 
+lp_status lp_set_pingpong(lp_ctx *ctx, int enable, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    if (!enable && ctx->cur != 0 && ctx->cfg.np > 0) {        // bring the state home to the bound arrays
+        LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+        cudaStream_t s = static_cast<cudaStream_t>(stream);
+        const lp_ctx::Set n = ctx->now(), b = ctx->set(0);
+        const size_t np = (size_t)ctx->cfg.np;
+        LP_CUDA(ctx, cudaMemcpyAsync(b.x, n.x, np * 8, cudaMemcpyDeviceToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(b.y, n.y, np * 8, cudaMemcpyDeviceToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(b.z, n.z, np * 8, cudaMemcpyDeviceToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(b.id, n.id, np * 8, cudaMemcpyDeviceToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(b.chi, n.chi, np * (size_t)ctx->cfg.nbins * 8, cudaMemcpyDeviceToDevice, s));
+    }
+    if (!enable) ctx->cur = 0;
+    ctx->pingpong = enable != 0;
+    return LP_OK;
+}
+
+lp_status lp_current_particles(const lp_ctx *ctx, double **x, double **y, double **z, uint64_t **id, double **chi)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (!ctx->ws || (ctx->cfg.np > 0 && !ctx->x)) return LP_ERR_STATE;
+    const lp_ctx::Set n = ctx->now();
+    if (x) *x = n.x;
+    if (y) *y = n.y;
+    if (z) *z = n.z;
+    if (id) *id = n.id;
+    if (chi) *chi = n.chi;
+    return LP_OK;
+}
+
 lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
 {
     lp_status st = need_ready(ctx, true);
@@ -613,17 +702,27 @@ lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
     if (ctx->cfg.np == 0) return LP_OK;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    const double *chi_in = ctx->chi, *pos_in = nullptr;
     const bool sort_now = ctx->cfg.sort_every > 0 && (ctx->steps - 1) % ctx->cfg.sort_every == 0;
-    if (sort_now) {
+    SpectralIO io = io_in_place(ctx);
+    bool flip = false;
+    if (sort_now && ctx->pingpong) {
+        // the re-sort is folded into the fused kernel: it reads the current set through the permutation
+        // and writes the other set in the new order -- no permute pass, no copy back
+        uint32_t *perm = nullptr;
+        if ((st = sort_permutation(ctx, &perm, s)) != LP_OK) return st;
+        const lp_ctx::Set n = ctx->now(), o = ctx->other();
+        io = SpectralIO{ n.x, n.y, n.z, n.chi, o.x, o.y, o.z, o.chi, perm, n.id, o.id };
+        sort_invalidates(ctx);
+        flip = true;
+    } else if (sort_now) {
         // the permuted rows and positions stay in the workspace; the fused kernel reads them from there
         // and writes the bound arrays
-        if ((st = do_sort(ctx, false, s)) != LP_OK) return st;
-        chi_in = ctx->at<double>(ctx->lay.chi_alt);
-        pos_in = ctx->at<double>(ctx->lay.xs);
+        if ((st = do_sort(ctx, false, &io, s)) != LP_OK) return st;
     }
     // frozen fields: both push stages run inside the spectral kernel's per-particle phase
-    return do_spectral(ctx, dt, chi_in, true, s, 0, -1, pos_in);
+    st = do_spectral(ctx, dt, io, true, s);
+    if (st == LP_OK && flip) ctx->cur ^= 1;
+    return st;
 }
 
 lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *hz, uint64_t *hid, double *hchi,
@@ -641,20 +740,22 @@ lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *h
     if (np < kMinPipelined || sort_now) {
         // whole arrays in, one lp_step, whole arrays out (a re-sort needs every row on the device first)
         if (np) {
-            LP_CUDA(ctx, cudaMemcpyAsync(ctx->x, hx, np * 8, cudaMemcpyHostToDevice, s));
-            LP_CUDA(ctx, cudaMemcpyAsync(ctx->y, hy, np * 8, cudaMemcpyHostToDevice, s));
-            LP_CUDA(ctx, cudaMemcpyAsync(ctx->z, hz, np * 8, cudaMemcpyHostToDevice, s));
-            LP_CUDA(ctx, cudaMemcpyAsync(ctx->id, hid, np * 8, cudaMemcpyHostToDevice, s));
-            LP_CUDA(ctx, cudaMemcpyAsync(ctx->chi, hchi, np * nb * 8, cudaMemcpyHostToDevice, s));
+            const lp_ctx::Set n = ctx->now();
+            LP_CUDA(ctx, cudaMemcpyAsync(n.x, hx, np * 8, cudaMemcpyHostToDevice, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(n.y, hy, np * 8, cudaMemcpyHostToDevice, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(n.z, hz, np * 8, cudaMemcpyHostToDevice, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(n.id, hid, np * 8, cudaMemcpyHostToDevice, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(n.chi, hchi, np * nb * 8, cudaMemcpyHostToDevice, s));
             ctx->id_bits_stale = true;                  // the host may hand in other ids than last time
         }
         if ((st = lp_step(ctx, dt, stream)) != LP_OK) return st;
         if (np) {
-            LP_CUDA(ctx, cudaMemcpyAsync(hx, ctx->x, np * 8, cudaMemcpyDeviceToHost, s));
-            LP_CUDA(ctx, cudaMemcpyAsync(hy, ctx->y, np * 8, cudaMemcpyDeviceToHost, s));
-            LP_CUDA(ctx, cudaMemcpyAsync(hz, ctx->z, np * 8, cudaMemcpyDeviceToHost, s));
-            LP_CUDA(ctx, cudaMemcpyAsync(hid, ctx->id, np * 8, cudaMemcpyDeviceToHost, s));
-            LP_CUDA(ctx, cudaMemcpyAsync(hchi, ctx->chi, np * nb * 8, cudaMemcpyDeviceToHost, s));
+            const lp_ctx::Set n = ctx->now();            // (a folded re-sort has moved the state to the other set)
+            LP_CUDA(ctx, cudaMemcpyAsync(hx, n.x, np * 8, cudaMemcpyDeviceToHost, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(hy, n.y, np * 8, cudaMemcpyDeviceToHost, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(hz, n.z, np * 8, cudaMemcpyDeviceToHost, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(hid, n.id, np * 8, cudaMemcpyDeviceToHost, s));
+            LP_CUDA(ctx, cudaMemcpyAsync(hchi, n.chi, np * nb * 8, cudaMemcpyDeviceToHost, s));
         }
         LP_CUDA(ctx, cudaStreamSynchronize(s));
         return LP_OK;
@@ -672,33 +773,34 @@ lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *h
             ctx->ev_pipe.push_back(e);
         }
     }
+    const lp_ctx::Set n = ctx->now();
     cudaEvent_t *ev_in = ctx->ev_pipe.data(), *ev_k = ev_in + kBatches;
     cudaEvent_t ev_start = ctx->ev_pipe[2 * kBatches], ev_done = ctx->ev_pipe[2 * kBatches + 1];
     const size_t per = ((np + kBatches - 1) / kBatches + 31) / 32 * 32;
     LP_CUDA(ctx, cudaEventRecord(ev_start, s));                 // copies start after earlier work on s
     LP_CUDA(ctx, cudaStreamWaitEvent(ctx->s_in, ev_start, 0));
     LP_CUDA(ctx, cudaStreamWaitEvent(ctx->s_out, ev_start, 0));
-    LP_CUDA(ctx, cudaMemcpyAsync(ctx->x, hx, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
-    LP_CUDA(ctx, cudaMemcpyAsync(ctx->y, hy, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
-    LP_CUDA(ctx, cudaMemcpyAsync(ctx->z, hz, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
-    LP_CUDA(ctx, cudaMemcpyAsync(ctx->id, hid, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    LP_CUDA(ctx, cudaMemcpyAsync(n.x, hx, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    LP_CUDA(ctx, cudaMemcpyAsync(n.y, hy, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    LP_CUDA(ctx, cudaMemcpyAsync(n.z, hz, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    LP_CUDA(ctx, cudaMemcpyAsync(n.id, hid, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
     ++ctx->steps;
     for (int b = 0; b < kBatches; ++b) {
         const size_t p0 = (size_t)b * per;
         if (p0 >= np) break;
         const size_t cnt = std::min(per, np - p0);
-        LP_CUDA(ctx, cudaMemcpyAsync(ctx->chi + p0 * nb, hchi + p0 * nb, cnt * nb * 8, cudaMemcpyHostToDevice, ctx->s_in));
+        LP_CUDA(ctx, cudaMemcpyAsync(n.chi + p0 * nb, hchi + p0 * nb, cnt * nb * 8, cudaMemcpyHostToDevice, ctx->s_in));
         LP_CUDA(ctx, cudaEventRecord(ev_in[b], ctx->s_in));
         LP_CUDA(ctx, cudaStreamWaitEvent(s, ev_in[b], 0));
-        if ((st = do_spectral(ctx, dt, ctx->chi, true, s, (long long)p0, (long long)cnt)) != LP_OK) return st;
+        if ((st = do_spectral(ctx, dt, io_in_place(ctx), true, s, (long long)p0, (long long)cnt)) != LP_OK) return st;
         LP_CUDA(ctx, cudaEventRecord(ev_k[b], s));
         LP_CUDA(ctx, cudaStreamWaitEvent(ctx->s_out, ev_k[b], 0));
-        LP_CUDA(ctx, cudaMemcpyAsync(hchi + p0 * nb, ctx->chi + p0 * nb, cnt * nb * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+        LP_CUDA(ctx, cudaMemcpyAsync(hchi + p0 * nb, n.chi + p0 * nb, cnt * nb * 8, cudaMemcpyDeviceToHost, ctx->s_out));
     }
     // positions are final once the last batch has run (s_out already waits for it); ids are unchanged
-    LP_CUDA(ctx, cudaMemcpyAsync(hx, ctx->x, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
-    LP_CUDA(ctx, cudaMemcpyAsync(hy, ctx->y, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
-    LP_CUDA(ctx, cudaMemcpyAsync(hz, ctx->z, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+    LP_CUDA(ctx, cudaMemcpyAsync(hx, n.x, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+    LP_CUDA(ctx, cudaMemcpyAsync(hy, n.y, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+    LP_CUDA(ctx, cudaMemcpyAsync(hz, n.z, np * 8, cudaMemcpyDeviceToHost, ctx->s_out));
     LP_CUDA(ctx, cudaEventRecord(ev_done, ctx->s_out));
     LP_CUDA(ctx, cudaStreamWaitEvent(s, ev_done, 0));
     LP_CUDA(ctx, cudaStreamSynchronize(s));
@@ -724,7 +826,7 @@ lp_status lp_get_diag(lp_ctx *ctx, lp_diag *out, void *stream)
     if (!have) LP_CUDA(ctx, cudaMemsetAsync(ctx->at<int32_t>(ctx->lay.nsub), 0, (size_t)ctx->cfg.np * 4, s));
     st = count(ctx, lp_launch_diag(ctx->at<int32_t>(ctx->lay.nsub),
                                    (have && ctx->lost_user) ? ctx->at<double>(ctx->lay.lost) : nullptr,
-                                   ctx->status_valid ? ctx->at<int32_t>(ctx->lay.status) : nullptr, ctx->chi, ctx->tab,
+                                   ctx->status_valid ? ctx->at<int32_t>(ctx->lay.status) : nullptr, ctx->now().chi, ctx->tab,
                                    ctx->cfg.nbins, ctx->cfg.np, ctx->at<double>(ctx->lay.partial), d, s),
                "lp_diag_kernel launch");
     if (st != LP_OK) return st;

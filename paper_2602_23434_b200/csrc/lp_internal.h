@@ -40,7 +40,14 @@ struct LpSpectralArgs {
     LpLamCand cand;
     LpCells cells;
     double *x, *y, *z;           // staged: x^{n+1} (read only).  fused: x^{n+1} out
-    const double *xin, *yin, *zin;   // positions read (== x, y, z except right after a re-sort: permuted scratch)
+    const double *xin, *yin, *zin;   // positions read (== x, y, z unless the step re-sorts: the other buffer set)
+    // Re-sort folded into the fused step (lp_step on a sort step, ping-pong buffers): particle p of the new
+    // order is the particle stored at index perm[p] of xin, yin, zin, id_in and chi_in; everything is written
+    // at index p of the other buffer set (x, y, z, id_out, chi_out), so the row permute costs no pass of its
+    // own.  perm == NULL: identity (no re-sort), id_in / id_out unused.
+    const uint32_t *perm;
+    const uint64_t *id_in;
+    uint64_t *id_out;
     const double *rho_old;       // staged: from push stage 0.  fused: unused
     int32_t *status;             // fused: outside-box flags [np]
     const double *chi_in;        // [np][nbins]  (may differ from chi_out after a re-sort)

@@ -505,11 +505,14 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
     for (long long chunk = gw; chunk < nchunks; chunk += nw) {
         const long long base = chunk << 5;
         const bool have = base + lane < A.np;
-        const double px = have ? A.xin[base + lane] : 0.0, py = have ? A.yin[base + lane] : 0.0,
-                     pz = have ? A.zin[base + lane] : 0.0;
+        // source index of this lane's particle (a re-sort folded into the step reads through the permutation)
+        const long long src = have ? (A.perm ? (long long)A.perm[base + lane] : base + lane) : 0;
+        auto src_of = [&](int j) -> long long { return __shfl_sync(kFull, src, j); };
+        const double px = have ? A.xin[src] : 0.0, py = have ? A.yin[src] : 0.0, pz = have ? A.zin[src] : 0.0;
+        if (A.perm && have) A.id_out[base + lane] = A.id_in[src];
         double2 ahead[kStaged ? M / 2 : 1];                 // (staged, U == 1) the next row, fetched a row ahead
         if constexpr (kStaged) {
-            if (base < A.np) LpStage<M>::fetch(A.chi_in + base * NB, lane, ahead);      // flies during phase 1
+            if (base < A.np) LpStage<M>::fetch(A.chi_in + src_of(0) * NB, lane, ahead);      // flies during phase 1
         }
         lp_chunk_phase1<NB, FUSED>(A, base, lane, px, py, pz, sE, sR, sAC[warp], sNS[warp]);
         for (int j0 = 0; j0 < 32; j0 += U) {
@@ -517,12 +520,13 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const long long pj = base + j0 + u;
+                const long long sj = src_of(j0 + u), sj1 = src_of((j0 + u + 1) & 31);      // (all lanes shuffle)
                 if (pj < A.np) {
                     if constexpr (kStaged) {
                         LpStage<M>::place(ahead, sStage[warp], lane, buf[u]);
-                        if (j0 + 1 < 32 && pj + 1 < A.np) LpStage<M>::fetch(A.chi_in + (pj + 1) * NB, lane, ahead);
+                        if (j0 + 1 < 32 && pj + 1 < A.np) LpStage<M>::fetch(A.chi_in + sj1 * NB, lane, ahead);
                     } else {
-                        lp_load_row<M>(A.chi_in + pj * NB + lane * M, buf[u]);
+                        lp_load_row<M>(A.chi_in + sj * NB + lane * M, buf[u]);
                     }
                 } else {
 #pragma unroll
@@ -770,22 +774,40 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
 
     if (warp < NP) {
         // ---------------------------------------------------------------- particle warp
-        // positions are fetched one chunk ahead, so that their latency is off the dependent chain
+        // positions are fetched one chunk ahead, so that their latency is off the dependent chain; when the
+        // step re-sorts (A.perm) they are read through the permutation, whose entries are fetched a chunk
+        // earlier still, and the ids move with them
         auto chunk_of = [&](uint32_t t) -> uint32_t { return (blockIdx.x + t * gridDim.x) << 5; };
+        const uint32_t *perm = A.perm;
+        auto own_index = [&](uint32_t t, bool &valid) -> uint32_t {      // index of this lane's particle of chunk t
+            valid = t < nblk && chunk_of(t) + lane < np;
+            return valid ? chunk_of(t) + lane : 0u;
+        };
         double nx = 0.0, ny = 0.0, nz = 0.0;
-        if ((uint32_t)warp < nblk && chunk_of(warp) + lane < np) {
-            const size_t p = (size_t)chunk_of(warp) + lane;
-            nx = __ldcs(A.xin + p); ny = __ldcs(A.yin + p); nz = __ldcs(A.zin + p);   // touched once: streaming
+        uint32_t q1 = 0;                    // perm entry of this lane's particle of the chunk after next
+        {
+            bool v0, v1;
+            const uint32_t p0 = own_index(warp, v0), p1 = own_index(warp + NP, v1);
+            if (v0) {
+                const size_t p = perm ? (size_t)perm[p0] : (size_t)p0;
+                nx = __ldcs(A.xin + p); ny = __ldcs(A.yin + p); nz = __ldcs(A.zin + p);   // touched once: streaming
+                if (perm) __stcs(A.id_out + p0, __ldcs(A.id_in + p));
+            }
+            if (perm && v1) q1 = perm[p1];
         }
 #pragma unroll 1
         for (uint32_t t = warp; t < nblk; t += NP) {
             const uint32_t cs = t % D, use = t / D;
             const uint32_t base = chunk_of(t);
             const double px = nx, py = ny, pz = nz;
-            if (t + NP < nblk && chunk_of(t + NP) + lane < np) {
-                const size_t p = (size_t)chunk_of(t + NP) + lane;
+            bool v1, v2;
+            const uint32_t p1 = own_index(t + NP, v1), p2 = own_index(t + 2 * NP, v2);
+            if (v1) {
+                const size_t p = perm ? (size_t)q1 : (size_t)p1;
                 nx = __ldcs(A.xin + p); ny = __ldcs(A.yin + p); nz = __ldcs(A.zin + p);   // touched once: streaming
+                if (perm) __stcs(A.id_out + p1, __ldcs(A.id_in + p));
             }
+            if (perm && v2) q1 = perm[p2];
             if (use >= 1) lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u);
             lp_chunk_phase1<NB, FUSED>(A, (long long)base, lane, px, py, pz, sE, sR, sAC + cs * 32, sNS + cs * 32);
             if (lane == 0) lp_mbar_arrive(full_u32 + 8 * cs);      // (lp_chunk_phase1 ends with __syncwarp)
@@ -810,8 +832,9 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
     constexpr bool kHint = (LP_BULK_L2HINT != 0) && NB <= 128;
     const uint64_t pol = lp_policy_evict_first();
     auto chunk_base = [&](uint32_t k) -> uint32_t { return (blockIdx.x + (rw + k * NR) * gridDim.x) << 5; };
-    auto issue_load = [&](uint32_t j, int slot) {        // lane 0 only
-        const uint32_t row0 = chunk_base(j / GPC) + (j % GPC) * R;
+    auto group_row0 = [&](uint32_t j) -> uint32_t { return chunk_base(j / GPC) + (j % GPC) * R; };
+    auto issue_load = [&](uint32_t j, int slot) {        // lane 0 only: the group's rows are contiguous
+        const uint32_t row0 = group_row0(j);
         if (row0 < np) {
             const uint32_t left = np - row0;
             const uint32_t bytes = (left < (uint32_t)R ? left : (uint32_t)R) * C::ROW_BYTES;
@@ -819,7 +842,34 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
             lp_bulk_load<kHint>(ring_u32 + slot * C::SLOT_BYTES, A.chi_in + (size_t)row0 * NB, bytes, bar_u32 + 8 * slot, pol);
         }
     };
-    if (lane == 0) {
+    // Re-sort folded into the step: row r of the group comes from row perm[row0 + r] of chi_in -- one bulk copy
+    // per row, issued by lane r, all completing on the slot's barrier.  Whole warp calls; `src` = this lane's
+    // perm entry for the group (fetched an iteration ahead, so that its latency is not on the issue path).
+    const uint32_t *perm = A.perm;
+    auto perm_entry = [&](uint32_t j) -> uint32_t {      // perm[row0(j) + lane], 0 if there is no such row
+        if (j >= ngroups || lane >= R) return 0u;
+        const uint32_t r = group_row0(j) + lane;
+        return r < np ? perm[r] : 0u;
+    };
+    auto issue_load_perm = [&](uint32_t j, int slot, uint32_t src) {
+        const uint32_t row0 = group_row0(j);
+        if (row0 < np) {
+            const uint32_t left = np - row0;
+            const uint32_t nrows = left < (uint32_t)R ? left : (uint32_t)R;
+            if (lane == 0) lp_mbar_expect_tx(bar_u32 + 8 * slot, nrows * C::ROW_BYTES);
+            __syncwarp();
+            if ((uint32_t)lane < nrows)
+                lp_bulk_load<kHint>(ring_u32 + slot * C::SLOT_BYTES + lane * C::ROW_BYTES, A.chi_in + (size_t)src * NB,
+                                    C::ROW_BYTES, bar_u32 + 8 * slot, pol);
+        }
+    };
+    uint32_t src_next = 0;          // (perm) this lane's entry for the next group to be loaded
+    if (perm) {
+#pragma unroll
+        for (int k = 0; k < S; ++k)
+            if ((uint32_t)k < ngroups) issue_load_perm(k, k, perm_entry(k));
+        src_next = perm_entry(S);
+    } else if (lane == 0) {
 #pragma unroll
         for (int k = 0; k < S; ++k)
             if ((uint32_t)k < ngroups) issue_load(k, k);
@@ -901,9 +951,15 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
             }
             // refill the slot drained in the previous iteration (its store may still be reading: wait
             // for all but the newest store group), keeping S-1 loads in flight
-            if (lane == 0 && q >= 1 && q + (S - 1) < ngroups) {
-                lp_bulk_wait_read<1>();
-                issue_load(q + (S - 1), pslot);
+            if (q >= 1 && q + (S - 1) < ngroups) {
+                if (lane == 0) lp_bulk_wait_read<1>();
+                if (perm) {
+                    __syncwarp();                                   // lane 0's stores have left the slot
+                    issue_load_perm(q + (S - 1), pslot, src_next);
+                    src_next = perm_entry(q + S);
+                } else if (lane == 0) {
+                    issue_load(q + (S - 1), pslot);
+                }
             }
 #endif
             pslot = slot;

@@ -18,7 +18,8 @@ class LP:
         off = (-self.workspace.data_ptr()) % 256
         B.lp_bind_workspace(self.ctx, self.workspace.data_ptr() + off, nbytes)
         self.workspace_bytes = nbytes
-        self.x = self.y = self.z = self.id = self.chi = None
+        self._bound = None            # the caller-side tensors x, y, z, id, chi (the bound arrays)
+        self.capacity = cfg.np
         self.nsub = self.lost = None
         self._fields = None
 
@@ -47,13 +48,41 @@ class LP:
     def bind_particles(self, x, y, z, pid, chi):
         import numpy as np
         n, nb = self.cfg.np, self.cfg.nbins
-        self.x = self._dev(x, torch.float64); self.y = self._dev(y, torch.float64); self.z = self._dev(z, torch.float64)
+        bx = self._dev(x, torch.float64); by = self._dev(y, torch.float64); bz = self._dev(z, torch.float64)
         pid = torch.as_tensor(np.ascontiguousarray(pid).view(np.int64)) if not torch.is_tensor(pid) else pid
-        self.id = pid.to(self.device).contiguous()
-        self.chi = self._dev(chi, torch.float64)
-        assert self.x.numel() == n and self.chi.shape == (n, nb) and self.id.numel() == n
-        B.lp_bind_particles(self.ctx, self.x.data_ptr(), self.y.data_ptr(), self.z.data_ptr(),
-                            self.id.data_ptr(), self.chi.data_ptr())
+        bid = pid.to(self.device).contiguous()
+        bchi = self._dev(chi, torch.float64)
+        assert bx.numel() == n and bchi.shape == (n, nb) and bid.numel() == n
+        B.lp_bind_particles(self.ctx, bx.data_ptr(), by.data_ptr(), bz.data_ptr(), bid.data_ptr(), bchi.data_ptr())
+        self._bound = (bx, by, bz, bid, bchi)
+
+    def set_pingpong(self, enable=True):
+        """Let a re-sort leave the state in the workspace twins of the bound arrays (no copy back): x, y, z,
+        id, chi of this object then follow lp_current_particles."""
+        B.lp_set_pingpong(self.ctx, enable, self.stream)
+
+    def _view(self, ptr, elems, dtype):
+        """A tensor over `elems` elements of the workspace starting at device address ptr (no copy)."""
+        off = ptr - self.workspace.data_ptr()
+        assert 0 <= off and off + elems * 8 <= self.workspace.numel()
+        return self.workspace[off: off + elems * 8].view(dtype)
+
+    def current(self):
+        """The tensors that hold the particle state now: (x, y, z, id, chi) -- the bound ones, or (ping-pong,
+        after a re-sort) views of their workspace twins.  Length = the capacity the context was created with."""
+        ptrs = B.lp_current_particles(self.ctx)
+        if ptrs[0] == self._bound[0].data_ptr():
+            return self._bound
+        n, nb = self.capacity, self.cfg.nbins
+        return (self._view(ptrs[0], n, torch.float64), self._view(ptrs[1], n, torch.float64),
+                self._view(ptrs[2], n, torch.float64), self._view(ptrs[3], n, torch.int64),
+                self._view(ptrs[4], n * nb, torch.float64).view(n, nb))
+
+    x = property(lambda self: self.current()[0])
+    y = property(lambda self: self.current()[1])
+    z = property(lambda self: self.current()[2])
+    id = property(lambda self: self.current()[3])
+    chi = property(lambda self: self.current()[4])
 
     def bind_diag(self, nsub=True, lost=True):
         n = self.cfg.np
@@ -75,10 +104,6 @@ class LP:
         B.lp_interpolate(self.ctx, out7.data_ptr() if want_fields else None,
                          key.data_ptr() if want_key else None, self.stream)
         return out7, key
-
-    def current(self):
-        """The tensors that hold the particle state now: (x, y, z, id, chi)."""
-        return self.x, self.y, self.z, self.id, self.chi
 
     def sort(self):
         B.lp_sort(self.ctx, self.stream)

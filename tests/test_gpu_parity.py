@@ -23,11 +23,12 @@ def small_turbulent(n=12, np_=1000 + 37, nbins=64, sort_every=0, **kw):
 DIAG_KINDS = ("full", "nsub")      # "nsub": no `lost` output bound = the DIAG=false kernels (what bench.py times)
 
 
-def setup_pair(w, shuffle_ids=False, diag="full", jitter=True):
+def setup_pair(w, shuffle_ids=False, diag="full", jitter=True, pingpong=False):
     """Returns (lp, prm, fields_np, x, y, z, pid, chi) with the GPU side bound to copies.
     diag: "full" binds n_sub and lost (the DIAG=true kernel instantiations), "nsub" binds n_sub only
     (lp_api.cu picks DIAG=false when no `lost` output is bound: the instantiations bench.py times), None
-    binds nothing."""
+    binds nothing.  pingpong: re-sorts leave the state in the workspace twins of the bound arrays
+    (lp_set_pingpong); lp.x, lp.chi ... follow it."""
     fields = I.make_fields(w, device="cpu")
     u_rad = u_rad_of(w, fields)
     f_np = fields_to_numpy(fields)
@@ -38,6 +39,8 @@ def setup_pair(w, shuffle_ids=False, diag="full", jitter=True):
     lp.bind_particles(x, y, z, pid, chi)
     if diag:
         lp.bind_diag(nsub=True, lost=(diag == "full"))
+    if pingpong:
+        lp.set_pingpong(True)
     return lp, oracle_params(w, u_rad), f_np, x, y, z, pid, chi
 
 
@@ -100,13 +103,15 @@ def test_push_positions_bit_exact_over_steps(periodic):
 
 # ------------------------------------------------------------------ a2: sort
 
+@pytest.mark.parametrize("pingpong", [False, True])
 @pytest.mark.parametrize("np_,id_shift", [(1, 33), (31, 33), (4097, 33), (50000, 33), (5003, 62)])
-def test_sort_order_and_permutation_bit_exact(np_, id_shift):
+def test_sort_order_and_permutation_bit_exact(np_, id_shift, pingpong):
     """ids wider than 32 bits (35 and 64 significant bits: five and eight radix passes over the ids)."""
     w = small_turbulent(n=6, np_=np_, nbins=16)          # 216 cells: many ties per key
     lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
     pid = pid + np.uint64(1 << id_shift) * (pid % np.uint64(3))
     lp.bind_particles(x, y, z, pid, chi)
+    lp.set_pingpong(pingpong)
     lp.sort()
     torch.cuda.synchronize()
     sx, sy, sz, sid, schi, skey, perm = oracle_sort_state(prm, x, y, z, pid, chi)
@@ -309,11 +314,14 @@ def test_injection_within_capacity():
 
 # ------------------------------------------------------------------ whole step, with re-sort
 
+@pytest.mark.parametrize("pingpong", [False, True])
 @pytest.mark.parametrize("diag", DIAG_KINDS)
 @pytest.mark.parametrize("nbins,np_", [(64, 6000 + 3), (16, 2500), (128, 1500), (32, 4097), (256, 999), (512, 700)])
-def test_lp_step_with_resort_matches_oracle(nbins, np_, diag):
+def test_lp_step_with_resort_matches_oracle(nbins, np_, diag, pingpong):
+    """Eight fused steps with a re-sort every third.  pingpong: the re-sort is folded into the fused kernel
+    (rows, positions and ids read through the permutation, written to the other buffer set)."""
     w = small_turbulent(n=10, np_=np_, nbins=nbins, sort_every=3)
-    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, diag=diag)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, diag=diag, pingpong=pingpong)
     dt = w.dt
     for s in range(8):
         lp.step(dt)
@@ -327,6 +335,15 @@ def test_lp_step_with_resort_matches_oracle(nbins, np_, diag):
     assert_chi_close(host(lp.chi), chi)
     d = lp.diag()
     assert d["steps"] == 8 and d["sorts"] == 3
+    if pingpong:
+        # three re-sorts: the state is in the workspace twins now; switching ping-pong off brings it home
+        bound = lp._bound
+        assert lp.x.data_ptr() != bound[0].data_ptr()
+        lp.set_pingpong(False)
+        torch.cuda.synchronize()
+        assert lp.x.data_ptr() == bound[0].data_ptr()
+        assert np.array_equal(host(bound[0]), x) and np.array_equal(host(bound[3]).view(np.uint64), pid)
+        assert_chi_close(host(bound[4]), chi)
 
 
 @pytest.mark.parametrize("np_,nbins,sort_every,diag", [
@@ -334,12 +351,14 @@ def test_lp_step_with_resort_matches_oracle(nbins, np_, diag):
     # what bench.py's e2e leg runs: no diagnostics bound at all (DIAG=false kernels), and batch tails that are
     # not multiples of 32 at the bin counts with several ring slots per chunk
     (66000, 64, 2, None), (65536 + 1, 128, 0, None), (65536 + 31, 256, 0, "nsub"), (65536 + 33, 128, 2, "nsub"),
-    (65536 + 33, 512, 0, None)])
+    (65536 + 33, 512, 0, None), (66000, 64, 2, "pingpong"), (65536 + 33, 128, 1, "pingpong")])
 def test_lp_step_host_roundtrip(np_, nbins, sort_every, diag):
     """lp_step on host buffers: whole-array path (small sets, re-sort steps) and the batched pipeline
     (>= 65536 particles: copy-in, kernels and copy-out overlap) must both give the oracle's step."""
     w = small_turbulent(np_=np_, nbins=nbins, sort_every=sort_every)
-    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, diag=diag)
+    pingpong = diag == "pingpong"
+    diag = "nsub" if pingpong else diag
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, diag=diag, pingpong=pingpong)
     hx, hy, hz = (torch.from_numpy(a.copy()).pin_memory() for a in (x, y, z))
     hid = torch.from_numpy(pid.view(np.int64).copy()).pin_memory()
     hchi = torch.from_numpy(chi.copy()).pin_memory()
@@ -358,10 +377,11 @@ def test_lp_step_host_roundtrip(np_, nbins, sort_every, diag):
 
 # ------------------------------------------------------------------ edge cases and error paths
 
-def test_empty_and_tiny_particle_sets():
+@pytest.mark.parametrize("pingpong", [False, True])
+def test_empty_and_tiny_particle_sets(pingpong):
     for n_p in (0, 1, 2, 33):
         w = small_turbulent(np_=n_p, nbins=16 if n_p % 2 else 64, sort_every=1)
-        lp, prm, f_np, x, y, z, pid, chi = setup_pair(w)
+        lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, pingpong=pingpong)
         lp.step(w.dt)
         lp.step(w.dt)
         torch.cuda.synchronize()
@@ -443,12 +463,13 @@ def test_nsub_when_cfl_ratio_is_next_to_an_integer(nbins, diag):
 
 # ------------------------------------------------------------------ a2 after injection: ids wider than any bound id
 
-def test_sort_after_compaction_and_injection_of_wider_ids():
+@pytest.mark.parametrize("pingpong", [False, True])
+def test_sort_after_compaction_and_injection_of_wider_ids(pingpong):
     """The number of radix passes over the ids must follow the ids that are there when the sort runs, not
     those bound at the start: delete some particles, inject new ones with ids far above every earlier id
     (more significant bits), raise the count, sort -- the order must be the oracle's (key, id) order."""
     w = small_turbulent(n=6, np_=6000, nbins=16)
-    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, pingpong=pingpong)
     lp.sort()                                                     # a sort with the narrow ids first
     x, y, z, pid, chi, _, _ = oracle_sort_state(prm, x, y, z, pid, chi)
     rng = np.random.default_rng(7)
@@ -473,7 +494,7 @@ def test_sort_after_compaction_and_injection_of_wider_ids():
 
 # ------------------------------------------------------------------ seeded random configurations
 
-@pytest.mark.parametrize("seed", range(16))
+@pytest.mark.parametrize("seed", range(24))
 def test_random_small_configurations(seed):
     """Ragged sizes against the ring / chunk / batch boundaries of the kernels: random particle counts, bin
     counts, boundary kinds and re-sort periods; three fused steps, everything compared as in the other tests."""
@@ -484,7 +505,8 @@ def test_random_small_configurations(seed):
     sort_every = int(rng.choice([0, 1, 2]))
     w = small_turbulent(n=int(rng.choice([4, 7, 12])), np_=np_, nbins=nbins, sort_every=sort_every).scaled(
         periodic=periodic, dt=float(rng.choice([0.01, 0.05])))
-    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, diag=DIAG_KINDS[seed % 2])
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, diag=DIAG_KINDS[seed % 2],
+                                                  pingpong=bool((seed // 2) % 2))
     for s in range(3):
         lp.step(w.dt)
         if sort_every and s % sort_every == 0:

@@ -105,7 +105,7 @@ def cached_fields(w, dev):
     return _FIELD_CACHE[k]
 
 
-def run_sampled(w, steps, nsample=2048, check_sort=True, diag="full"):
+def run_sampled(w, steps, nsample=2048, check_sort=True, diag="full", pingpong=False):
     """Run `steps` lp_step on the GPU at full size and the oracle on a sample; compare by id.
     diag = "nsub": only n_sub is bound, so the DIAG=false kernel instantiations run -- the ones bench.py
     times (it binds no `lost` output); the number-conservation property needs `lost` and is then skipped."""
@@ -121,6 +121,7 @@ def run_sampled(w, steps, nsample=2048, check_sort=True, diag="full"):
     lp.set_fields(fields)
     lp.bind_particles(x, y, z, pid, chi_dev)
     lp.bind_diag(nsub=True, lost=(diag == "full"))
+    lp.set_pingpong(pingpong)
     n0 = lp.diag()["number"]
     # oracle sample (ids chosen by a seeded draw)
     srng = np.random.default_rng(12345)
@@ -167,7 +168,7 @@ def test_workload3_full_length_bench_kernels():
     """All 50 steps of BASELINE.json configs[2] in the kernels bench.py times (no `lost` output bound)."""
     w = I.workload(3)
     assert w.steps == 50
-    lp, d, nsub = run_sampled(w, steps=w.steps, diag="nsub")
+    lp, d, nsub = run_sampled(w, steps=w.steps, diag="nsub", pingpong=True)
     assert d["steps"] == 50
 
 
@@ -196,7 +197,7 @@ def test_workload4_full_length_bench_kernels():
     """All 20 steps of BASELINE.json configs[3] (two re-sorts) in the kernels bench.py times."""
     w = I.workload(4)
     assert w.steps == 20
-    lp, d, nsub = run_sampled(w, steps=w.steps, nsample=4096, diag="nsub")
+    lp, d, nsub = run_sampled(w, steps=w.steps, nsample=4096, diag="nsub", pingpong=True)     # as bench.py runs it
     assert d["sorts"] == 2 and d["steps"] == 20
     check_sorted_after_explicit_sort(lp)
 
@@ -214,5 +215,5 @@ def test_workload5_full_length_bench_kernels(nbins):
     """All 10 steps of BASELINE.json configs[4] at every bin count, in the kernels bench.py times."""
     w = I.workload(5).scaled(nbins=nbins)
     assert w.steps == 10
-    lp, d, nsub = run_sampled(w, steps=w.steps, nsample=1024, diag="nsub")
+    lp, d, nsub = run_sampled(w, steps=w.steps, nsample=1024, diag="nsub", pingpong=True)
     assert d["steps"] == 10 and d["sorts"] == 1
