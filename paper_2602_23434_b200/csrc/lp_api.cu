@@ -17,9 +17,10 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t recA, recB, k1, xs, rho_old, nsub, lost, status, key, idx_a, idx_b, hist, alt_id, pos_alt, chi_alt,
-        partial, diag, maxid, total;
+    size_t rec, k1, xs, rho_old, nsub, lost, status, key, idx_a, idx_b, hist, alt_id, pos_alt, chi_alt,
+        partial, diag, maxid, cellcnt, tile_sum, total;
     size_t hist_elems;
+    bool counting;          // sort by one counter per cell (else radix passes only)
 };
 
 Layout make_layout(const lp_config &c)
@@ -29,8 +30,7 @@ Layout make_layout(const lp_config &c)
     const size_t np = (size_t)c.np;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
-    L.recA = take(ncell * 32);
-    L.recB = take(ncell * 32);
+    L.rec = take(ncell * 64);
     L.k1 = take(np * 24);
     L.xs = take(np * 24);
     L.rho_old = take(np * 8);
@@ -47,7 +47,12 @@ Layout make_layout(const lp_config &c)
     L.chi_alt = take(np * (size_t)c.nbins * 8);
     L.partial = take(2 * 296 * 8);
     L.diag = take(sizeof(LpDiagDev));
-    L.maxid = take(8);
+    L.maxid = take(16);                  // largest id | overflow flag of the counting sort
+    // Counting sort by cell: 4 bytes per cell.  Worth it unless the grid dwarfs the particle set (then the
+    // O(cells) scan costs more than the radix passes over the particles it replaces).
+    L.counting = ncell <= 64 * (np > 0 ? np : 1);
+    L.cellcnt = take(L.counting ? (ncell + 1) * 4 : 0);
+    L.tile_sum = take(L.counting ? lp_sort_scan_tiles((long long)ncell) * 4 : 0);
     L.total = off;
     return L;
 }
@@ -168,9 +173,15 @@ struct lp_ctx {
     // (lp_set_pingpong) a re-sort reads one set through the permutation and writes the other, and `cur` flips.
     bool pingpong = false;
     int cur = 0;
+    bool split_records = false;            // cell records as two 32-byte arrays (dense sets) or one 64-byte array (LpCells)
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
-    LpCells cells() const { return LpCells{ at<const double4>(lay.recA), at<const double4>(lay.recB) }; }
+    LpCells cells() const
+    {
+        const double4 *r = at<const double4>(lay.rec);
+        if (split_records) return LpCells{ r, r + (size_t)cfg.nx * cfg.ny * cfg.nz, 1u };
+        return LpCells{ r, r + 1, 2u };
+    }
     struct Set { double *x, *y, *z; uint64_t *id; double *chi; };
     Set set(int which) const
     {
@@ -351,6 +362,17 @@ lp_status sort_permutation(lp_ctx *c, uint32_t **perm, cudaStream_t s)
         c->id_bits = bit_length(h);
         c->id_bits_stale = false;
     }
+    if (c->lay.counting) {
+        // one counter per cell, rank counting inside the cells; the radix passes are enqueued behind it as a
+        // fallback that runs only if a cell holds more than 64 particles (a flag on the device gates them)
+        LpCountBufs cb;
+        cb.cnt = c->at<uint32_t>(c->lay.cellcnt);
+        cb.tile_sum = c->at<uint32_t>(c->lay.tile_sum);
+        cb.seg_id = c->other().id;                 // scratch until the permuted ids are written there
+        cb.overflow = c->at<uint32_t>(c->lay.maxid) + 2;
+        return count(c, lp_launch_sort_perm_counting(c->geom, n.x, n.y, n.z, n.id, np, c->id_bits, c->key_bits, b, cb, perm, s),
+                     "sort kernels launch");
+    }
     return count(c, lp_launch_sort_perm(c->geom, n.x, n.y, n.z, n.id, np, c->id_bits, c->key_bits, b, perm, s),
                  "sort kernels launch");
 }
@@ -420,6 +442,11 @@ lp_status lp_create(const lp_config *cfg, lp_ctx **out)
     c->cfg = *cfg;
     c->capacity = cfg->np;
     c->lay = make_layout(*cfg);
+#ifdef LP_FORCE_SPLIT_RECORDS               // (sweeps only)
+    c->split_records = LP_FORCE_SPLIT_RECORDS != 0;
+#else
+    c->split_records = cfg->np >= (long long)cfg->nx * cfg->ny * cfg->nz;      // a particle or more per cell
+#endif
     LpGeom &g = c->geom;
     g.nx = cfg->nx; g.ny = cfg->ny; g.nz = cfg->nz;
     const int n[3] = { cfg->nx, cfg->ny, cfg->nz };
@@ -523,7 +550,8 @@ lp_status lp_set_fields(lp_ctx *ctx, const double *vx, const double *vy, const d
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     const double *f[7] = { vx, vy, vz, bx, by, bz, rho };
     const long long ncell = (long long)ctx->cfg.nx * ctx->cfg.ny * ctx->cfg.nz;
-    lp_status st = count(ctx, lp_launch_repack(f, ctx->at<double4>(ctx->lay.recA), ctx->at<double4>(ctx->lay.recB), ncell,
+    const LpCells cl = ctx->cells();
+    lp_status st = count(ctx, lp_launch_repack(f, const_cast<double4 *>(cl.recA), const_cast<double4 *>(cl.recB), cl.stride, ncell,
                                                static_cast<cudaStream_t>(stream)), "lp_repack_kernel launch");
     if (st == LP_OK) ctx->have_fields = true;
     return st;

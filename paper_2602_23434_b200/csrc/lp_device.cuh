@@ -108,7 +108,7 @@ struct LpCornersA {
     __device__ __forceinline__ void load(const LpCells &cells, const LpStencil &st)
     {
 #pragma unroll
-        for (int n = 0; n < 8; ++n) r[n] = lp_ldg_rec(cells.recA + st.c[n]);
+        for (int n = 0; n < 8; ++n) r[n] = lp_ldg_rec(cells.recA + (size_t)cells.stride * st.c[n]);
         c0 = st.c[0];
         c7 = st.c[7];
     }
@@ -163,7 +163,7 @@ struct LpCornersB {
     __device__ __forceinline__ void load(const LpCells &cells, const LpStencil &st)
     {
 #pragma unroll
-        for (int n = 0; n < 8; ++n) r[n] = lp_ldg_rec(cells.recB + st.c[n]);
+        for (int n = 0; n < 8; ++n) r[n] = lp_ldg_rec(cells.recB + (size_t)cells.stride * st.c[n]);
     }
     __device__ __forceinline__ void gather3(const LpStencil &st, double out[3]) const
     {

@@ -15,11 +15,20 @@ struct LpGeom {
     double len[3];           // xhi - xlo
 };
 
-// Interleaved per-cell records built by lp_set_fields:
-//   recA[c] = (vx, vy, vz, rho)   32 B     recB[c] = (bx, by, bz, 0)   32 B
+// Per-cell records built by lp_set_fields, two 32-byte halves per cell,
+//   A = (vx, vy, vz, rho)    B = (bx, by, bz, 0),
+// half A of cell c at recA[stride * c], half B at recB[stride * c], in one of two layouts chosen at lp_create:
+//  * stride 2, recB = recA + 1: one 64-byte record per cell.  A 64-byte record is one DRAM access whatever
+//    its alignment, so a particle with no neighbour in its cells fetches 8 x 64 bytes, all but 8 of them used,
+//    where separate 32-byte arrays fetch 1.5 x that (DRAM moves 64 bytes at a time).  The layout for sparse
+//    particle sets (fewer particles than cells): workload 5 gains 10-22 %, workload 3 2 %.
+//  * stride 1, recB = recA + cells: two arrays.  With a particle or more in every cell the A halves are read
+//    three times per step by neighbouring particles and four of them share an L1 line; workload 4 is 3 %
+//    faster this way (measured, profiles/r02_gather_layout.md).
 struct LpCells {
     const double4 *recA;
     const double4 *recB;
+    unsigned stride;
 };
 
 // Bins at which the outflow rate (max(w_{i+1},0) - min(w_i,0))/dE_i can be the maximum over the
@@ -75,7 +84,7 @@ struct LpPushArgs {
 };
 
 // ---- launchers (each returns the number of kernels it enqueued, or -1 with cudaGetLastError set)
-int lp_launch_repack(const double *const f[7], double4 *recA, double4 *recB, long long ncell,
+int lp_launch_repack(const double *const f[7], double4 *recA, double4 *recB, unsigned stride, long long ncell,
                      cudaStream_t s);
 int lp_launch_interpolate(const LpGeom &g, const LpCells &c, const double *x, const double *y,
                           const double *z, long long np, double *out7, uint32_t *key, cudaStream_t s);
@@ -110,6 +119,19 @@ size_t lp_sort_hist_elems(long long np);
 int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const double *z,
                         const uint64_t *id, long long np, int id_bits, int key_bits,
                         const LpSortBufs &b, uint32_t **perm_out, cudaStream_t s);
+// Counting sort by cell (lp_sort.cu): one counter per cell plus rank counting inside the cells; falls back to
+// the radix passes on the device when a cell holds more than 64 particles.  id_bits: as for the radix sort
+// (64 when not measured).
+struct LpCountBufs {
+    uint32_t *cnt;       // [ncell + 1]  counters, then exclusive offsets
+    uint32_t *tile_sum;  // [lp_sort_scan_tiles(ncell)]
+    uint64_t *seg_id;    // [np]  ids grouped by cell (scratch: the id array of the other buffer set)
+    uint32_t *overflow;  // [1]
+};
+size_t lp_sort_scan_tiles(long long ncell);
+int lp_launch_sort_perm_counting(const LpGeom &g, const double *x, const double *y, const double *z,
+                                 const uint64_t *id, long long np, int id_bits, int key_bits, const LpSortBufs &b,
+                                 const LpCountBufs &cb, uint32_t **perm_out, cudaStream_t s);
 int lp_launch_permute_f64(const uint32_t *perm, const double *src, double *dst, long long np, cudaStream_t s);
 int lp_launch_permute_u64(const uint32_t *perm, const uint64_t *src, uint64_t *dst, long long np, cudaStream_t s);
 int lp_launch_permute_rows(const uint32_t *perm, const double *src, double *dst, long long np,

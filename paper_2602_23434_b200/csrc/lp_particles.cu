@@ -12,17 +12,17 @@ inline int blocks_for(long long n, int threads)
     return (int)(b < 1 ? 1 : b);
 }
 
-// a3: seven SoA grid arrays -> two interleaved 32-byte records per cell.
+// a3: seven SoA grid arrays -> one 64-byte record per cell, written as its two 32-byte halves.
 __global__ void __launch_bounds__(kThreads)
 lp_repack_kernel(const double *__restrict__ vx, const double *__restrict__ vy, const double *__restrict__ vz,
                  const double *__restrict__ bx, const double *__restrict__ by, const double *__restrict__ bz,
                  const double *__restrict__ rho, double4 *__restrict__ recA, double4 *__restrict__ recB,
-                 long long ncell)
+                 unsigned stride, long long ncell)
 {
     long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= ncell) return;
-    double2 *a = reinterpret_cast<double2 *>(recA + c);
-    double2 *b = reinterpret_cast<double2 *>(recB + c);
+    double2 *a = reinterpret_cast<double2 *>(recA + (size_t)stride * c);
+    double2 *b = reinterpret_cast<double2 *>(recB + (size_t)stride * c);
     a[0] = make_double2(vx[c], vy[c]);
     a[1] = make_double2(vz[c], rho[c]);
     b[0] = make_double2(bx[c], by[c]);
@@ -146,10 +146,11 @@ int lp_launch_push_rk3(const LpPushArgs &a, int stage, cudaStream_t s)
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
-int lp_launch_repack(const double *const f[7], double4 *recA, double4 *recB, long long ncell, cudaStream_t s)
+int lp_launch_repack(const double *const f[7], double4 *recA, double4 *recB, unsigned stride, long long ncell,
+                     cudaStream_t s)
 {
     lp_repack_kernel<<<blocks_for(ncell, kThreads), kThreads, 0, s>>>(f[0], f[1], f[2], f[3], f[4], f[5], f[6],
-                                                                      recA, recB, ncell);
+                                                                      recA, recB, stride, ncell);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -34,8 +34,10 @@ __device__ __forceinline__ uint32_t lp_digit(const uint32_t *idx_in, const uint6
 __global__ void __launch_bounds__(kThreads)
 lp_radix_hist_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__restrict__ id,
                      const uint32_t *__restrict__ key, long long np, int use_key, int shift,
-                     uint32_t *__restrict__ hist, int nblocks, uint8_t *__restrict__ digit)
+                     uint32_t *__restrict__ hist, int nblocks, uint8_t *__restrict__ digit,
+                     const uint32_t *__restrict__ enable)
 {
+    if (enable && *enable == 0) return;          // fallback of the counting sort, not needed this time
     __shared__ uint32_t sh[256];
     sh[threadIdx.x] = 0;
     __syncthreads();
@@ -56,8 +58,10 @@ lp_radix_hist_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__rest
 // Per-digit exclusive scan over blocks: block d scans hist[d][0..nblocks) in place and writes the
 // digit total to totals[d].  The scatter kernel adds the exclusive prefix of the totals itself.
 __global__ void __launch_bounds__(kThreads)
-lp_scan_rows_kernel(uint32_t *__restrict__ hist, int nblocks, uint32_t *__restrict__ totals)
+lp_scan_rows_kernel(uint32_t *__restrict__ hist, int nblocks, uint32_t *__restrict__ totals,
+                    const uint32_t *__restrict__ enable)
 {
+    if (enable && *enable == 0) return;
     __shared__ uint32_t wsum[kWarps];
     __shared__ uint32_t carry_s;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -90,8 +94,10 @@ __global__ void __launch_bounds__(kThreads)
 lp_radix_scatter_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__restrict__ id,
                         const uint32_t *__restrict__ key, long long np, int use_key, int shift,
                         const uint32_t *__restrict__ hist, const uint32_t *__restrict__ totals, int nblocks,
-                        uint32_t *__restrict__ idx_out, const uint8_t *__restrict__ digit)
+                        uint32_t *__restrict__ idx_out, const uint8_t *__restrict__ digit,
+                        const uint32_t *__restrict__ enable)
 {
+    if (enable && *enable == 0) return;
     __shared__ uint32_t base[256];
     __shared__ uint32_t wcount[kWarps][256];
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -136,6 +142,159 @@ lp_radix_scatter_kernel(const uint32_t *__restrict__ idx_in, const uint64_t *__r
         if (valid) idx_out[wcount[warp][d] + rank] = src;
         __syncthreads();
     }
+}
+
+// ---- counting sort by cell (the usual path): the key space is the grid, so one counter per cell orders the
+// particles by key in O(N_p + cells) -- no radix passes -- and the few particles that share a cell are put in
+// id order by rank counting inside their cell's segment.  The result is the same total (key, id) order.
+//   K1 count:  key[p]; rank0[p] = atomicAdd(&cnt[key[p]], 1)        (arrival order inside the cell, arbitrary)
+//   scan:      cnt -> exclusive offsets (cnt[ncell] = N_p)
+//   K3 place:  seg_id[offset[key[p]] + rank0[p]] = id[p]            (the ids of a cell, contiguous)
+//   K4 rank:   r = #{ids of my cell's segment smaller than mine};  perm[offset + r] = p
+// A cell with more than kMaxSeg particles would make K4 quadratic: it raises *overflow instead and the radix
+// passes (launched behind, every kernel gated on that flag) redo the whole sort.
+constexpr int kMaxSeg = 64;
+
+__global__ void __launch_bounds__(kThreads)
+lp_cell_count_kernel(LpGeom g, const double *__restrict__ x, const double *__restrict__ y,
+                     const double *__restrict__ z, long long np, uint32_t *__restrict__ key,
+                     uint32_t *__restrict__ cnt, uint32_t *__restrict__ rank0)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    const uint32_t k = lp_cell_key(g, x[p], y[p], z[p]);
+    key[p] = k;
+    rank0[p] = atomicAdd(cnt + k, 1u);
+}
+
+// exclusive scan of v[0..n) in place, v[n] = total: tile sums, scan of the tile sums (one block), tiles again
+constexpr int kScanItems = 16;
+constexpr int kScanTile = kThreads * kScanItems;
+
+__device__ __forceinline__ uint32_t lp_block_excl_scan(uint32_t v, uint32_t *total)
+{
+    __shared__ uint32_t wsum[kWarps];
+    __shared__ uint32_t tot;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t u = __shfl_up_sync(kFull, inc, o);
+        if (lane >= o) inc += u;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    uint32_t wbase = 0;
+    for (int w = 0; w < warp; ++w) wbase += wsum[w];
+    if (threadIdx.x == kThreads - 1) tot = wbase + inc;
+    __syncthreads();
+    *total = tot;
+    const uint32_t r = wbase + inc - v;
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_scan_tile_sums_kernel(const uint32_t *__restrict__ v, long long n, uint32_t *__restrict__ tile_sum)
+{
+    const long long i0 = (long long)blockIdx.x * kScanTile + (long long)threadIdx.x * kScanItems;
+    uint32_t c = 0;
+    if (i0 + kScanItems <= n) {
+        const uint4 *q = reinterpret_cast<const uint4 *>(v + i0);
+#pragma unroll
+        for (int k = 0; k < kScanItems / 4; ++k) { const uint4 t = q[k]; c += t.x + t.y + t.z + t.w; }
+    } else {
+        for (int k = 0; k < kScanItems; ++k) if (i0 + k < n) c += v[i0 + k];
+    }
+    uint32_t total;
+    lp_block_excl_scan(c, &total);
+    if (threadIdx.x == 0) tile_sum[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_scan_tile_offsets_kernel(uint32_t *__restrict__ tile_sum, int ntiles)
+{
+    uint32_t carry = 0;
+    for (int b0 = 0; b0 < ntiles; b0 += kThreads) {
+        const int i = b0 + threadIdx.x;
+        const uint32_t v = i < ntiles ? tile_sum[i] : 0u;
+        uint32_t total;
+        const uint32_t ex = lp_block_excl_scan(v, &total);
+        if (i < ntiles) tile_sum[i] = carry + ex;
+        carry += total;
+    }
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_scan_tiles_kernel(uint32_t *__restrict__ v, long long n, const uint32_t *__restrict__ tile_off)
+{
+    const long long i0 = (long long)blockIdx.x * kScanTile + (long long)threadIdx.x * kScanItems;
+    uint32_t f[kScanItems], c = 0;
+    const bool full = i0 + kScanItems <= n;
+    if (full) {
+        const uint4 *q = reinterpret_cast<const uint4 *>(v + i0);
+#pragma unroll
+        for (int k = 0; k < kScanItems / 4; ++k) {
+            const uint4 t = q[k];
+            f[4 * k] = t.x; f[4 * k + 1] = t.y; f[4 * k + 2] = t.z; f[4 * k + 3] = t.w;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) f[k] = i0 + k < n ? v[i0 + k] : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) c += f[k];
+    uint32_t total;
+    uint32_t run = tile_off[blockIdx.x] + lp_block_excl_scan(c, &total);
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) { const uint32_t t = f[k]; f[k] = run; run += t; }
+    if (full) {
+        uint4 *q = reinterpret_cast<uint4 *>(v + i0);
+#pragma unroll
+        for (int k = 0; k < kScanItems / 4; ++k) q[k] = make_uint4(f[4 * k], f[4 * k + 1], f[4 * k + 2], f[4 * k + 3]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) if (i0 + k < n) v[i0 + k] = f[k];
+    }
+    // the total behind the last element: the tile that holds index n - 1 writes v[n]
+    if (i0 <= n - 1 && n - 1 < i0 + kScanItems) v[n] = run;
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_cell_place_kernel(const uint32_t *__restrict__ key, const uint32_t *__restrict__ rank0,
+                     const uint32_t *__restrict__ off, const uint64_t *__restrict__ id, long long np,
+                     uint64_t *__restrict__ seg_id)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    seg_id[off[key[p]] + rank0[p]] = id[p];
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_cell_rank_kernel(const uint32_t *__restrict__ key, const uint32_t *__restrict__ off,
+                    const uint64_t *__restrict__ id, const uint64_t *__restrict__ seg_id, long long np,
+                    uint32_t *__restrict__ perm, uint32_t *__restrict__ overflow)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    const uint32_t k = key[p];
+    const uint32_t o = off[k], n = off[k + 1] - o;
+    uint32_t r = 0;
+    if (n > 1) {
+        if (n > (uint32_t)kMaxSeg) { *overflow = 1u; return; }
+        const uint64_t mine = id[p];
+        for (uint32_t j = 0; j < n; ++j) r += seg_id[o + j] < mine ? 1u : 0u;
+    }
+    perm[o + r] = (uint32_t)p;
+}
+
+__global__ void __launch_bounds__(kThreads)
+lp_copy_if_kernel(const uint32_t *__restrict__ src, uint32_t *__restrict__ dst, long long n,
+                  const uint32_t *__restrict__ enable)
+{
+    if (*enable == 0) return;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        dst[i] = src[i];
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -263,13 +422,11 @@ inline bool ok() { return cudaPeekAtLastError() == cudaSuccess; }
 
 size_t lp_sort_hist_elems(long long np) { return (size_t)256 * (size_t)blocks_for(np, kTile) + 256; }
 
-int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const double *z, const uint64_t *id,
-                        long long np, int id_bits, int key_bits, const LpSortBufs &b, uint32_t **perm_out,
-                        cudaStream_t s)
+// radix passes into b.idx_a / b.idx_b; enable (device flag, or NULL = always): see the counting sort
+static int radix_passes(const uint64_t *id, long long np, int id_bits, int key_bits, const LpSortBufs &b,
+                        const uint32_t *enable, uint32_t **perm_out, cudaStream_t s)
 {
     int launches = 0;
-    lp_key_kernel<<<blocks_for(np, kThreads), kThreads, 0, s>>>(g, x, y, z, np, b.key);
-    ++launches;
     const int nblocks = blocks_for(np, kTile);
     const uint32_t *in = nullptr;       // identity
     uint32_t *bufs[2] = { b.idx_a, b.idx_b };
@@ -279,16 +436,54 @@ int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const
     for (int pass = 0; pass < (total > 0 ? total : 1); ++pass) {
         const int use_key = pass >= id_passes ? 1 : 0;
         const int shift = 8 * (use_key ? pass - id_passes : pass);
-        lp_radix_hist_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, nblocks, b.digit);
+        lp_radix_hist_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, nblocks, b.digit, enable);
         uint32_t *totals = b.hist + (size_t)256 * nblocks;
-        lp_scan_rows_kernel<<<256, kThreads, 0, s>>>(b.hist, nblocks, totals);
+        lp_scan_rows_kernel<<<256, kThreads, 0, s>>>(b.hist, nblocks, totals, enable);
         lp_radix_scatter_kernel<<<nblocks, kThreads, 0, s>>>(in, id, b.key, np, use_key, shift, b.hist, totals, nblocks, bufs[cur],
-                                                             b.digit);
+                                                             b.digit, enable);
         launches += 3;
         in = bufs[cur];
         cur ^= 1;
     }
     *perm_out = const_cast<uint32_t *>(in);
+    return launches;
+}
+
+int lp_launch_sort_perm(const LpGeom &g, const double *x, const double *y, const double *z, const uint64_t *id,
+                        long long np, int id_bits, int key_bits, const LpSortBufs &b, uint32_t **perm_out,
+                        cudaStream_t s)
+{
+    lp_key_kernel<<<blocks_for(np, kThreads), kThreads, 0, s>>>(g, x, y, z, np, b.key);
+    const int launches = 1 + radix_passes(id, np, id_bits, key_bits, b, nullptr, perm_out, s);
+    return ok() ? launches : -1;
+}
+
+size_t lp_sort_scan_tiles(long long ncell) { return (size_t)blocks_for(ncell, kScanTile); }
+
+int lp_launch_sort_perm_counting(const LpGeom &g, const double *x, const double *y, const double *z,
+                                 const uint64_t *id, long long np, int id_bits, int key_bits, const LpSortBufs &b,
+                                 const LpCountBufs &cb, uint32_t **perm_out, cudaStream_t s)
+{
+    const long long ncell = (long long)g.nx * g.ny * g.nz;
+    const int pblocks = blocks_for(np, kThreads), ntiles = blocks_for(ncell, kScanTile);
+    if (cudaMemsetAsync(cb.cnt, 0, (size_t)(ncell + 1) * 4, s) != cudaSuccess) return -1;
+    if (cudaMemsetAsync(cb.overflow, 0, 4, s) != cudaSuccess) return -1;
+    uint32_t *rank0 = b.idx_a, *perm = b.idx_b;
+    lp_cell_count_kernel<<<pblocks, kThreads, 0, s>>>(g, x, y, z, np, b.key, cb.cnt, rank0);
+    lp_scan_tile_sums_kernel<<<ntiles, kThreads, 0, s>>>(cb.cnt, ncell, cb.tile_sum);
+    lp_scan_tile_offsets_kernel<<<1, kThreads, 0, s>>>(cb.tile_sum, ntiles);
+    lp_scan_tiles_kernel<<<ntiles, kThreads, 0, s>>>(cb.cnt, ncell, cb.tile_sum);
+    lp_cell_place_kernel<<<pblocks, kThreads, 0, s>>>(b.key, rank0, cb.cnt, id, np, cb.seg_id);
+    lp_cell_rank_kernel<<<pblocks, kThreads, 0, s>>>(b.key, cb.cnt, id, cb.seg_id, np, perm, cb.overflow);
+    int launches = 6;
+    // fallback, gated on *overflow: the radix sort of the same keys, its result copied over perm
+    uint32_t *rperm = nullptr;
+    launches += radix_passes(id, np, id_bits, key_bits, b, cb.overflow, &rperm, s);
+    if (rperm != perm) {
+        lp_copy_if_kernel<<<blocks_for(np, kThreads * 8), kThreads, 0, s>>>(rperm, perm, np, cb.overflow);
+        ++launches;
+    }
+    *perm_out = perm;
     return ok() ? launches : -1;
 }
 

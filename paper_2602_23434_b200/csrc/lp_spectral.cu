@@ -54,11 +54,13 @@ __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, 
     if (FUSED) {
         lp_stencil(A.g, px, py, pz, st);
         ka.load(A.cells, st);
-        // B is gathered last, at x^{n+1}, whose cells are these or their neighbours: start them on their way
-        // from DRAM to L2 now (the four x-lower corners; every prefetch is an L1 request, and eight cost more
-        // than they save)
+        // B is gathered last, at x^{n+1}, whose cells are these or their neighbours.  With split record arrays
+        // start the B halves of the four x-lower corners on their way from DRAM to L2 now (every prefetch is an
+        // L1 request, and eight cost more than they save); in a 64-byte record the B half arrives in L2 with A.
+        if (A.cells.stride == 1) {
 #pragma unroll
-        for (int n = 0; n < 8; n += 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.cells.recB + st.c[n]));
+            for (int n = 0; n < 8; n += 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.cells.recB + st.c[n]));
+        }
         ka.gather4(st, qa);                                 // k1 = v(x^n), rho_old = rho(x^n)
         rho_old = qa[3];
         lp_stencil(A.g, __dadd_rn(px, __dmul_rn(A.dt, qa[0])), __dadd_rn(py, __dmul_rn(A.dt, qa[1])),
@@ -704,6 +706,9 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #ifndef LP_BULK_RI
 #define LP_BULK_RI 1            // rows a lane group advances together (ILP)
 #endif
+#ifndef LP_BULK_GROUP
+#define LP_BULK_GROUP 1         // consecutive chunks dealt to a block at a time (power of two)
+#endif
 
 template <int NB>
 struct LpBulkCfg {
@@ -770,14 +775,25 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
     const uint32_t empty_u32 = full_u32 + 8 * D;
     const uint32_t np = (uint32_t)A.np;
     const uint32_t nchunks = (uint32_t)((A.np + 31) >> 5);
-    const uint32_t nblk = blockIdx.x < nchunks ? (nchunks - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    // Chunks are dealt to the blocks in groups of GS consecutive ones (group g goes to block g % gridDim):
+    // neighbouring chunks hold particles of neighbouring cells (the set is sorted by cell), so a block that
+    // works through a run of them finds the cell records of the row above or below already in its L1.
+    constexpr uint32_t GS = LP_BULK_GROUP;
+    const uint32_t ngroups_all = (nchunks + GS - 1) / GS;
+    const uint32_t ngb = blockIdx.x < ngroups_all ? (ngroups_all - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    // this block's chunks, t = 0 .. nblk-1 (the last group of all may be short)
+    const uint32_t nblk = ngb == 0 ? 0
+                          : ngb * GS - (((ngb - 1) * gridDim.x + blockIdx.x == ngroups_all - 1) ? ngroups_all * GS - nchunks : 0);
+    auto chunk_start = [&](uint32_t t) -> uint32_t {      // first particle of this block's chunk t
+        return ((((t / GS) * gridDim.x + blockIdx.x) * GS) + (t % GS)) << 5;
+    };
 
     if (warp < NP) {
         // ---------------------------------------------------------------- particle warp
         // positions are fetched one chunk ahead, so that their latency is off the dependent chain; when the
         // step re-sorts (A.perm) they are read through the permutation, whose entries are fetched a chunk
         // earlier still, and the ids move with them
-        auto chunk_of = [&](uint32_t t) -> uint32_t { return (blockIdx.x + t * gridDim.x) << 5; };
+        auto chunk_of = [&](uint32_t t) -> uint32_t { return chunk_start(t); };
         const uint32_t *perm = A.perm;
         auto own_index = [&](uint32_t t, bool &valid) -> uint32_t {      // index of this lane's particle of chunk t
             valid = t < nblk && chunk_of(t) + lane < np;
@@ -831,7 +847,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
 
     constexpr bool kHint = (LP_BULK_L2HINT != 0) && NB <= 128;
     const uint64_t pol = lp_policy_evict_first();
-    auto chunk_base = [&](uint32_t k) -> uint32_t { return (blockIdx.x + (rw + k * NR) * gridDim.x) << 5; };
+    auto chunk_base = [&](uint32_t k) -> uint32_t { return chunk_start(rw + k * NR); };
     auto group_row0 = [&](uint32_t j) -> uint32_t { return chunk_base(j / GPC) + (j % GPC) * R; };
     auto issue_load = [&](uint32_t j, int slot) {        // lane 0 only: the group's rows are contiguous
         const uint32_t row0 = group_row0(j);
