@@ -27,6 +27,7 @@
  *   orc_shock_row/update spectrum reset at a shock crossing  PAPER.md:110-122 (Eq. 7-8)          S1-S4
  *   orc_compact          deletion with hole filling          PAPER.md:190-199                    C1
  *   orc_push_rk3_stage   three-stage third-order pusher      PAPER.md:245, 258-260               K1
+ *   orc_migrate_pack/unpack  exchange across rank interfaces PAPER.md:201-214                    M1-M3
  *   orc_step             one whole step with frozen fields   PAPER.md:216-233 (Table 1)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force cell search and O(N^2)
@@ -415,6 +416,104 @@ int64_t orc_compact(int64_t np, const int32_t *flag, int32_t nbins,
     }
     free(holes); free(fill);
     return keep;                                                                  /* step 5 */
+}
+
+/* ---------------------------------------------------------------- particle migration (NEXT-3) */
+
+/* Exchange of the particles that crossed an inter-rank interface, one direction at a
+ * time ("three steps for the three parallel directions"), a left and a right neighbour per direction.
+ * The paper's eight steps, as seen by ONE rank that owns [lo, hi) along `axis`:
+ *   1. collect holes (the leavers) and count how many particles go to each neighbour
+ *   2.-3. (receive posted, buffers sized: the caller's business)
+ *   4. pack the leavers into the two send buffers
+ *   5.-7. (send, resize the container, wait)
+ *   8. copy the arrivals into the holes left by the leavers and compact.
+ * Readings (M1-M3; the paper gives the steps, not these details):
+ *  M1 where a particle goes.  Positions were wrapped into the global box [glo, ghi) by the pusher
+ *     (Particles_Boundary precedes Particles_Exchange), so a particle that left through
+ *     the low face of the first rank of a periodic axis sits near ghi.  A particle outside [lo, hi) goes to
+ *     the neighbour through whose face the shorter way leads, the other way being the one around the
+ *     periodic box:  x < lo:  left over lo - x,  right over (x + L) - hi;   x >= hi:  right over x - hi,
+ *     left over lo - (x - L);  L = ghi - glo.  A tie, or a non-periodic axis, takes the plain side.
+ *  M2 order inside a send buffer: ascending index of the leavers.
+ *  M3 where arrivals go: the arrivals from the left, then those from the right, in buffer order; the k-th
+ *     arrival goes into the k-th hole (ascending index); arrivals beyond the holes are appended behind the
+ *     last particle; holes beyond the arrivals are closed by the compaction of Section 3.2 (orc_compact,
+ *     reading C1) with exactly those holes flagged. */
+int32_t orc_migrate_dest(double x, double lo, double hi, double glo, double ghi, int32_t periodic)
+{
+    if (x >= lo && x < hi) return 0;
+    const double L = ghi - glo;
+    if (x < lo) {
+        if (periodic) {
+            const double left = lo - x, right = (x + L) - hi;
+            if (right >= 0.0 && right < left) return 2;
+        }
+        return 1;
+    }
+    if (periodic) {
+        const double right = x - hi, left = lo - (x - L);
+        if (left >= 0.0 && left < right) return 1;
+    }
+    return 2;      /* x >= hi (or NaN) */
+}
+
+/* Steps 1 and 4.  dest[p] in {0, 1, 2}; holes[] = the leavers' indices ascending (n_left + n_right of
+ * them); the leavers' parameters are copied, in ascending index order, into the left buffer
+ * (lx, ly, lz, lid, lchi[.][nbins]) and the right buffer (r...), each with room for np particles. */
+void orc_migrate_pack(int64_t np, int32_t nbins, int32_t axis, double lo, double hi, double glo, double ghi,
+                      int32_t periodic, const double *x, const double *y, const double *z, const uint64_t *id,
+                      const double *chi, int32_t *dest, int64_t *holes, int64_t *n_left, int64_t *n_right,
+                      double *lx, double *ly, double *lz, uint64_t *lid, double *lchi,
+                      double *rx, double *ry, double *rz, uint64_t *rid, double *rchi)
+{
+    const double *pos = axis == 0 ? x : (axis == 1 ? y : z);
+    int64_t nl = 0, nr = 0, nh = 0;
+    for (int64_t p = 0; p < np; ++p) {                                           /* step 1 */
+        dest[p] = orc_migrate_dest(pos[p], lo, hi, glo, ghi, periodic);
+        if (dest[p]) holes[nh++] = p;
+    }
+    for (int64_t p = 0; p < np; ++p) {                                           /* step 4 */
+        if (dest[p] == 1) {
+            lx[nl] = x[p]; ly[nl] = y[p]; lz[nl] = z[p]; lid[nl] = id[p];
+            for (int32_t b = 0; b < nbins; ++b) lchi[nl * nbins + b] = chi[p * nbins + b];
+            ++nl;
+        } else if (dest[p] == 2) {
+            rx[nr] = x[p]; ry[nr] = y[p]; rz[nr] = z[p]; rid[nr] = id[p];
+            for (int32_t b = 0; b < nbins; ++b) rchi[nr * nbins + b] = chi[p * nbins + b];
+            ++nr;
+        }
+    }
+    *n_left = nl; *n_right = nr;
+}
+
+/* Step 8.  The arrays have room for np + n_from_left + n_from_right particles.  Returns the new count. */
+int64_t orc_migrate_unpack(int64_t np, int32_t nbins, const int64_t *holes, int64_t nholes,
+                           int64_t n_from_left, const double *lx, const double *ly, const double *lz,
+                           const uint64_t *lid, const double *lchi,
+                           int64_t n_from_right, const double *rx, const double *ry, const double *rz,
+                           const uint64_t *rid, const double *rchi,
+                           double *x, double *y, double *z, uint64_t *id, double *chi)
+{
+    const int64_t nin = n_from_left + n_from_right;
+    int64_t count = np;
+    for (int64_t k = 0; k < nin; ++k) {
+        const int from_right = k >= n_from_left;
+        const int64_t s = from_right ? k - n_from_left : k;
+        const int64_t d = k < nholes ? holes[k] : count++;                       /* hole, else appended */
+        x[d] = from_right ? rx[s] : lx[s];
+        y[d] = from_right ? ry[s] : ly[s];
+        z[d] = from_right ? rz[s] : lz[s];
+        id[d] = from_right ? rid[s] : lid[s];
+        for (int32_t b = 0; b < nbins; ++b) chi[d * nbins + b] = from_right ? rchi[s * nbins + b] : lchi[s * nbins + b];
+    }
+    if (nin < nholes) {                                                          /* compact the rest away */
+        int32_t *flag = (int32_t *)calloc((size_t)(np > 0 ? np : 1), sizeof(int32_t));
+        for (int64_t k = nin; k < nholes; ++k) flag[holes[k]] = 1;
+        count = orc_compact(np, flag, nbins, x, y, z, id, chi);
+        free(flag);
+    }
+    return count;
 }
 
 /* ---------------------------------------------------------------- whole update / step */

@@ -212,6 +212,76 @@ def compact(flag, x, y, z, pid, chi):
     return x[:keep], y[:keep], z[:keep], pid[:keep], chi[:keep]
 
 
+def migrate_dest(x, lo, hi, glo, ghi, periodic):
+    f = lib().orc_migrate_dest
+    f.restype = C.c_int32
+    return int(f(C.c_double(x), C.c_double(lo), C.c_double(hi), C.c_double(glo), C.c_double(ghi), C.c_int32(periodic)))
+
+
+def migrate_pack(axis, lo, hi, glo, ghi, periodic, x, y, z, pid, chi):
+    """Steps 1 and 4 of the exchange along `axis` for the rank owning [lo, hi).  Returns
+    (dest [np] int32, holes [n_left+n_right] int64, left buffer, right buffer); a buffer is the tuple
+    (x, y, z, id, chi) of the particles sent that way, in ascending index order."""
+    x, px = _d(x); y, py = _d(y); z, pz = _d(z)
+    pid = np.ascontiguousarray(pid, dtype=np.uint64)
+    chi = np.ascontiguousarray(chi, dtype=np.float64)
+    n = x.shape[0]
+    nb = chi.shape[1]
+    dest = np.zeros(n, dtype=np.int32); holes = np.zeros(max(n, 1), dtype=np.int64)
+    nl = C.c_int64(); nr = C.c_int64()
+    bufs = [[np.zeros(max(n, 1)), np.zeros(max(n, 1)), np.zeros(max(n, 1)), np.zeros(max(n, 1), dtype=np.uint64),
+             np.zeros((max(n, 1), nb))] for _ in range(2)]
+    dp = C.POINTER(C.c_double); up = C.POINTER(C.c_uint64)
+    args = []
+    for b in bufs:
+        args += [b[0].ctypes.data_as(dp), b[1].ctypes.data_as(dp), b[2].ctypes.data_as(dp), b[3].ctypes.data_as(up),
+                 b[4].ctypes.data_as(dp)]
+    f = lib().orc_migrate_pack
+    f.restype = None
+    f(C.c_int64(n), C.c_int32(nb), C.c_int32(axis), C.c_double(lo), C.c_double(hi), C.c_double(glo), C.c_double(ghi),
+      C.c_int32(periodic), px, py, pz, pid.ctypes.data_as(up), chi.ctypes.data_as(dp),
+      dest.ctypes.data_as(C.POINTER(C.c_int32)), holes.ctypes.data_as(C.POINTER(C.c_int64)),
+      C.byref(nl), C.byref(nr), *args)
+    left = tuple(a[:nl.value].copy() for a in bufs[0])
+    right = tuple(a[:nr.value].copy() for a in bufs[1])
+    return dest, holes[:nl.value + nr.value].copy(), left, right
+
+
+def migrate_unpack(holes, from_left, from_right, x, y, z, pid, chi):
+    """Step 8: the arrivals (buffers as returned by migrate_pack of the neighbours; None = nothing) into the
+    holes / behind the last particle, the remaining holes compacted away.  Returns (x, y, z, id, chi) of the
+    new particle set."""
+    nb = np.asarray(chi).shape[1]
+    empty = (np.zeros(0), np.zeros(0), np.zeros(0), np.zeros(0, dtype=np.uint64), np.zeros((0, nb)))
+    L = from_left if from_left is not None else empty
+    R = from_right if from_right is not None else empty
+    n = np.asarray(x).shape[0]
+    nin = L[0].shape[0] + R[0].shape[0]
+    cap = n + nin
+    def grow(a, dtype, cols=None):
+        out = np.zeros((cap,) if cols is None else (cap, cols), dtype=dtype)
+        out[:n] = a
+        return out
+    x = grow(x, np.float64); y = grow(y, np.float64); z = grow(z, np.float64)
+    pid = grow(pid, np.uint64); chi = grow(chi, np.float64, nb)
+    holes = np.ascontiguousarray(holes, dtype=np.int64)
+    dp = C.POINTER(C.c_double); up = C.POINTER(C.c_uint64)
+    def buf(b):
+        b = (np.ascontiguousarray(b[0], dtype=np.float64), np.ascontiguousarray(b[1], dtype=np.float64),
+             np.ascontiguousarray(b[2], dtype=np.float64), np.ascontiguousarray(b[3], dtype=np.uint64),
+             np.ascontiguousarray(b[4], dtype=np.float64))
+        return b, [b[0].ctypes.data_as(dp), b[1].ctypes.data_as(dp), b[2].ctypes.data_as(dp), b[3].ctypes.data_as(up),
+                   b[4].ctypes.data_as(dp)]
+    Lk, La = buf(L); Rk, Ra = buf(R)
+    f = lib().orc_migrate_unpack
+    f.restype = C.c_int64
+    cnt = f(C.c_int64(n), C.c_int32(nb), holes.ctypes.data_as(C.POINTER(C.c_int64)), C.c_int64(holes.shape[0]),
+            C.c_int64(Lk[0].shape[0]), *La, C.c_int64(Rk[0].shape[0]), *Ra,
+            x.ctypes.data_as(dp), y.ctypes.data_as(dp), z.ctypes.data_as(dp), pid.ctypes.data_as(up),
+            chi.ctypes.data_as(dp))
+    return x[:cnt], y[:cnt], z[:cnt], pid[:cnt], chi[:cnt]
+
+
 def row_number(dE, chi):
     dE, pdE = _d(dE); chi, pchi = _d(chi)
     return float(lib().orc_row_number(C.c_int32(dE.shape[0]), pdE, pchi))
