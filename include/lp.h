@@ -166,6 +166,34 @@ LP_API lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new /*
 LP_API lp_status lp_chunked_capacity(int64_t n, int32_t e, int64_t *capacity /*host*/);
 LP_API lp_status lp_set_count(lp_ctx *ctx, int64_t np_new);
 
+/* Exchange of the particles that crossed a rank interface (not part of lp_step), for a
+ * domain decomposed into boxes, one direction (axis 0, 1, 2) at a time with a left and a right neighbour per
+ * direction.  The library does the steps that touch particle data; sizing buffers and moving them between
+ * ranks (NCCL send/recv, a peer copy over NVLink, or a plain pointer between contexts on one GPU) is the
+ * caller's.  This rank owns [lo, hi) along `axis`; the global box and its periodicity are the context's.
+ *   lp_migrate_count   steps 1: destination of every particle -- 0 stays, 1 left, 2 right; a particle outside
+ *                      [lo, hi) goes to the neighbour through whose face the shorter way leads, the other way
+ *                      being the one around a periodic axis (positions were wrapped into the global box by the
+ *                      pusher) -- and the two totals.  Synchronises `stream` (the totals size the buffers).
+ *   lp_migrate_pack    step 4: the leavers' x, y, z, id and chi row, in ascending index order, into the send
+ *                      buffers.  A buffer for n particles is n * lp_migrate_record_bytes bytes, 16-byte
+ *                      aligned, laid out as arrays  x[n] | y[n] | z[n] | id[n] | chi[n][nbins];
+ *                      NULL is allowed for a buffer whose total is 0.
+ *   lp_migrate_unpack  step 8: the n_from_left particles of from_left, then the n_from_right of from_right
+ *                      (same layout, written by the neighbours' lp_migrate_pack): the k-th arrival goes into
+ *                      the k-th hole (ascending index), arrivals beyond the holes behind the last particle,
+ *                      holes beyond the arrivals are closed as lp_compact closes them.  *np_new = the new
+ *                      count; LP_ERR_WORKSPACE if it exceeds the capacity (grow with lp_rebind first: the
+ *                      paper's step 6).  Synchronises `stream` only when holes are left to compact.
+ * Order: count -> pack -> unpack, nothing that moves particles in between (LP_ERR_STATE otherwise); particles
+ * outside the global box on a non-periodic axis must have been deleted (lp_compact) before. */
+LP_API lp_status lp_migrate_record_bytes(const lp_ctx *ctx, size_t *bytes /*host*/);
+LP_API lp_status lp_migrate_count(lp_ctx *ctx, int axis, double lo, double hi, int64_t *n_left /*host*/,
+                                  int64_t *n_right /*host*/, void *stream);
+LP_API lp_status lp_migrate_pack(lp_ctx *ctx, void *buf_left, void *buf_right, void *stream);
+LP_API lp_status lp_migrate_unpack(lp_ctx *ctx, const void *from_left, int64_t n_from_left, const void *from_right,
+                                   int64_t n_from_right, int64_t *np_new /*host*/, void *stream);
+
 /* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
  * spectral update (order of Table 1, without the fluid stages). */
 LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);

@@ -18,7 +18,8 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_bind_particles", "lp_bind_diag", "lp_set_fields", "lp_interpolate", "lp_sort", "lp_push",
            "lp_spectral_update", "lp_step", "lp_step_host", "lp_get_diag", "lp_launch_count", "lp_get_bins",
            "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3", "lp_chunked_capacity", "lp_set_count",
-           "lp_measure_fp64_peak", "lp_set_pingpong", "lp_current_particles")
+           "lp_measure_fp64_peak", "lp_set_pingpong", "lp_current_particles",
+           "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack")
 
 
 class LPError(RuntimeError):
@@ -90,6 +91,10 @@ def load():
     lib.lp_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
     lib.lp_set_pingpong.argtypes = [vp, C.c_int, vp]
     lib.lp_current_particles.argtypes = [vp] + [C.POINTER(C.c_void_p)] * 5
+    lib.lp_migrate_record_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+    lib.lp_migrate_count.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int64), C.POINTER(C.c_int64), vp]
+    lib.lp_migrate_pack.argtypes = [vp, dp, dp, vp]
+    lib.lp_migrate_unpack.argtypes = [vp, dp, C.c_int64, dp, C.c_int64, C.POINTER(C.c_int64), vp]
     for name in EXPORTS:
         if name != "lp_last_error":
             getattr(lib, name).restype = C.c_int
@@ -199,6 +204,28 @@ def lp_push_rk3(ctx, dt, stage, stream=None):
 def lp_compact(ctx, flag_ptr, stream=None):
     n = C.c_int64()
     _check(ctx, load().lp_compact(ctx, flag_ptr, C.byref(n), stream))
+    return int(n.value)
+
+
+def lp_migrate_record_bytes(ctx):
+    out = C.c_size_t()
+    _check(ctx, load().lp_migrate_record_bytes(ctx, C.byref(out)))
+    return out.value
+
+
+def lp_migrate_count(ctx, axis, lo, hi, stream=None):
+    nl = C.c_int64(); nr = C.c_int64()
+    _check(ctx, load().lp_migrate_count(ctx, int(axis), float(lo), float(hi), C.byref(nl), C.byref(nr), stream))
+    return int(nl.value), int(nr.value)
+
+
+def lp_migrate_pack(ctx, buf_left, buf_right, stream=None):
+    _check(ctx, load().lp_migrate_pack(ctx, buf_left, buf_right, stream))
+
+
+def lp_migrate_unpack(ctx, from_left, n_from_left, from_right, n_from_right, stream=None):
+    n = C.c_int64()
+    _check(ctx, load().lp_migrate_unpack(ctx, from_left, int(n_from_left), from_right, int(n_from_right), C.byref(n), stream))
     return int(n.value)
 
 

@@ -173,6 +173,9 @@ struct lp_ctx {
     // (lp_set_pingpong) a re-sort reads one set through the permutation and writes the other, and `cur` flips.
     bool pingpong = false;
     int cur = 0;
+    // particle exchange in progress (lp_migrate_count -> _pack -> _unpack): 0 none, 1 counted, 2 packed
+    int mig_stage = 0;
+    long long mig_left = 0, mig_right = 0;
     bool split_records = false;            // cell records as two 32-byte arrays (dense sets) or one 64-byte array (LpCells)
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
@@ -331,6 +334,7 @@ lp_status do_spectral(lp_ctx *c, double dt, const SpectralIO &io, bool fused, cu
     }
     if (st == LP_OK) {
         c->spectra_done = true;
+        c->mig_stage = 0;                   // (the fused step moves the particles)
         c->stage0_done = false; c->rk3_next = 0; c->push_done = false;
         if (fused) c->status_valid = true;
     }
@@ -382,6 +386,7 @@ void sort_invalidates(lp_ctx *c)
     c->stage0_done = false; c->rk3_next = 0; c->push_done = false;      // k1 / x* / rho_old refer to the old order
     c->spectra_done = false;     // so do the per-particle n_sub / lost of the last update
     c->status_valid = false;
+    c->mig_stage = 0;
     ++c->sorts;
 }
 
@@ -525,6 +530,7 @@ lp_status lp_bind_particles(lp_ctx *ctx, double *x, double *y, double *z, uint64
     if (reinterpret_cast<uintptr_t>(chi) % 16) return fail(ctx, LP_ERR_INVALID_ARG, "chi not 16-byte aligned");
     ctx->x = x; ctx->y = y; ctx->z = z; ctx->id = id; ctx->chi = chi;
     ctx->cur = 0;                       // the state is what the caller just bound
+    ctx->mig_stage = 0;
     ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
     ctx->spectra_done = false;
     ctx->status_valid = false;
@@ -593,7 +599,7 @@ lp_status lp_push(lp_ctx *ctx, double dt, int stage, void *stream)
         return st;
     }
     st = count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch");
-    if (st == LP_OK) { ctx->status_valid = true; ctx->push_done = true; }
+    if (st == LP_OK) { ctx->status_valid = true; ctx->push_done = true; ctx->mig_stage = 0; }
     return st;
 }
 
@@ -610,6 +616,7 @@ lp_status lp_push_rk3(lp_ctx *ctx, double dt, int stage, void *stream)
         st = count(ctx, lp_launch_push_rk3(a, stage, static_cast<cudaStream_t>(stream)), "lp_push_rk3_kernel launch");
         if (st != LP_OK) return st;
     }
+    ctx->mig_stage = 0;                 // every stage writes the bound positions
     if (stage == 0) { ctx->stage0_done = true; ctx->push_kind = 2; ctx->status_valid = false; ctx->push_done = false; }
     if (stage == 2) { ctx->status_valid = true; ctx->push_done = true; }
     ctx->rk3_next = stage == 2 ? 0 : stage + 1;
@@ -660,6 +667,7 @@ lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *st
     LP_CUDA(ctx, cudaMemcpyAsync(h_counts, counts, sizeof h_counts, cudaMemcpyDeviceToHost, s));
     LP_CUDA(ctx, cudaStreamSynchronize(s));
     ctx->cfg.np -= (long long)h_counts[0];          // the workspace keeps its size (capacity)
+    ctx->mig_stage = 0;
     ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
     ctx->spectra_done = false;
     ctx->status_valid = false;
@@ -683,6 +691,7 @@ lp_status lp_set_count(lp_ctx *ctx, int64_t np_new)
     if (np_new > 0 && ctx->ws && !ctx->x) return fail(ctx, LP_ERR_STATE, "no particles bound (lp_bind_particles)");
     if (np_new > ctx->cfg.np) ctx->id_bits_stale = true;      // injected particles bring their own ids
     ctx->cfg.np = np_new;
+    ctx->mig_stage = 0;
     ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
     ctx->spectra_done = false;
     ctx->status_valid = false;
@@ -719,6 +728,106 @@ lp_status lp_current_particles(const lp_ctx *ctx, double **x, double **y, double
     if (z) *z = n.z;
     if (id) *id = n.id;
     if (chi) *chi = n.chi;
+    return LP_OK;
+}
+
+lp_status lp_migrate_record_bytes(const lp_ctx *ctx, size_t *bytes)
+{
+    if (!ctx || !bytes) return LP_ERR_INVALID_ARG;
+    *bytes = 32 + 8 * (size_t)ctx->cfg.nbins;
+    return LP_OK;
+}
+
+lp_status lp_migrate_count(lp_ctx *ctx, int axis, double lo, double hi, int64_t *n_left, int64_t *n_right, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    if (axis < 0 || axis > 2 || !n_left || !n_right || !(hi > lo)) return fail(ctx, LP_ERR_INVALID_ARG, "bad axis, interval or NULL output");
+    ctx->mig_stage = 0;
+    *n_left = *n_right = 0;
+    ctx->mig_left = ctx->mig_right = 0;
+    if (ctx->cfg.np > 0) {
+        LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+        cudaStream_t s = static_cast<cudaStream_t>(stream);
+        const lp_ctx::Set n = ctx->now();
+        const double *pos = axis == 0 ? n.x : (axis == 1 ? n.y : n.z);
+        unsigned long long *counts = ctx->at<unsigned long long>(ctx->lay.partial), h[2] = { 0, 0 };
+        st = count(ctx, lp_launch_migrate_count(pos, ctx->cfg.np, lo, hi, ctx->geom.len[axis], ctx->geom.per[axis],
+                                                ctx->at<uint32_t>(ctx->lay.key), ctx->at<unsigned long long>(ctx->lay.hist), counts,
+                                                ctx->at<uint32_t>(ctx->lay.idx_a), ctx->at<uint32_t>(ctx->lay.idx_b), s),
+                   "exchange count kernels launch");
+        if (st != LP_OK) return st;
+        LP_CUDA(ctx, cudaMemcpyAsync(h, counts, sizeof h, cudaMemcpyDeviceToHost, s));
+        LP_CUDA(ctx, cudaStreamSynchronize(s));
+        ctx->mig_left = (long long)h[0];
+        ctx->mig_right = (long long)h[1];
+    }
+    *n_left = ctx->mig_left;
+    *n_right = ctx->mig_right;
+    ctx->mig_stage = 1;
+    return LP_OK;
+}
+
+lp_status lp_migrate_pack(lp_ctx *ctx, void *buf_left, void *buf_right, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    if (ctx->mig_stage != 1) return fail(ctx, LP_ERR_STATE, "lp_migrate_pack needs lp_migrate_count first");
+    if ((ctx->mig_left > 0 && !buf_left) || (ctx->mig_right > 0 && !buf_right)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL send buffer");
+    if (reinterpret_cast<uintptr_t>(buf_left) % 16 || reinterpret_cast<uintptr_t>(buf_right) % 16)
+        return fail(ctx, LP_ERR_INVALID_ARG, "send buffer not 16-byte aligned");
+    const long long nleave = ctx->mig_left + ctx->mig_right;
+    if (nleave > 0) {
+        LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+        const lp_ctx::Set n = ctx->now();
+        st = count(ctx, lp_launch_migrate_pack(ctx->at<unsigned long long>(ctx->lay.partial), nleave, ctx->at<uint32_t>(ctx->lay.idx_b),
+                                               n.x, n.y, n.z, n.id, n.chi, ctx->cfg.nbins, buf_left, buf_right, ctx->sm_count,
+                                               static_cast<cudaStream_t>(stream)), "exchange pack kernel launch");
+        if (st != LP_OK) return st;
+    }
+    ctx->mig_stage = 2;
+    return LP_OK;
+}
+
+lp_status lp_migrate_unpack(lp_ctx *ctx, const void *from_left, int64_t n_from_left, const void *from_right,
+                            int64_t n_from_right, int64_t *np_new, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    if (!np_new) return fail(ctx, LP_ERR_INVALID_ARG, "np_new is NULL");
+    *np_new = ctx->cfg.np;
+    if (ctx->mig_stage != 2) return fail(ctx, LP_ERR_STATE, "lp_migrate_unpack needs lp_migrate_pack first");
+    if (n_from_left < 0 || n_from_right < 0 || (n_from_left > 0 && !from_left) || (n_from_right > 0 && !from_right))
+        return fail(ctx, LP_ERR_INVALID_ARG, "bad receive buffer");
+    if (reinterpret_cast<uintptr_t>(from_left) % 16 || reinterpret_cast<uintptr_t>(from_right) % 16)
+        return fail(ctx, LP_ERR_INVALID_ARG, "receive buffer not 16-byte aligned");
+    const long long np = ctx->cfg.np, nholes = ctx->mig_left + ctx->mig_right, nin = n_from_left + n_from_right;
+    const long long grown = np + (nin > nholes ? nin - nholes : 0);
+    if (grown > ctx->capacity)
+        return fail(ctx, LP_ERR_WORKSPACE, "arrivals exceed the capacity of the particle arrays (lp_rebind to grow)");
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const lp_ctx::Set n = ctx->now();
+    int32_t *flag = ctx->at<int32_t>(ctx->lay.nsub);          // (per-particle n_sub is invalidated below anyway)
+    const bool rest = nin < nholes;
+    if (rest) LP_CUDA(ctx, cudaMemsetAsync(flag, 0, (size_t)np * 4, s));
+    if (nin > 0 || rest) {
+        st = count(ctx, lp_launch_migrate_unpack(from_left, n_from_left, from_right, n_from_right, ctx->at<uint32_t>(ctx->lay.idx_a),
+                                                 nholes, np, n.x, n.y, n.z, n.id, n.chi, ctx->cfg.nbins, rest ? flag : nullptr,
+                                                 ctx->sm_count, s), "exchange unpack kernels launch");
+        if (st != LP_OK) return st;
+    }
+    ctx->mig_stage = 0;
+    ctx->cfg.np = grown;
+    ctx->id_bits_stale = true;                                // arrivals bring their own ids
+    ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
+    ctx->spectra_done = false;
+    ctx->status_valid = false;
+    if (rest) {                                               // holes no arrival filled: the compaction of Section 3.2
+        int64_t after = 0;
+        if ((st = lp_compact(ctx, flag, &after, stream)) != LP_OK) return st;
+    }
+    *np_new = ctx->cfg.np;
     return LP_OK;
 }
 

@@ -137,6 +137,29 @@ class LP:
         self.cfg.np = n
         return n
 
+    # ---- particle exchange across rank interfaces: count -> pack -> (move buffers) -> unpack
+    def migrate_count(self, axis, lo, hi):
+        """(n_left, n_right): particles leaving [lo, hi) along `axis` towards the left / right neighbour."""
+        return B.lp_migrate_count(self.ctx, axis, lo, hi, self.stream)
+
+    def migrate_buffer(self, n):
+        """An (uninitialised) send / receive buffer for n particles: uint8 CUDA tensor, n * (32 + 8 nbins) bytes."""
+        return torch.empty(max(1, n) * B.lp_migrate_record_bytes(self.ctx), dtype=torch.uint8, device=self.device)
+
+    def migrate_pack(self, n_left, n_right):
+        """Packs the leavers counted by migrate_count; returns (buf_left, buf_right)."""
+        bl, br = self.migrate_buffer(n_left), self.migrate_buffer(n_right)
+        B.lp_migrate_pack(self.ctx, bl.data_ptr() if n_left else None, br.data_ptr() if n_right else None, self.stream)
+        return bl, br
+
+    def migrate_unpack(self, from_left, n_from_left, from_right, n_from_right):
+        """Arrivals into the holes / behind the last particle; returns the new particle count."""
+        n = B.lp_migrate_unpack(self.ctx, from_left.data_ptr() if n_from_left else None, n_from_left,
+                                from_right.data_ptr() if n_from_right else None, n_from_right, self.stream)
+        self._keep = (from_left, from_right)      # alive until the stream has consumed them
+        self.cfg.np = n
+        return n
+
     def step(self, dt):
         B.lp_step(self.ctx, dt, self.stream)
 
