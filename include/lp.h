@@ -194,6 +194,23 @@ LP_API lp_status lp_migrate_pack(lp_ctx *ctx, void *buf_left, void *buf_right, v
 LP_API lp_status lp_migrate_unpack(lp_ctx *ctx, const void *from_left, int64_t n_from_left, const void *from_right,
                                    int64_t n_from_right, int64_t *np_new /*host*/, void *stream);
 
+/* Growing and shrinking the particle storage in whole chunks (Listing 1; Reserve() / Shrink()
+ * of Listing 2).  The paper's BlockedContainer appends or frees chunks of L = 2^e elements; here
+ * every array is one flat caller-owned allocation (the kernels need contiguous rows), so a change of capacity is:
+ * the caller allocates particle arrays and a workspace for the new capacity -- lp_chunked_capacity(N, e) particles,
+ * lp_workspace_bytes_for bytes -- and lp_rebind moves the context onto them.  On `stream` it copies the current
+ * particles (x, y, z, id, chi rows, from wherever they live: the bound arrays or their ping-pong twins) and the
+ * staged cell records (the fields stay set); the old arrays and workspace may be released once the stream has
+ * passed the call.  capacity >= the current count (Shrink() only ever drops trailing free chunks).  Afterwards the
+ * state is in the new bound arrays, the lp_bind_diag outputs are unbound (they were sized for the old capacity),
+ * per-particle results of earlier calls are invalid, and an exchange between lp_migrate_pack and
+ * lp_migrate_unpack survives (the paper's step 6: "resize the particle container to accommodate the new
+ * particles"). */
+LP_API lp_status lp_capacity(const lp_ctx *ctx, int64_t *capacity /*host*/);
+LP_API lp_status lp_workspace_bytes_for(const lp_ctx *ctx, int64_t capacity, size_t *out_bytes /*host*/);
+LP_API lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_t bytes, double *x, double *y,
+                           double *z, uint64_t *id, double *chi, void *stream);
+
 /* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
  * spectral update (order of Table 1, without the fluid stages). */
 LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);

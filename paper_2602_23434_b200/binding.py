@@ -19,7 +19,8 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_spectral_update", "lp_step", "lp_step_host", "lp_get_diag", "lp_launch_count", "lp_get_bins",
            "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3", "lp_chunked_capacity", "lp_set_count",
            "lp_measure_fp64_peak", "lp_set_pingpong", "lp_current_particles",
-           "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack")
+           "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack",
+           "lp_capacity", "lp_workspace_bytes_for", "lp_rebind")
 
 
 class LPError(RuntimeError):
@@ -91,6 +92,9 @@ def load():
     lib.lp_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
     lib.lp_set_pingpong.argtypes = [vp, C.c_int, vp]
     lib.lp_current_particles.argtypes = [vp] + [C.POINTER(C.c_void_p)] * 5
+    lib.lp_capacity.argtypes = [vp, C.POINTER(C.c_int64)]
+    lib.lp_workspace_bytes_for.argtypes = [vp, C.c_int64, C.POINTER(C.c_size_t)]
+    lib.lp_rebind.argtypes = [vp, C.c_int64, dp, C.c_size_t, dp, dp, dp, dp, dp, vp]
     lib.lp_migrate_record_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     lib.lp_migrate_count.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int64), C.POINTER(C.c_int64), vp]
     lib.lp_migrate_pack.argtypes = [vp, dp, dp, vp]
@@ -227,6 +231,22 @@ def lp_migrate_unpack(ctx, from_left, n_from_left, from_right, n_from_right, str
     n = C.c_int64()
     _check(ctx, load().lp_migrate_unpack(ctx, from_left, int(n_from_left), from_right, int(n_from_right), C.byref(n), stream))
     return int(n.value)
+
+
+def lp_capacity(ctx):
+    out = C.c_int64()
+    _check(ctx, load().lp_capacity(ctx, C.byref(out)))
+    return int(out.value)
+
+
+def lp_workspace_bytes_for(ctx, capacity):
+    out = C.c_size_t()
+    _check(ctx, load().lp_workspace_bytes_for(ctx, int(capacity), C.byref(out)))
+    return out.value
+
+
+def lp_rebind(ctx, capacity, workspace, nbytes, x, y, z, pid, chi, stream=None):
+    _check(ctx, load().lp_rebind(ctx, int(capacity), workspace, nbytes, x, y, z, pid, chi, stream))
 
 
 def lp_set_pingpong(ctx, enable, stream=None):

@@ -698,6 +698,70 @@ lp_status lp_set_count(lp_ctx *ctx, int64_t np_new)
     return LP_OK;
 }
 
+lp_status lp_capacity(const lp_ctx *ctx, int64_t *capacity)
+{
+    if (!ctx || !capacity) return LP_ERR_INVALID_ARG;
+    *capacity = ctx->capacity;
+    return LP_OK;
+}
+
+lp_status lp_workspace_bytes_for(const lp_ctx *ctx, int64_t capacity, size_t *out_bytes)
+{
+    if (!ctx || !out_bytes || capacity < 0 || capacity > 0xffffffffll) return LP_ERR_INVALID_ARG;
+    lp_config c = ctx->cfg;
+    c.np = capacity;
+    *out_bytes = make_layout(c).total;
+    return LP_OK;
+}
+
+lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_t bytes, double *x, double *y, double *z,
+                    uint64_t *id, double *chi, void *stream)
+{
+    lp_status st = need_ready(ctx, false);
+    if (st != LP_OK) return st;
+    if (capacity < ctx->cfg.np || capacity > 0xffffffffll) return fail(ctx, LP_ERR_INVALID_ARG, "capacity below the particle count or >= 2^32");
+    if (capacity > 0 && (!x || !y || !z || !id || !chi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL particle array");
+    if (reinterpret_cast<uintptr_t>(chi) % 16) return fail(ctx, LP_ERR_INVALID_ARG, "chi not 16-byte aligned");
+    if (!workspace) return fail(ctx, LP_ERR_WORKSPACE, "workspace is NULL");
+    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return fail(ctx, LP_ERR_WORKSPACE, "workspace not 256-byte aligned");
+    lp_config ncfg = ctx->cfg;
+    ncfg.np = capacity;
+    const Layout nl = make_layout(ncfg);
+    if (bytes < nl.total) return fail(ctx, LP_ERR_WORKSPACE, "workspace smaller than lp_workspace_bytes_for(capacity)");
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    unsigned char *nws = static_cast<unsigned char *>(workspace);
+    const size_t np = (size_t)ctx->cfg.np, nb = (size_t)ctx->cfg.nbins;
+    const lp_ctx::Set n = ctx->now();
+    if (np) {
+        LP_CUDA(ctx, cudaMemcpyAsync(x, n.x, np * 8, cudaMemcpyDeviceToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(y, n.y, np * 8, cudaMemcpyDeviceToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(z, n.z, np * 8, cudaMemcpyDeviceToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(id, n.id, np * 8, cudaMemcpyDeviceToDevice, s));
+        LP_CUDA(ctx, cudaMemcpyAsync(chi, n.chi, np * nb * 8, cudaMemcpyDeviceToDevice, s));
+    }
+    if (ctx->have_fields)
+        LP_CUDA(ctx, cudaMemcpyAsync(nws + nl.rec, ctx->ws + ctx->lay.rec, (size_t)ctx->cfg.nx * ctx->cfg.ny * ctx->cfg.nz * 64,
+                                     cudaMemcpyDeviceToDevice, s));
+    if (ctx->mig_stage == 2) {          // an exchange is under way: its hole list moves along
+        const size_t nholes = (size_t)(ctx->mig_left + ctx->mig_right);
+        if (nholes) LP_CUDA(ctx, cudaMemcpyAsync(nws + nl.idx_a, ctx->ws + ctx->lay.idx_a, nholes * 4, cudaMemcpyDeviceToDevice, s));
+    } else {
+        ctx->mig_stage = 0;
+    }
+    ctx->ws = nws;
+    ctx->lay = nl;
+    ctx->capacity = capacity;
+    ctx->x = x; ctx->y = y; ctx->z = z; ctx->id = id; ctx->chi = chi;
+    ctx->cur = 0;
+    ctx->nsub_user = nullptr;
+    ctx->lost_user = nullptr;
+    ctx->stage0_done = false; ctx->rk3_next = 0; ctx->push_done = false;
+    ctx->spectra_done = false;
+    ctx->status_valid = false;
+    return LP_OK;
+}
+
 lp_status lp_set_pingpong(lp_ctx *ctx, int enable, void *stream)
 {
     lp_status st = need_ready(ctx, false);

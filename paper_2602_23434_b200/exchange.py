@@ -10,8 +10,8 @@ import torch.distributed as dist
 def exchange_direction(lp, axis, lo, hi, left, right, group=None):
     """One directional sweep for this rank, which owns [lo, hi) along `axis`.  `left` / `right`: the ranks of
     the two neighbours (None: no neighbour on that side; both may be the same rank on a periodic axis cut in
-    two).  Steps 1-8 of PAPER.md:201-214: count, post receives, size buffers, pack, send, (the arrays were
-    created with room for the arrivals), wait, unpack.  Returns the new particle count."""
+    two).  Steps 1-8 of PAPER.md:201-214: count, post receives, size buffers, pack, send, grow the particle
+    arrays by whole chunks if the arrivals do not fit, wait, unpack.  Returns the new particle count."""
     n_left, n_right = lp.migrate_count(axis, lo, hi)                      # step 1
     if (left is None and n_left) or (right is None and n_right):
         raise RuntimeError("particles leave through a side without a neighbour (delete them first: lp_compact)")
@@ -24,6 +24,9 @@ def exchange_direction(lp, axis, lo, hi, left, right, group=None):
     n_from_left, n_from_right = int(recv_l.item()), int(recv_r.item())
     in_l, in_r = lp.migrate_buffer(n_from_left), lp.migrate_buffer(n_from_right)      # steps 2-3
     out_l, out_r = lp.migrate_pack(n_left, n_right)                       # step 4
+    surplus = n_from_left + n_from_right - (n_left + n_right)
+    if surplus > 0 and hasattr(lp, "reserve"):
+        lp.reserve(surplus)                                               # step 6 (no-op while the capacity suffices)
     _p2p([(out_l, left if n_left else None), (out_r, right if n_right else None)],
          [(in_r, right if n_from_right else None), (in_l, left if n_from_left else None)], group)    # steps 5, 7
     return lp.migrate_unpack(in_l, n_from_left, in_r, n_from_right)       # steps 6, 8

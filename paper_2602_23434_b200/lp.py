@@ -14,14 +14,17 @@ class LP:
         B.load()
         self.ctx = B.lp_create(cfg)
         nbytes = B.lp_workspace_bytes(cfg)
-        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-        off = (-self.workspace.data_ptr()) % 256
-        B.lp_bind_workspace(self.ctx, self.workspace.data_ptr() + off, nbytes)
+        self.workspace, ptr = self._alloc_workspace(nbytes)
+        B.lp_bind_workspace(self.ctx, ptr, nbytes)
         self.workspace_bytes = nbytes
         self._bound = None            # the caller-side tensors x, y, z, id, chi (the bound arrays)
         self.capacity = cfg.np
         self.nsub = self.lost = None
         self._fields = None
+
+    def _alloc_workspace(self, nbytes):
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        return ws, ws.data_ptr() + (-ws.data_ptr()) % 256
 
     def close(self):
         if self.ctx is not None:
@@ -85,7 +88,7 @@ class LP:
     chi = property(lambda self: self.current()[4])
 
     def bind_diag(self, nsub=True, lost=True):
-        n = self.cfg.np
+        n = self.capacity
         self.nsub = torch.zeros(n, dtype=torch.int32, device=self.device) if nsub else None
         self.lost = torch.zeros(n, dtype=torch.float64, device=self.device) if lost else None
         B.lp_bind_diag(self.ctx, self.nsub.data_ptr() if nsub else None, self.lost.data_ptr() if lost else None)
@@ -126,6 +129,40 @@ class LP:
         """Use the first n particles of the bound arrays (n <= the capacity the context was created with)."""
         B.lp_set_count(self.ctx, n)
         self.cfg.np = n            # (the binding's copy of the count sizes the outputs of interpolate)
+
+    # ---- chunked growth (PAPER.md:176-184 Listing 1; Reserve() / Shrink() of Listing 2)
+    def _rebind(self, capacity):
+        n, nb = self.cfg.np, self.cfg.nbins
+        f64 = lambda *shape: torch.empty(shape, dtype=torch.float64, device=self.device)
+        new = (f64(capacity), f64(capacity), f64(capacity),
+               torch.empty(capacity, dtype=torch.int64, device=self.device), f64(capacity, nb))
+        nbytes = B.lp_workspace_bytes_for(self.ctx, capacity)
+        ws, ptr = self._alloc_workspace(nbytes)
+        B.lp_rebind(self.ctx, capacity, ptr, nbytes, *[t.data_ptr() for t in new], self.stream)
+        # the old tensors stay referenced until the stream has passed the copies
+        self._retired = (self._bound, self.workspace, self.nsub, self.lost)
+        self._bound, self.workspace, self.workspace_bytes, self.capacity = new, ws, nbytes, capacity
+        had = (self.nsub is not None, self.lost is not None)
+        self.nsub = self.lost = None
+        if any(had):
+            self.bind_diag(*had)
+
+    def reserve(self, n_new, e=18):
+        """Room for n_new more particles behind the current ones (Listing 2's Reserve): when the capacity does
+        not suffice, storage for lp_chunked_capacity(count + n_new, e) particles -- whole chunks of 2^e -- is
+        allocated and the state moved there (lp_rebind).  Write the new particles into x, y, z, id, chi
+        [count : count + n_new] and call set_count.  Returns the capacity."""
+        need = self.cfg.np + int(n_new)
+        if need > self.capacity:
+            self._rebind(B.lp_chunked_capacity(need, e))
+        return self.capacity
+
+    def shrink(self, e=18):
+        """Release the trailing chunks that hold no particle (Listing 2's Shrink).  Returns the capacity."""
+        cap = max(B.lp_chunked_capacity(self.cfg.np, e), 1 << e)
+        if cap < self.capacity:
+            self._rebind(cap)
+        return self.capacity
 
     def compact(self, flag=None):
         """Delete the flagged particles (int32 CUDA tensor [np], nonzero = delete; None = those outside the
