@@ -28,6 +28,7 @@
  *   orc_compact          deletion with hole filling          PAPER.md:190-199                    C1
  *   orc_push_rk3_stage   three-stage third-order pusher      PAPER.md:245, 258-260               K1
  *   orc_migrate_pack/unpack  exchange across rank interfaces PAPER.md:201-214                    M1-M3
+ *   orc_moving_row/update    per-particle moving energy grid PAPER.md:107, 122, 606-613, 685     E1-E4
  *   orc_step             one whole step with frozen fields   PAPER.md:216-233 (Table 1)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force cell search and O(N^2)
@@ -514,6 +515,53 @@ int64_t orc_migrate_unpack(int64_t np, int32_t nbins, const int64_t *holes, int6
         free(flag);
     }
     return count;
+}
+
+/* ---------------------------------------------------------------- moving energy grid (NEXT-5) */
+
+/* Listing 3 gives every particle its own energy array eng_ next to chi_ and the text
+ * defers the method to Section 2.3.2 of [19], which is not available.  Readings (DESIGN.md
+ * section 3, E1-E4):
+ *  E1 eng holds the particle's N_b + 1 bin edges, chi_i the mean of chi over [eng_i, eng_{i+1}].
+ *  E2 over one step the edges follow the characteristics of Eq. 6,
+ *       d(eps)/d(tau) = -eps (a + c_r eps),      a, c_r as orc_coefficients, frozen over the step (R9),
+ *     whose solution over dtau is, with s = a dtau:
+ *       eps(dtau) = eps0 e^{-s} / (1 + beta eps0),   beta = c_r dtau (1 - e^{-s}) / s   (= c_r dtau for s = 0).
+ *     (e^{-s} = (rho_new/rho_old)^{1/3}: the adiabatic law; a = 0: eps0 / (1 + c_r eps0 dtau), the
+ *     synchrotron law of north_star.)
+ *  E3 Eq. 6 is a conservation law, so the number of a bin moves with its edges:
+ *       chi_i <- chi_i (eng_{i+1} - eng_i)_old / (eng_{i+1} - eng_i)_new.
+ *     No flux crosses an edge: no CFL limit, no substeps, nothing is lost through the ends.
+ *  E4 the grid starts as the fixed log-spaced table (orc_bin_table). */
+void orc_moving_row(int32_t nbins, double a, double cr, double dtau,
+                    double *eng /*[nbins+1] in/out*/, double *chi /*[nbins] in/out*/)
+{
+    const double s = a * dtau;
+    const double alpha = exp(-s);
+    const double beta = (s != 0.0) ? cr * dtau * (-expm1(-s) / s) : cr * dtau;
+    double *en = (double *)malloc((size_t)(nbins + 1) * sizeof(double));
+    for (int k = 0; k <= nbins; ++k) en[k] = eng[k] * alpha / (1.0 + beta * eng[k]);
+    for (int i = 0; i < nbins; ++i) chi[i] = chi[i] * (eng[i + 1] - eng[i]) / (en[i + 1] - en[i]);
+    for (int k = 0; k <= nbins; ++k) eng[k] = en[k];
+    free(en);
+}
+
+/* Particles_Spectra with the moving grid: gather at the current position, coefficients, orc_moving_row. */
+void orc_moving_update(const orc_params *g, const double *const *fields7, int64_t np,
+                       const double *x, const double *y, const double *z, const double *rho_old, double dt,
+                       double *eng /*[np][nbins+1]*/, double *chi /*[np][nbins]*/, int32_t nthreads)
+{
+    const int nb = g->nbins;
+    (void)nthreads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads > 0 ? nthreads : 1)
+#endif
+    for (int64_t p = 0; p < np; ++p) {
+        double o[7], a, cr, dtau;
+        gather_point(g, 7, fields7, x[p], y[p], z[p], o);
+        orc_coefficients(g, dt, &o[0], &o[3], o[6], rho_old[p], &a, &cr, &dtau);
+        orc_moving_row(nb, a, cr, dtau, eng + p * (nb + 1), chi + p * nb);
+    }
 }
 
 /* ---------------------------------------------------------------- whole update / step */

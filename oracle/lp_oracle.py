@@ -282,6 +282,32 @@ def migrate_unpack(holes, from_left, from_right, x, y, z, pid, chi):
     return x[:cnt], y[:cnt], z[:cnt], pid[:cnt], chi[:cnt]
 
 
+def moving_row(a, cr, dtau, eng, chi):
+    """One step of the moving energy grid on one particle; returns (new edges, new chi)."""
+    eng = np.array(eng, dtype=np.float64); chi = np.array(chi, dtype=np.float64)
+    f = lib().orc_moving_row
+    f.restype = None
+    dp = C.POINTER(C.c_double)
+    f(C.c_int32(chi.shape[0]), C.c_double(a), C.c_double(cr), C.c_double(dtau), eng.ctypes.data_as(dp),
+      chi.ctypes.data_as(dp))
+    return eng, chi
+
+
+def moving_update(prm, fields7, x, y, z, rho_old, dt, eng, chi, nthreads=1):
+    """Returns (new eng [np,nbins+1], new chi [np,nbins])."""
+    keep, fa = _fields(fields7)
+    x, px = _d(x); y, py = _d(y); z, pz = _d(z); rho_old, pr = _d(rho_old)
+    eng = np.array(eng, dtype=np.float64, order="C"); chi = np.array(chi, dtype=np.float64, order="C")
+    n = x.shape[0]
+    assert chi.shape == (n, prm.nbins) and eng.shape == (n, prm.nbins + 1)
+    f = lib().orc_moving_update
+    f.restype = None
+    dp = C.POINTER(C.c_double)
+    f(C.byref(prm), fa, C.c_int64(n), px, py, pz, pr, C.c_double(dt), eng.ctypes.data_as(dp), chi.ctypes.data_as(dp),
+      C.c_int32(nthreads))
+    return eng, chi
+
+
 def row_number(dE, chi):
     dE, pdE = _d(dE); chi, pchi = _d(chi)
     return float(lib().orc_row_number(C.c_int32(dE.shape[0]), pdE, pchi))
