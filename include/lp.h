@@ -211,6 +211,23 @@ LP_API lp_status lp_workspace_bytes_for(const lp_ctx *ctx, int64_t capacity, siz
 LP_API lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_t bytes, double *x, double *y,
                            double *z, uint64_t *id, double *chi, void *stream);
 
+/* Per-particle moving energy grid (the eng_ array of Listing 3; the method is deferred to
+ * [19] by PAPER.md:122 -- readings E1-E4 of DESIGN.md): an alternative to the fixed log-spaced bins.  Every particle
+ * carries its own nbins + 1 bin edges eng[p*(nbins+1) + k]; over a step they follow the characteristics of Eq. 6
+ * (PAPER.md:107), eps' = eps e^{-s} / (1 + beta eps) with s = a dtau, beta = c_r dtau (1 - e^{-s})/s, and every bin
+ * keeps its number, chi_i' = chi_i dE_i / dE_i': exact for frozen coefficients, no CFL limit, no substeps, no
+ * numerical diffusion, nothing lost through the ends.
+ *   lp_bind_energy_grid  eng [capacity][nbins+1] (device, caller-owned, updated in place) switches the context to the
+ *                        moving grid: lp_spectral_update and lp_step use it (lp_step then runs the staged kernels in a
+ *                        row), n_sub reads 1, lp_get_diag's number uses the particle's own widths.  eng_scratch: a
+ *                        second array of the same size through which a sort moves the rows (NULL: sorts return
+ *                        LP_ERR_STATE).  eng = NULL switches back to the fixed bins.
+ *   lp_init_energy_grid  rows [first, first + count) <- the fixed table's edges (the grid every particle starts on).
+ * Calls that move particles without their grid rows -- lp_compact, lp_migrate_*, lp_rebind, lp_step_host -- and
+ * lp_shock_update (its bin centres are the fixed table's) return LP_ERR_UNSUPPORTED while a grid is bound. */
+LP_API lp_status lp_bind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch);
+LP_API lp_status lp_init_energy_grid(lp_ctx *ctx, int64_t first, int64_t count, void *stream);
+
 /* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
  * spectral update (order of Table 1, without the fluid stages). */
 LP_API lp_status lp_step(lp_ctx *ctx, double dt, void *stream);

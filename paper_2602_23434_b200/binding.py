@@ -20,7 +20,8 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3", "lp_chunked_capacity", "lp_set_count",
            "lp_measure_fp64_peak", "lp_set_pingpong", "lp_current_particles",
            "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack",
-           "lp_capacity", "lp_workspace_bytes_for", "lp_rebind")
+           "lp_capacity", "lp_workspace_bytes_for", "lp_rebind",
+           "lp_bind_energy_grid", "lp_init_energy_grid")
 
 
 class LPError(RuntimeError):
@@ -92,6 +93,8 @@ def load():
     lib.lp_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
     lib.lp_set_pingpong.argtypes = [vp, C.c_int, vp]
     lib.lp_current_particles.argtypes = [vp] + [C.POINTER(C.c_void_p)] * 5
+    lib.lp_bind_energy_grid.argtypes = [vp, dp, dp]
+    lib.lp_init_energy_grid.argtypes = [vp, C.c_int64, C.c_int64, vp]
     lib.lp_capacity.argtypes = [vp, C.POINTER(C.c_int64)]
     lib.lp_workspace_bytes_for.argtypes = [vp, C.c_int64, C.POINTER(C.c_size_t)]
     lib.lp_rebind.argtypes = [vp, C.c_int64, dp, C.c_size_t, dp, dp, dp, dp, dp, vp]
@@ -231,6 +234,14 @@ def lp_migrate_unpack(ctx, from_left, n_from_left, from_right, n_from_right, str
     n = C.c_int64()
     _check(ctx, load().lp_migrate_unpack(ctx, from_left, int(n_from_left), from_right, int(n_from_right), C.byref(n), stream))
     return int(n.value)
+
+
+def lp_bind_energy_grid(ctx, eng, eng_scratch=None):
+    _check(ctx, load().lp_bind_energy_grid(ctx, eng, eng_scratch))
+
+
+def lp_init_energy_grid(ctx, first, count, stream=None):
+    _check(ctx, load().lp_init_energy_grid(ctx, int(first), int(count), stream))
 
 
 def lp_capacity(ctx):

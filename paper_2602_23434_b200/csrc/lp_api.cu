@@ -145,6 +145,7 @@ struct lp_ctx {
     uint64_t *id = nullptr;
     int32_t *nsub_user = nullptr;
     double *lost_user = nullptr;
+    double *eng = nullptr, *eng_scratch = nullptr;      // per-particle energy grid (lp_bind_energy_grid): moving-grid mode
     // owned small tables
     double *tab = nullptr;                 // E[nb+1] | dE[nb] | rdE[nb]
     std::vector<double> h_edges, h_widths;
@@ -250,6 +251,32 @@ lp_status need_ready(lp_ctx *c, bool fields)
     if (c->cfg.np > 0 && !c->x) return fail(c, LP_ERR_STATE, "no particles bound (lp_bind_particles)");
     if (fields && !c->have_fields) return fail(c, LP_ERR_STATE, "fields not set (lp_set_fields)");
     return LP_OK;
+}
+
+lp_status not_with_energy_grid(lp_ctx *c, const char *what)
+{
+    if (c->eng) return fail(c, LP_ERR_UNSUPPORTED, std::string(what) + " does not move the per-particle energy grid (lp_bind_energy_grid is active)");
+    return LP_OK;
+}
+
+// spectral update on the per-particle moving grid (lp_moving.cu)
+lp_status do_moving(lp_ctx *c, double dt, cudaStream_t s)
+{
+    const lp_ctx::Set n = c->now();
+    const bool rec = c->timing && c->ev_used + 2 <= c->ev.size();
+    if (rec) LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used], s));
+    lp_status st = count(c, lp_launch_moving(c->geom, c->cells(), n.x, n.y, n.z, c->at<double>(c->lay.rho_old), c->eng, n.chi,
+                                             c->at<int32_t>(c->lay.nsub), c->nsub_user, c->cfg.np, c->cfg.nbins, dt,
+                                             c->cfg.kappa, c->cfg.u_rad, c->sm_count, s), "lp_moving_kernel launch");
+    if (rec) {
+        LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], s));
+        c->ev_used += 2;
+    }
+    if (st == LP_OK) {
+        c->spectra_done = true;
+        c->stage0_done = false; c->rk3_next = 0; c->push_done = false;
+    }
+    return st;
 }
 
 LpPushArgs push_args(lp_ctx *c, double dt)
@@ -400,9 +427,15 @@ lp_status do_sort(lp_ctx *c, bool in_place, SpectralIO *io, cudaStream_t s)
 {
     const long long np = c->cfg.np;
     if (np == 0) return LP_OK;
+    if (c->eng && !c->eng_scratch) return fail(c, LP_ERR_STATE, "a sort needs the eng_scratch array of lp_bind_energy_grid");
     uint32_t *perm = nullptr;
     lp_status st = sort_permutation(c, &perm, s);
     if (st != LP_OK) return st;
+    if (c->eng) {                       // the energy-grid rows follow their particles (through the scratch and back)
+        const int len = c->cfg.nbins + 1;
+        if ((st = count(c, lp_launch_permute_rows8(perm, c->eng, c->eng_scratch, np, len, s), "permute launch")) != LP_OK) return st;
+        LP_CUDA(c, cudaMemcpyAsync(c->eng, c->eng_scratch, (size_t)np * len * 8, cudaMemcpyDeviceToDevice, s));
+    }
     const lp_ctx::Set n = c->now();
     lp_ctx::Set o = c->other();
     if (!c->pingpong) {
@@ -632,6 +665,7 @@ lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
         return fail(ctx, LP_ERR_STATE, "lp_spectral_update needs the push finished (lp_push stage 1 / lp_push_rk3 stage 2)");
     if (ctx->cfg.np == 0) return LP_OK;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    if (ctx->eng) return do_moving(ctx, dt, static_cast<cudaStream_t>(stream));
     return do_spectral(ctx, dt, io_in_place(ctx), false, static_cast<cudaStream_t>(stream));
 }
 
@@ -639,6 +673,7 @@ lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void *stream
 {
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
+    if ((st = not_with_energy_grid(ctx, "lp_shock_update")) != LP_OK) return st;
     if (ctx->cfg.np == 0) return LP_OK;
     if (!r) return fail(ctx, LP_ERR_INVALID_ARG, "r is NULL");
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
@@ -650,6 +685,7 @@ lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *st
 {
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
+    if ((st = not_with_energy_grid(ctx, "lp_compact")) != LP_OK) return st;
     if (!np_new) return fail(ctx, LP_ERR_INVALID_ARG, "np_new is NULL");
     *np_new = ctx->cfg.np;
     if (ctx->cfg.np == 0) return LP_OK;
@@ -719,6 +755,7 @@ lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_t bytes
 {
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
+    if ((st = not_with_energy_grid(ctx, "lp_rebind")) != LP_OK) return st;
     if (capacity < ctx->cfg.np || capacity > 0xffffffffll) return fail(ctx, LP_ERR_INVALID_ARG, "capacity below the particle count or >= 2^32");
     if (capacity > 0 && (!x || !y || !z || !id || !chi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL particle array");
     if (reinterpret_cast<uintptr_t>(chi) % 16) return fail(ctx, LP_ERR_INVALID_ARG, "chi not 16-byte aligned");
@@ -806,6 +843,7 @@ lp_status lp_migrate_count(lp_ctx *ctx, int axis, double lo, double hi, int64_t 
 {
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
+    if ((st = not_with_energy_grid(ctx, "lp_migrate_count")) != LP_OK) return st;
     if (axis < 0 || axis > 2 || !n_left || !n_right || !(hi > lo)) return fail(ctx, LP_ERR_INVALID_ARG, "bad axis, interval or NULL output");
     ctx->mig_stage = 0;
     *n_left = *n_right = 0;
@@ -895,6 +933,27 @@ lp_status lp_migrate_unpack(lp_ctx *ctx, const void *from_left, int64_t n_from_l
     return LP_OK;
 }
 
+lp_status lp_bind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (!eng && eng_scratch) return fail(ctx, LP_ERR_INVALID_ARG, "eng_scratch without eng");
+    if (eng && ctx->cur != 0) return fail(ctx, LP_ERR_STATE, "bind the energy grid while the state is in the bound arrays");
+    ctx->eng = eng;
+    ctx->eng_scratch = eng_scratch;
+    ctx->spectra_done = false;
+    return LP_OK;
+}
+
+lp_status lp_init_energy_grid(lp_ctx *ctx, int64_t first, int64_t count_, void *stream)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (!ctx->eng) return fail(ctx, LP_ERR_STATE, "no energy grid bound (lp_bind_energy_grid)");
+    if (first < 0 || count_ < 0 || first + count_ > ctx->capacity) return fail(ctx, LP_ERR_INVALID_ARG, "rows outside the capacity");
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    return count(ctx, lp_launch_moving_init(ctx->tab, ctx->cfg.nbins, ctx->eng, first, count_, static_cast<cudaStream_t>(stream)),
+                 "lp_moving_init_kernel launch");
+}
+
 lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
 {
     lp_status st = need_ready(ctx, true);
@@ -904,6 +963,16 @@ lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const bool sort_now = ctx->cfg.sort_every > 0 && (ctx->steps - 1) % ctx->cfg.sort_every == 0;
+    if (ctx->eng) {
+        // moving energy grid: the staged kernels in a row (sort, push 0, push 1, moving-grid update)
+        if (sort_now && (st = do_sort(ctx, true, nullptr, s)) != LP_OK) return st;
+        LpPushArgs a = push_args(ctx, dt);
+        if ((st = count(ctx, lp_launch_push0(a, s), "lp_push0_kernel launch")) != LP_OK) return st;
+        if ((st = count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch")) != LP_OK) return st;
+        ctx->status_valid = true;
+        ctx->mig_stage = 0;
+        return do_moving(ctx, dt, s);
+    }
     SpectralIO io = io_in_place(ctx);
     bool flip = false;
     if (sort_now && ctx->pingpong) {
@@ -931,6 +1000,7 @@ lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *h
 {
     lp_status st = need_ready(ctx, true);
     if (st != LP_OK) return st;
+    if ((st = not_with_energy_grid(ctx, "lp_step_host")) != LP_OK) return st;
     if (ctx->cfg.np > 0 && (!hx || !hy || !hz || !hid || !hchi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL host array");
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -1026,8 +1096,8 @@ lp_status lp_get_diag(lp_ctx *ctx, lp_diag *out, void *stream)
     // before the first spectral update n_sub / lost / status hold no data: reduce chi only
     if (!have) LP_CUDA(ctx, cudaMemsetAsync(ctx->at<int32_t>(ctx->lay.nsub), 0, (size_t)ctx->cfg.np * 4, s));
     st = count(ctx, lp_launch_diag(ctx->at<int32_t>(ctx->lay.nsub),
-                                   (have && ctx->lost_user) ? ctx->at<double>(ctx->lay.lost) : nullptr,
-                                   ctx->status_valid ? ctx->at<int32_t>(ctx->lay.status) : nullptr, ctx->now().chi, ctx->tab,
+                                   (have && ctx->lost_user && !ctx->eng) ? ctx->at<double>(ctx->lay.lost) : nullptr,
+                                   ctx->status_valid ? ctx->at<int32_t>(ctx->lay.status) : nullptr, ctx->now().chi, ctx->eng, ctx->tab,
                                    ctx->cfg.nbins, ctx->cfg.np, ctx->at<double>(ctx->lay.partial), d, s),
                "lp_diag_kernel launch");
     if (st != LP_OK) return st;

@@ -150,6 +150,13 @@ int lp_launch_permute_rows(const uint32_t *perm, const double *src, double *dst,
                            int nbins, cudaStream_t s);
 int lp_launch_max_u64(const uint64_t *v, long long np, unsigned long long *out, cudaStream_t s);
 
+// moving energy grid (lp_moving.cu)
+int lp_launch_moving(const LpGeom &g, const LpCells &cells, const double *x, const double *y, const double *z,
+                     const double *rho_old, double *eng, double *chi, int32_t *nsub_ws, int32_t *nsub_user, long long np,
+                     int nbins, double dt, double kappa, double u_rad, int sm_count, cudaStream_t s);
+int lp_launch_moving_init(const double *tab, int nbins, double *eng, long long first, long long count, cudaStream_t s);
+int lp_launch_permute_rows8(const uint32_t *perm, const double *src, double *dst, long long np, int len, cudaStream_t s);
+
 // diagnostics reduction
 struct LpDiagDev {
     long long sum_substeps;
@@ -161,5 +168,5 @@ struct LpDiagDev {
     double lost;
 };
 int lp_launch_diag(const int32_t *nsub, const double *lost, const int32_t *status, const double *chi,
-                   const double *tab, int nbins, long long np, double *partial /*scratch*/,
+                   const double *eng /*[np][nbins+1] per-particle edges, or NULL: the table's widths*/, const double *tab, int nbins, long long np, double *partial /*scratch*/,
                    LpDiagDev *out, cudaStream_t s);

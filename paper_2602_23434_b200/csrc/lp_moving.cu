@@ -1,0 +1,223 @@
+// lp_moving.cu -- spectral update on a per-particle moving energy grid (NEXT-5; readings E1-E4 of DESIGN.md
+// section 3; the eng_ array of Listing 3; Eq. 6).
+//
+// Every particle carries its own N_b + 1 bin edges.  Over a step they follow the characteristics of Eq. 6,
+//   eps' = alpha eps / (1 + beta eps),   alpha = e^{-s},  s = a dtau,  beta = c_r dtau (1 - e^{-s}) / s,
+// and every bin keeps its number: chi_i' = chi_i dE_i / dE_i'.  With t_k = 1 + beta eps_k the new width is
+// dE_i' = alpha dE_i / (t_i t_{i+1}) exactly, so chi_i' = chi_i t_i t_{i+1} / alpha -- no subtraction of nearly
+// equal edges and one division per edge instead of two per bin.  No CFL limit and no substeps: the kernel is a
+// pure stream of 16 (2 N_b + 1) bytes per particle behind a per-particle phase (gather, coefficients) that is
+// the same as the fixed-grid kernel's (lp_spectral.cu).
+//
+// A block takes 128 particles at a time: phase 1 with one thread per particle leaves (alpha, beta) in shared
+// memory, then its four warps stream the 128 rows, RI rows per warp in flight.  Several blocks are resident
+// per SM, so the latency-bound phase of one overlaps the stream of the others.  sm_100a.
+#include "lp_device.cuh"
+
+namespace {
+
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kThreads = 128;
+constexpr int kWarps = kThreads / 32;
+
+struct LpMovingArgs {
+    LpGeom g;
+    LpCells cells;
+    const double *x, *y, *z;     // x^{n+1}
+    const double *rho_old;       // from push stage 0
+    double *eng;                 // [np][nbins + 1] in/out
+    double *chi;                 // [np][nbins] in/out
+    int32_t *nsub_ws;            // [np]: 1 (one exact step per particle)
+    int32_t *nsub_user;          // or NULL
+    long long np;
+    double dt, kappa, u_rad;
+};
+
+// per-particle phase: (alpha, beta) of the step  (a7 of DESIGN.md section 1, then reading E2)
+__device__ __forceinline__ double2 lp_moving_coef(const LpMovingArgs &A, long long p)
+{
+    const double px = A.x[p], py = A.y[p], pz = A.z[p];
+    LpStencil st;
+    lp_stencil(A.g, px, py, pz, st);
+    double qa[4], qb[3];
+    {
+        LpCornersA ka;
+        ka.load(A.cells, st);
+        ka.gather4(st, qa);
+    }
+    {
+        LpCornersB kb;
+        kb.load(A.cells, st);
+        kb.gather3(st, qb);
+    }
+    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(qa[0], qa[0]), __dmul_rn(qa[1], qa[1])), __dmul_rn(qa[2], qa[2]));
+    const double b2 = __dadd_rn(__dadd_rn(__dmul_rn(qb[0], qb[0]), __dmul_rn(qb[1], qb[1])), __dmul_rn(qb[2], qb[2]));
+    const double gam = __ddiv_rn(1.0, __dsqrt_rn(__dsub_rn(1.0, v2)));
+    const double dtau = __ddiv_rn(A.dt, gam);
+    const double cr = __dmul_rn(A.kappa, __dadd_rn(__dmul_rn(0.5, b2), A.u_rad));
+    const double a = __ddiv_rn(-log(__ddiv_rn(qa[3], A.rho_old[p])), __dmul_rn(3.0, dtau));
+    const double s = __dmul_rn(a, dtau);
+    const double alpha = exp(-s);
+    const double crt = __dmul_rn(cr, dtau);
+    const double beta = (s != 0.0) ? __dmul_rn(crt, __ddiv_rn(-expm1(-s), s)) : crt;
+    return make_double2(alpha, beta);
+}
+
+template <int NB>
+__global__ void __launch_bounds__(kThreads) lp_moving_kernel(LpMovingArgs A)
+{
+    constexpr int G = NB < 32 ? NB : 32;         // lanes per row
+    constexpr int PPW = 32 / G;                  // rows a warp holds side by side
+    constexpr int M = NB / G;                    // bins per lane: bin sub + G j
+    constexpr int RI = M <= 2 ? 4 : (M == 4 ? 2 : 1);      // row sets in flight per warp
+    constexpr int ROWS = PPW * RI;               // rows per warp trip
+    static_assert(32 % ROWS == 0 || ROWS <= 32, "rows per trip");
+
+    __shared__ double2 sAB[kThreads];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sub = lane % G, grp = lane / G;
+    const long long ngroups = (A.np + kThreads - 1) / kThreads;
+
+    for (long long gidx = blockIdx.x; gidx < ngroups; gidx += gridDim.x) {
+        const long long base = gidx * kThreads;
+        {
+            const long long p = base + threadIdx.x;
+            double2 ab = make_double2(1.0, 0.0);
+            if (p < A.np) {
+                ab = lp_moving_coef(A, p);
+                __stcs(A.nsub_ws + p, 1);
+                if (A.nsub_user) __stcs(A.nsub_user + p, 1);
+            }
+            sAB[threadIdx.x] = ab;
+        }
+        __syncthreads();
+        // rows of this warp: base + warp*32 + [0, 32)
+        for (int r0 = 0; r0 < 32; r0 += ROWS) {
+            double e[RI][M], en[RI], c[RI][M];
+            double2 ab[RI];
+            long long row[RI];
+            bool have[RI];
+#pragma unroll
+            for (int u = 0; u < RI; ++u) {
+                const int rl = warp * 32 + r0 + u * PPW + grp;          // row within the block's 128
+                row[u] = base + rl;
+                have[u] = row[u] < A.np;
+                ab[u] = sAB[rl];
+                const double *er = A.eng + row[u] * (NB + 1);
+                const double *cp = A.chi + row[u] * NB;
+#pragma unroll
+                for (int j = 0; j < M; ++j) {
+                    e[u][j] = have[u] ? __ldcs(er + sub + G * j) : 1.0;
+                    c[u][j] = have[u] ? __ldcs(cp + sub + G * j) : 0.0;
+                }
+                en[u] = have[u] ? __ldcs(er + NB) : 1.0;               // the top edge (same address in the group)
+            }
+#pragma unroll
+            for (int u = 0; u < RI; ++u) {
+                const double alpha = ab[u].x, beta = ab[u].y;
+                const double ralpha = 1.0 / alpha;
+                double t[M], tn;
+#pragma unroll
+                for (int j = 0; j < M; ++j) t[j] = fma(beta, e[u][j], 1.0);
+                tn = fma(beta, en[u], 1.0);
+                double *er = A.eng + row[u] * (NB + 1);
+                double *cp = A.chi + row[u] * NB;
+#pragma unroll
+                for (int j = 0; j < M; ++j) {
+                    // t of the next edge: the next lane's, or (last lane of the group) the group's first lane
+                    // one round further on, or the top edge
+                    const double from_next = __shfl_down_sync(kFull, t[j], 1, G);
+                    const double wrap = (j + 1 < M) ? __shfl_sync(kFull, t[(j + 1 < M) ? j + 1 : j], 0, G) : tn;
+                    const double t_up = (sub == G - 1) ? wrap : from_next;
+                    if (have[u]) {
+                        __stcs(er + sub + G * j, alpha * e[u][j] / t[j]);
+                        __stcs(cp + sub + G * j, c[u][j] * (t[j] * t_up) * ralpha);
+                    }
+                }
+                if (have[u] && sub == 0) __stcs(er + NB, alpha * en[u] / tn);
+            }
+        }
+        __syncthreads();                       // sAB is rewritten by the next group
+    }
+}
+
+// eng rows [first, first + count) <- the fixed table's edges (reading E4)
+__global__ void __launch_bounds__(256)
+lp_moving_init_kernel(const double *__restrict__ tab, int nbins, double *__restrict__ eng, long long first, long long count)
+{
+    const long long n = count * (nbins + 1);
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        eng[first * (nbins + 1) + i] = tab[i % (nbins + 1)];
+}
+
+// rows of `len` doubles through a permutation (rows may be 8-byte aligned only): a warp per row
+__global__ void __launch_bounds__(256)
+lp_permute_rows8_kernel(const uint32_t *__restrict__ perm, const double *__restrict__ src, double *__restrict__ dst,
+                        long long np, int len)
+{
+    const int lane = threadIdx.x & 31;
+    const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long r = gw; r < np; r += nw) {
+        const double *s = src + (long long)perm[r] * len;
+        double *d = dst + r * len;
+        for (int i = lane; i < len; i += 32) __stcs(d + i, __ldcs(s + i));
+    }
+}
+
+template <int NB>
+int launch(const LpMovingArgs &a, int sm_count, cudaStream_t s)
+{
+    int per_sm = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_moving_kernel<NB>, kThreads, 0);
+    if (per_sm < 1) per_sm = 1;
+    const long long want = (a.np + kThreads - 1) / kThreads;
+    const long long cap = (long long)sm_count * per_sm;
+    int blocks = (int)(want < cap ? want : cap);
+    if (blocks < 1) blocks = 1;
+    lp_moving_kernel<NB><<<blocks, kThreads, 0, s>>>(a);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace
+
+int lp_launch_moving(const LpGeom &g, const LpCells &cells, const double *x, const double *y, const double *z,
+                     const double *rho_old, double *eng, double *chi, int32_t *nsub_ws, int32_t *nsub_user, long long np,
+                     int nbins, double dt, double kappa, double u_rad, int sm_count, cudaStream_t s)
+{
+    LpMovingArgs a;
+    a.g = g; a.cells = cells;
+    a.x = x; a.y = y; a.z = z;
+    a.rho_old = rho_old;
+    a.eng = eng; a.chi = chi;
+    a.nsub_ws = nsub_ws; a.nsub_user = nsub_user;
+    a.np = np;
+    a.dt = dt; a.kappa = kappa; a.u_rad = u_rad;
+    switch (nbins) {
+    case 16:  return launch<16>(a, sm_count, s);
+    case 32:  return launch<32>(a, sm_count, s);
+    case 64:  return launch<64>(a, sm_count, s);
+    case 128: return launch<128>(a, sm_count, s);
+    case 256: return launch<256>(a, sm_count, s);
+    case 512: return launch<512>(a, sm_count, s);
+    default:  return -1;
+    }
+}
+
+int lp_launch_moving_init(const double *tab, int nbins, double *eng, long long first, long long count, cudaStream_t s)
+{
+    if (count <= 0) return 0;
+    long long blocks = (count * (nbins + 1) + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    lp_moving_init_kernel<<<(int)blocks, 256, 0, s>>>(tab, nbins, eng, first, count);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+int lp_launch_permute_rows8(const uint32_t *perm, const double *src, double *dst, long long np, int len, cudaStream_t s)
+{
+    long long blocks = (np + 7) / 8;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks < 1) blocks = 1;
+    lp_permute_rows8_kernel<<<(int)blocks, 256, 0, s>>>(perm, src, dst, np, len);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}

@@ -352,8 +352,8 @@ lp_max_u64_kernel(const uint64_t *__restrict__ v, long long np, unsigned long lo
 __global__ void __launch_bounds__(kThreads)
 lp_diag_kernel(const int32_t *__restrict__ nsub, const double *__restrict__ lost,
                const int32_t *__restrict__ status, const double *__restrict__ chi,
-               const double *__restrict__ tab, int nbins, long long np, double *__restrict__ partial,
-               LpDiagDev *out)
+               const double *__restrict__ eng, const double *__restrict__ tab, int nbins, long long np,
+               double *__restrict__ partial, LpDiagDev *out)
 {
     __shared__ double snum[kWarps], slost[kWarps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -375,11 +375,16 @@ lp_diag_kernel(const int32_t *__restrict__ nsub, const double *__restrict__ lost
     for (long long r = gw; r < np; r += 4 * nw) {
         for (int i = lane; i < nbins; i += 32) {
             const double w = dE[i];
-            double v[4];
+            double v[4], wk[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) v[k] = (r + k * nw < np) ? chi[(r + k * nw) * nbins + i] : 0.0;
+            for (int k = 0; k < 4; ++k) {
+                const long long rr = r + k * nw;
+                v[k] = (rr < np) ? chi[rr * nbins + i] : 0.0;
+                // moving grid: the particle's own bin widths
+                wk[k] = (eng && rr < np) ? eng[rr * (nbins + 1) + i + 1] - eng[rr * (nbins + 1) + i] : w;
+            }
 #pragma unroll
-            for (int k = 0; k < 4; ++k) num = fma(v[k], w, num);
+            for (int k = 0; k < 4; ++k) num = fma(v[k], wk[k], num);
         }
     }
 #pragma unroll
@@ -520,10 +525,11 @@ int lp_launch_max_u64(const uint64_t *v, long long np, unsigned long long *out, 
 }
 
 int lp_launch_diag(const int32_t *nsub, const double *lost, const int32_t *status, const double *chi,
-                   const double *tab, int nbins, long long np, double *partial, LpDiagDev *out, cudaStream_t s)
+                   const double *eng, const double *tab, int nbins, long long np, double *partial, LpDiagDev *out,
+                   cudaStream_t s)
 {
     const int blocks = 296;      // (the scratch `partial` holds 2 x 296 doubles)
-    lp_diag_kernel<<<blocks, kThreads, 0, s>>>(nsub, lost, status, chi, tab, nbins, np, partial, out);
+    lp_diag_kernel<<<blocks, kThreads, 0, s>>>(nsub, lost, status, chi, eng, tab, nbins, np, partial, out);
     lp_diag_final_kernel<<<1, 1, 0, s>>>(partial, blocks, out);
     return ok() ? 2 : -1;
 }

@@ -130,6 +130,22 @@ class LP:
         B.lp_set_count(self.ctx, n)
         self.cfg.np = n            # (the binding's copy of the count sizes the outputs of interpolate)
 
+    # ---- per-particle moving energy grid (Listing 3's eng_; readings E1-E4 of DESIGN.md)
+    def bind_energy_grid(self, init=True, sortable=True):
+        """Switch to the moving energy grid: allocates eng [capacity][nbins+1] (and the scratch a sort needs),
+        starts every particle on the fixed table's edges."""
+        shape = (self.capacity, self.cfg.nbins + 1)
+        self.eng = torch.empty(shape, dtype=torch.float64, device=self.device)
+        self._eng_scratch = torch.empty(shape, dtype=torch.float64, device=self.device) if sortable else None
+        B.lp_bind_energy_grid(self.ctx, self.eng.data_ptr(), self._eng_scratch.data_ptr() if sortable else None)
+        if init:
+            B.lp_init_energy_grid(self.ctx, 0, self.capacity, self.stream)
+        return self.eng
+
+    def unbind_energy_grid(self):
+        B.lp_bind_energy_grid(self.ctx, None, None)
+        self.eng = self._eng_scratch = None
+
     # ---- chunked growth (PAPER.md:176-184 Listing 1; Reserve() / Shrink() of Listing 2)
     def _rebind(self, capacity):
         n, nb = self.cfg.np, self.cfg.nbins

@@ -1,0 +1,125 @@
+"""GPU parity of the per-particle moving energy grid (lp_bind_energy_grid, lp_moving.cu; NEXT-5, readings E1-E4)
+against oracle/orc_moving_update: edges and spectra elementwise within 1e-10 relative (positions bit for bit),
+at all six bin counts, staged and through lp_step with re-sorts, plus the two laws north_star names."""
+import numpy as np
+import pytest
+import torch
+
+import lp_inputs as I
+import paper_2602_23434_b200 as P
+from oracle import lp_oracle as orc
+from lp_testlib import assert_chi_close, fields_to_numpy, oracle_params, u_rad_of
+
+pytestmark = pytest.mark.gpu
+B = P.binding
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def setup(w, pingpong=False):
+    fields = I.make_fields(w, device="cpu")
+    u_rad = u_rad_of(w, fields)
+    x, y, z, pid = I.make_particles(w, shuffle_ids=True)
+    chi = I.make_spectrum(w)
+    lp = P.LP(P.config_from_workload(w, u_rad=u_rad))
+    lp.set_fields(fields)
+    lp.bind_particles(x, y, z, pid, chi)
+    lp.bind_diag(nsub=True, lost=False)
+    lp.bind_energy_grid()
+    if pingpong:
+        lp.set_pingpong(True)
+    E, dE, Ec = orc.bin_table(w.nbins, w.e_min, w.e_max)
+    return lp, oracle_params(w, u_rad), fields_to_numpy(fields), [x, y, z, pid, chi, np.tile(E, (w.np, 1))]
+
+
+def oracle_step(prm, f_np, st, dt, sort):
+    x, y, z, pid, chi, eng = st
+    if sort:
+        perm = orc.sort_perm(orc.cell_key(prm, x, y, z), pid)
+        x, y, z, pid, chi, eng = x[perm], y[perm], z[perm], pid[perm], chi[perm], eng[perm]
+    k1, rho_old, xs = orc.push_stage0(prm, f_np, x, y, z, dt, nthreads=8)
+    x, y, z, status = orc.push_stage1(prm, f_np, x, y, z, xs, k1, dt, nthreads=8)
+    eng, chi = orc.moving_update(prm, f_np, x, y, z, rho_old, dt, eng, chi, nthreads=8)
+    return [x, y, z, pid, chi, eng]
+
+
+def check(lp, st):
+    n = st[0].shape[0]
+    assert np.array_equal(host(lp.id)[:n].view(np.uint64), st[3])
+    for g, w in zip((lp.x, lp.y, lp.z), st[:3]):
+        assert np.array_equal(host(g)[:n], w)
+    assert_chi_close(host(lp.eng)[:n], st[5], what="eng")
+    assert_chi_close(host(lp.chi)[:n], st[4])
+    assert (host(lp.nsub)[:n] == 1).all()
+
+
+@pytest.mark.parametrize("nbins,np_", [(16, 3000 + 5), (32, 2000 + 31), (64, 4097), (128, 1500), (256, 777), (512, 300 + 33)])
+def test_moving_grid_staged_matches_oracle(nbins, np_):
+    w = I.workload(3).scaled(n=12, np=np_, nbins=nbins, sort_every=0)
+    lp, prm, f_np, st = setup(w)
+    for _ in range(3):
+        lp.push(w.dt, 0)
+        lp.push(w.dt, 1)
+        lp.spectral_update(w.dt)
+        st = oracle_step(prm, f_np, st, w.dt, False)
+    check(lp, st)
+    d = lp.diag()
+    want = float(np.sum(st[4] * np.diff(st[5], axis=1)))
+    assert abs(d["number"] - want) <= 1e-12 * abs(want) and d["max_substeps"] == 1
+    # every bin keeps its number (E3): compare with the initial spectrum on the fixed table
+    E, dE, Ec = orc.bin_table(w.nbins, w.e_min, w.e_max)
+    chi0 = I.make_spectrum(w)
+    pid0 = I.make_particles(w, shuffle_ids=True)[3]
+    order = np.argsort(pid0); back = np.argsort(st[3])
+    n_now = (host(lp.chi) * np.diff(host(lp.eng), axis=1))[back]
+    assert np.allclose(n_now, (chi0 * dE[None, :])[order], rtol=1e-11, atol=0)
+
+
+@pytest.mark.parametrize("pingpong", [False, True])
+@pytest.mark.parametrize("nbins,np_", [(64, 6000 + 3), (16, 2500), (256, 999)])
+def test_moving_grid_lp_step_with_resort(nbins, np_, pingpong):
+    w = I.workload(3).scaled(n=12, np=np_, nbins=nbins, sort_every=2)
+    lp, prm, f_np, st = setup(w, pingpong)
+    for k in range(5):
+        lp.step(w.dt)
+        st = oracle_step(prm, f_np, st, w.dt, k % 2 == 0)
+    check(lp, st)
+    lp.sort()
+    perm = orc.sort_perm(orc.cell_key(prm, *st[:3]), st[3])
+    check(lp, [a[perm] for a in st])
+
+
+def test_moving_grid_synchrotron_law_and_unsupported_calls():
+    """Workload 1 (uniform B, v = 0): after 100 lp_step every edge is E0 / (1 + c_r E0 t) (north_star)."""
+    w = I.workload(1)
+    E = I.bin_edges(w.nbins, w.e_min, w.e_max)
+    cr = w.kappa * 0.5 * w.b0 ** 2
+    dt = 0.9 * w.cfl_e / (cr * E[-2] ** 2 / (E[-1] - E[-2]))
+    lp, prm, f_np, st = setup(w)
+    for _ in range(100):
+        lp.step(dt)
+    eng = host(lp.eng)
+    assert np.allclose(eng, (E / (1.0 + cr * E * dt * 100))[None, :], rtol=1e-12, atol=0)
+    with pytest.raises(B.LPError) as e:
+        lp.compact(torch.zeros(w.np, dtype=torch.int32, device=lp.device))
+    assert e.value.status == B.LP_ERR_UNSUPPORTED
+    with pytest.raises(B.LPError):
+        lp.migrate_count(0, -1.0, 0.0)
+    lp.unbind_energy_grid()
+    lp.step(dt)                                  # back on the fixed bins
+    assert lp.diag()["max_substeps"] >= 1
+
+
+def test_sort_without_scratch_is_refused():
+    w = I.workload(3).scaled(n=8, np=500, nbins=32, sort_every=0)
+    fields = I.make_fields(w, device="cpu")
+    x, y, z, pid = I.make_particles(w)
+    lp = P.LP(P.config_from_workload(w, u_rad=0.0))
+    lp.set_fields(fields)
+    lp.bind_particles(x, y, z, pid, I.make_spectrum(w))
+    lp.bind_energy_grid(sortable=False)
+    with pytest.raises(B.LPError) as e:
+        lp.sort()
+    assert e.value.status == B.LP_ERR_STATE
