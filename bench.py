@@ -44,6 +44,9 @@ def parse():
                     help="also time lp_shock_update (Eq. 7-8) with this fraction of particles flagged")
     ap.add_argument("--compact-frac", type=float, default=0.0,
                     help="at the very end, time one lp_compact (PAPER.md:190-199) deleting this fraction of particles")
+    ap.add_argument("--migrate-frac", type=float, default=0.0,
+                    help="at the end, time one directional particle exchange (lp_migrate_count/_pack/_unpack, "
+                         "PAPER.md:201-214) in which this fraction of the particles leaves through the two x faces")
     ap.add_argument("--pusher", default="rk2", choices=["rk2", "rk3"],
                     help="with --staged: the two-stage pusher (lp_push) or the three-stage one (lp_push_rk3)")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -55,6 +58,8 @@ def parse():
     ap.add_argument("--no-pingpong", action="store_true",
                     help="keep the state in the bound arrays across re-sorts (permute pass + copies) instead of "
                          "lp_set_pingpong (re-sort folded into the fused kernel)")
+    ap.add_argument("--energy-grid", action="store_true",
+                    help="per-particle moving energy grid (lp_bind_energy_grid, NEXT-5) instead of the fixed bins")
     ap.add_argument("--no-parity", action="store_true", help="skip the oracle check of the timed state")
     ap.add_argument("--parity-sample", type=int, default=2048)
     return ap.parse_args()
@@ -144,11 +149,12 @@ def step_dt(w):
     return 0.9 * w.cfl_e / lam_top
 
 
-def config_dict(w, n_gpus, staged=False, pingpong=False):
+def config_dict(w, n_gpus, staged=False, pingpong=False, moving=False):
     return {"workload": "BASELINE.json configs[%d] %s" % (w.index - 1, w.name), "grid": "%d^3" % w.n,
             "particles_per_gpu": w.np, "nbins": w.nbins, "sort_every": w.sort_every,
             "parallelism": "replicas x%d (particles independent, no collective)" % n_gpus,
             "api": ("staged %s, lp_spectral_update" % staged) if staged else "fused lp_step",
+            "energy_grid": "per-particle moving grid (lp_bind_energy_grid)" if moving else "fixed log-spaced bins",
             "resort": "ping-pong buffers (lp_set_pingpong)" if pingpong else "bound arrays (permute + copy back)",
             "l2": "inputs larger than L2 (chi rows %.2f GB per GPU)" % (w.np * w.nbins * 8 / 1e9)}
 
@@ -232,7 +238,7 @@ def cpu_baseline(w, fields_np, u_rad, x, y, z, pid, chi_host_fn, dt, seconds):
     return out
 
 
-def parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_rows_fn, dt, nsteps, nsample, dev):
+def parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_rows_fn, dt, nsteps, nsample, dev, moving=False):
     """The timed state against the oracle: a seeded sample of particles is replayed on the CPU for the
     `nsteps` steps the GPU state has taken and compared by id (positions bit for bit, spectra relative).
     fields_for_step(k) -> (fields at t^n, fields at t^{n+1}) as numpy, the same object twice when frozen."""
@@ -244,9 +250,14 @@ def parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_rows_fn, dt, n
     sel = np.sort(np.random.default_rng(4321).choice(w.np, size=min(nsample, w.np), replace=False))
     sx, sy, sz, sid, schi = x[sel].copy(), y[sel].copy(), z[sel].copy(), pid[sel].copy(), chi_rows_fn(sel)
     nt = os.cpu_count() or 1
+    seng = np.tile(orc.bin_table(w.nbins, w.e_min, w.e_max)[0], (sel.size, 1)) if moving else None
     for k in range(nsteps):
         f0, f1 = fields_for_step(k)
-        if f0 is f1:
+        if moving:
+            k1, rho_old, xs = orc.push_stage0(prm, f0, sx, sy, sz, dt, nthreads=nt)
+            sx, sy, sz, status = orc.push_stage1(prm, f1, sx, sy, sz, xs, k1, dt, nthreads=nt)
+            seng, schi = orc.moving_update(prm, f1, sx, sy, sz, rho_old, dt, seng, schi, nthreads=nt)
+        elif f0 is f1:
             sx, sy, sz, schi, nsub, lost, status = orc.step(prm, f0, sx, sy, sz, dt, schi, nthreads=nt)
         else:
             k1, rho_old, xs = orc.push_stage0(prm, f0, sx, sy, sz, dt, nthreads=nt)
@@ -259,6 +270,9 @@ def parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_rows_fn, dt, n
     gx, gy, gz = (t[loc].cpu().numpy() for t in (cx, cy, cz))
     gchi = cchi[loc].cpu().numpy()
     rel = np.abs(gchi - schi) / np.maximum(np.abs(schi), 1e-290)
+    if moving:
+        geng = lp.eng[loc].cpu().numpy()
+        rel = np.maximum(rel.max(), (np.abs(geng - seng) / np.abs(seng)).max())
     return {"particles": int(sel.size), "steps": int(nsteps), "max_rel": float(rel.max()),
             "positions_bit_exact": bool(np.array_equal(gx, sx) and np.array_equal(gy, sy) and np.array_equal(gz, sz)),
             "tolerance": 1e-10, "ok": bool(rel.max() <= 1e-10 and np.array_equal(gx, sx)),
@@ -349,6 +363,8 @@ def run_ours(args):
     lp.set_fields(fields)
     lp.bind_particles(x, y, z, pid, chi_device())
     lp.set_pingpong(not args.no_pingpong)
+    if args.energy_grid:
+        lp.bind_energy_grid()
     B = P.binding
     total_steps = args.warmup + args.steps * max(1, args.repeats)
     field_at = None
@@ -422,7 +438,7 @@ def run_ours(args):
         else:
             fields_for_step = lambda k: tuple([f.cpu().numpy() for f in field_at(k + j)] for j in (0, 1))
         parity = parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_host.rows, dt, nstep[0],
-                              args.parity_sample, dev)
+                              args.parity_sample, dev, moving=args.energy_grid)
 
     # ---- further passes of the same K steps: median of all (SURVEY.md 8(d) "median of 5 repeats")
     passes = [(ms, spec_ms, spec_n)]
@@ -464,7 +480,7 @@ def run_ours(args):
 
     # ---- end to end through lp_step_host: pinned host buffers, H2D + D2H every step
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.energy_grid:
         hx, hy, hz = (t.cpu().pin_memory() for t in (lp.x, lp.y, lp.z))
         hid = lp.id.cpu().pin_memory()
         hchi = lp.chi.cpu().pin_memory()
@@ -482,6 +498,29 @@ def run_ours(args):
                "steps": args.e2e_steps,
                "api": "lp_step_host (pinned host x,y,z,id,chi in and out every step)"}
         del hx, hy, hz, hid, hchi
+
+    # ---- particle exchange (NEXT-3): this rank owns x in [xlo + d, xhi - d) of the periodic box; the leavers of
+    # each face come back in through the other one (what the neighbour would send), so the count is unchanged
+    migrate = None
+    if args.migrate_frac > 0 and not args.energy_grid:
+        L = w.xhi[0] - w.xlo[0]
+        dlt = 0.5 * args.migrate_frac * L
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        torch.cuda.synchronize(dev)
+        ev[0].record()
+        nl, nr = lp.migrate_count(0, w.xlo[0] + dlt, w.xhi[0] - dlt)
+        ev[1].record()
+        bl, br = lp.migrate_pack(nl, nr)
+        ev[2].record()
+        n_after = lp.migrate_unpack(br, nr, bl, nl)
+        ev[3].record()
+        torch.cuda.synchronize(dev)
+        rec = 32 + 8 * w.nbins
+        mbytes = w.np * (8 + 4 + 4) + (nl + nr) * (4 + 4 + 4 * rec)      # classify; lists; rows out, in, out, in
+        mms = [ev[i].elapsed_time(ev[i + 1]) for i in range(3)]
+        migrate = {"left": nl, "right": nr, "np_after": n_after, "count_ms": mms[0], "pack_ms": mms[1], "unpack_ms": mms[2],
+                   "algorithmic_bytes": mbytes, "achieved_gbs": mbytes / (sum(mms) * 1e-3) / 1e9,
+                   "leavers_per_s": (nl + nr) / (sum(mms) * 1e-3)}
 
     # ---- deletion with hole filling (NEXT-2): one call at the end (it shrinks the particle set)
     compact = None
@@ -512,11 +551,16 @@ def run_ours(args):
     #         min(cells, 8 corners x particles) -- the three gathers of the fused kernel share their cells.
     rows_bytes = 16 * w.nbins * w.np
     state_bytes = (32 if staged else 48) * w.np
+    if args.energy_grid:        # moving grid: chi and the N_b + 1 edges in and out; x, y, z, rho_old in
+        rows_bytes = 16 * (2 * w.nbins + 1) * w.np
+        state_bytes = 32 * w.np
     grid_bytes = 56 * min(w.n ** 3, 8 * w.np)
     alg_bytes = rows_bytes + state_bytes + grid_bytes
     spec_avg_ms = spec_ms / max(spec_n, 1)
     achieved = alg_bytes / (spec_avg_ms * 1e-3) / 1e9 if spec_n else None
     kname = "lp_spectral_%s_kernel<%d,0,%d>" % ("bulk" if w.nbins <= 256 else "direct", w.nbins, 0 if staged else 1)
+    if args.energy_grid:
+        kname = "lp_moving_kernel<%d>" % w.nbins
     # The secondary bound ("report both fractions"): fp64 arithmetic.  Algorithmic flops of a row:
     # per bin and substep the donor-cell update is 3 multiply-adds (6 flop), plus 12 flop per bin once for the
     # edge velocities and the update coefficients; the substep total is the kernel's own count (lp_get_diag).
@@ -525,6 +569,8 @@ def run_ours(args):
     try:
         alu_peak = B.lp_measure_fp64_peak(local)
         flops = 6.0 * w.nbins * d["sum_substeps"] + 12.0 * w.nbins * w.np
+        if args.energy_grid:    # per bin: t = 1 + beta e, e' = alpha e / t (a division ~ 10 flop), chi' = chi t t_up / alpha
+            flops = 16.0 * w.nbins * w.np
         alu_ach = flops / (spec_avg_ms * 1e-3) / 1e12 if spec_n else None
         alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s (fp64)",
                "frac": (alu_ach / alu_peak) if alu_ach else None,
@@ -535,7 +581,8 @@ def run_ours(args):
         alu = {"error": str(e)}
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
-                "traffic": stored_traffic(w.name, w.nbins, staged), "peak_source": peak_src,
+                "traffic": stored_traffic(w.name, w.nbins, staged) if not args.energy_grid
+                else stored_traffic(w.name + "/moving", w.nbins), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "algorithmic_bytes_split": {"rows": rows_bytes, "state": state_bytes, "grid": grid_bytes},
                 "achieved_rows_only": (rows_bytes / (spec_avg_ms * 1e-3) / 1e9) if spec_n else None,
@@ -551,13 +598,15 @@ def run_ours(args):
             api = "lp_set_fields(t^n), lp_push(0), lp_set_fields(t^n+1), lp_push(1)"
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, api, not args.no_pingpong),
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, world, api, not args.no_pingpong, args.energy_grid),
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
            "parity_checked": parity, "repeats": repeats,
            "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],
                     "sorts_total": d["sorts"]}}
     if compact is not None:
         out["compact"] = compact
+    if migrate is not None:
+        out["migrate"] = migrate
     if shock is not None:
         peak_s, _ = measured_peak()
         shock["frac_of_measured_peak"] = shock["achieved_gbs"] / peak_s
