@@ -157,7 +157,7 @@ struct lp_ctx {
     bool status_valid = false;             // the status array describes the bound particles in their current order
     bool push_done = false;                // a pusher ran to its last stage since stage 0 (x^{n+1} is in place)
     bool id_bits_stale = true;             // ids may have changed since id_bits was measured (bind, injection, host copy)
-    int spectral_blocks[4] = { 0, 0, 0, 0 };   // resident blocks per SM of the spectral kernel variants [diag][fused], 0 = not set up
+    int spectral_blocks[6] = { 0, 0, 0, 0, 0, 0 };   // resident blocks per SM of the spectral kernel variants [diag][mode], 0 = not set up
     long long capacity = 0;                // particles the workspace was sized for (cfg.np shrinks in lp_compact)
     int id_bits = 0, key_bits = 0;
     long long launches = 0, steps = 0, sorts = 0;

@@ -92,7 +92,8 @@ int lp_launch_push0(const LpPushArgs &a, cudaStream_t s);
 int lp_launch_push1(const LpPushArgs &a, cudaStream_t s);
 int lp_launch_push_rk3(const LpPushArgs &a, int stage, cudaStream_t s);     // stage 0, 1, 2 (x0 kept in a.xs)
 // fused = true: the kernel also does both push stages (a5, a6) in its per-particle phase (frozen fields)
-// blocks_cache: int[4] owned by the context, [diag][fused] resident blocks per SM (0 = variant not set up yet)
+// blocks_cache: int[6] owned by the context, [diag][mode: staged, fused, fused + re-sort] resident blocks per SM
+// (0 = variant not set up yet)
 int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, bool fused, int sm_count, int *blocks_cache,
                        cudaStream_t s);
 

@@ -164,7 +164,7 @@ __device__ __forceinline__ void lp_store_row(double *__restrict__ dst, const dou
 // are stored lane-interleaved (entry i of lane `sub` at [i*32 + sub]): a straight copy of the table would
 // put the lanes' slices M*8 bytes apart, i.e. all in the same banks (measured at M = 16: the kernel was
 // bound by these 32-way conflicts, l1tex at 94 %).
-template <int M, bool IN_REGS>
+template <int M, bool IN_REGS, int LANES = 32>
 struct LpLaneTab {
     double rE[IN_REGS ? M + 1 : 1], rR[IN_REGS ? M : 1];
     const double *pE, *pR;
@@ -182,21 +182,22 @@ struct LpLaneTab {
             pR = sR + sub;
         }
     }
-    __device__ __forceinline__ double E(int i) const { return IN_REGS ? rE[i] : pE[i * 32]; }
-    __device__ __forceinline__ double R(int i) const { return IN_REGS ? rR[i] : pR[i * 32]; }
+    __device__ __forceinline__ double E(int i) const { return IN_REGS ? rE[i] : pE[i * LANES]; }
+    __device__ __forceinline__ double R(int i) const { return IN_REGS ? rR[i] : pR[i * LANES]; }
 };
 
-// lane-interleaved copies of the bin table for LpLaneTab<M, false>: tE[(M+1)*32], tR[M*32]
-template <int M>
+// lane-interleaved copies of the bin table for LpLaneTab<M, false, LANES>: tE[(M+1)*LANES], tR[M*LANES]
+// (LANES lanes share a row: 32, or 64 when a pair of warps does)
+template <int M, int LANES = 32>
 __device__ __forceinline__ void lp_fill_interleaved(const double *tab, int nb, double *tE, double *tR, int tid, int nthreads)
 {
-    for (int k = tid; k < (M + 1) * 32; k += nthreads) {
-        const int i = k >> 5, lane = k & 31;
+    for (int k = tid; k < (M + 1) * LANES; k += nthreads) {
+        const int i = k / LANES, lane = k % LANES;
         const int e = lane * M + i;
         tE[k] = e <= nb ? tab[e] : 0.0;
     }
-    for (int k = tid; k < M * 32; k += nthreads) {
-        const int i = k >> 5, lane = k & 31;
+    for (int k = tid; k < M * LANES; k += nthreads) {
+        const int i = k / LANES, lane = k % LANES;
         const int b = lane * M + i;
         tR[k] = b < nb ? tab[(nb + 1) + nb + b] : 0.0;
     }
@@ -220,8 +221,9 @@ struct LpRow {
     double w_first, w_last, s0, s1;
     int ns;
 
+    // first / last: this lane holds the first / the last bin of the row
     template <class Tab>
-    __device__ __forceinline__ void setup(const Tab &tab, double a2, double cr2, int ns_, int sub)
+    __device__ __forceinline__ void setup(const Tab &tab, double a2, double cr2, int ns_, bool first, bool last)
     {
         ns = ns_;
         const double e0 = tab.E(0);
@@ -242,8 +244,8 @@ struct LpRow {
             w = w1;
         }
         w_last = w;
-        if (sub == 0) L[0] = 0.0;
-        if (sub == G - 1) U[M - 1] = 0.0;
+        if (first) L[0] = 0.0;
+        if (last) U[M - 1] = 0.0;
         s0 = 0.0;
         s1 = 0.0;
     }
@@ -252,7 +254,7 @@ struct LpRow {
     // chi_i <- D_i chi_i + U_i chi_{i+1}.  These are the same bits the general form gives for such a row
     // (there W + |W| = 0 exactly and the L term adds a zero).
     template <class Tab>
-    __device__ __forceinline__ void setup_cool(const Tab &tab, double a2, double cr2, int ns_, int sub)
+    __device__ __forceinline__ void setup_cool(const Tab &tab, double a2, double cr2, int ns_, bool last)
     {
         ns = ns_;
         const double e0 = tab.E(0);
@@ -271,7 +273,7 @@ struct LpRow {
             w = w1;
         }
         w_last = w;
-        if (sub == G - 1) U[M - 1] = 0.0;
+        if (last) U[M - 1] = 0.0;
         s0 = 0.0;
         s1 = 0.0;
     }
@@ -448,6 +450,30 @@ struct LpStage {
         }
         __syncwarp();
     }
+    // The same without registers in between: the row's 16-byte pieces go straight from global memory to their
+    // place in a stage buffer (cp.async, LDGSTS) and are collected by take() once they have landed -- a row can
+    // be fetched a whole row ahead at no register cost.
+    static __device__ __forceinline__ void fetch_async(const double *__restrict__ grow, unsigned char *stage, int lane)
+    {
+#pragma unroll
+        for (int k = 0; k < M / 2; ++k) {
+            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(stage + unit_offset(k * 32 + lane));
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(grow + 2 * (k * 32 + lane)) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    static __device__ __forceinline__ void take(unsigned char *stage, int lane, double (&v)[M])
+    {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < M / 2; ++j) {
+            const double2 u = *reinterpret_cast<const double2 *>(stage + lane * kSliceBytes + j * 16);
+            v[2 * j] = u.x;
+            v[2 * j + 1] = u.y;
+        }
+        __syncwarp();
+    }
     static __device__ __forceinline__ void store(double *__restrict__ grow, unsigned char *stage, int lane,
                                                  const double (&v)[M])
     {
@@ -468,28 +494,38 @@ struct LpStage {
 constexpr int kDirectThreads = 128;
 constexpr int kDirectWarps = kDirectThreads / 32;
 
-template <int NB, bool DIAG, bool FUSED>
-__global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSpectralArgs A)
+// MODE: 0 staged (lp_spectral_update), 1 fused step, 2 fused step that re-sorts (reads through A.perm)
+template <int NB, bool DIAG, int MODE>
+__global__ void __launch_bounds__(kDirectThreads, 3) lp_spectral_direct_kernel(LpSpectralArgs A)
 {
+    constexpr bool FUSED = MODE >= 1, PERM = MODE == 2;
     static_assert(NB >= 32, "one row per warp");
     constexpr int G = 32;                     // lanes that share one row
     constexpr int M = NB / G;                 // bins per lane (contiguous)
     constexpr int U = (M <= 2) ? 4 : (M == 4 ? 2 : 1);   // rows in flight per warp
 
-    __shared__ __align__(16) double sE[NB + 2];
-    __shared__ __align__(16) double sR[NB];
+    constexpr bool kTabRegs = (M <= 4);
+    // plain copies of the table: the lanes' register slices (M <= 4) are cut from them; with M >= 8 only the
+    // per-particle phase would read them (E_0, and every bin when the table has no CFL candidates), and it
+    // takes them from global memory instead -- the two row buffers need the shared memory
+    __shared__ __align__(16) double sEs[kTabRegs ? NB + 2 : 2];
+    __shared__ __align__(16) double sRs[kTabRegs ? NB : 2];
     __shared__ double2 sAC[kDirectWarps][32];
     __shared__ int sNS[kDirectWarps][32];
+    const double *sE = kTabRegs ? sEs : A.tab;
+    const double *sR = kTabRegs ? sRs : A.tab + (NB + 1) + NB;
 
-    for (int i = threadIdx.x; i <= NB; i += kDirectThreads) sE[i] = A.tab[i];
-    for (int i = threadIdx.x; i < NB; i += kDirectThreads) sR[i] = A.tab[(NB + 1) + NB + i];
-    __syncthreads();
+    if (kTabRegs) {
+        for (int i = threadIdx.x; i <= NB; i += kDirectThreads) sEs[i] = A.tab[i];
+        for (int i = threadIdx.x; i < NB; i += kDirectThreads) sRs[i] = A.tab[(NB + 1) + NB + i];
+        __syncthreads();
+    }
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    constexpr bool kTabRegs = (M <= 4);
     constexpr bool kStaged = (M >= 8);           // rows through the transposing staging buffer
     static_assert(!kStaged || U == 1, "the staged path keeps one row ahead");
     __shared__ __align__(16) unsigned char sStage[kDirectWarps][kStaged ? LpStage<M>::kBytes : 16];
+    __shared__ __align__(16) unsigned char sNext[kDirectWarps][kStaged ? LpStage<M>::kBytes : 16];     // the row fetched ahead
     __shared__ double sET[kTabRegs ? 1 : (M + 1) * 32];
     __shared__ double sRT[kTabRegs ? 1 : M * 32];
     if (!kTabRegs) {
@@ -508,13 +544,12 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
         const long long base = chunk << 5;
         const bool have = base + lane < A.np;
         // source index of this lane's particle (a re-sort folded into the step reads through the permutation)
-        const long long src = have ? (A.perm ? (long long)A.perm[base + lane] : base + lane) : 0;
+        const long long src = have ? (PERM ? (long long)A.perm[base + lane] : base + lane) : 0;
         auto src_of = [&](int j) -> long long { return __shfl_sync(kFull, src, j); };
         const double px = have ? A.xin[src] : 0.0, py = have ? A.yin[src] : 0.0, pz = have ? A.zin[src] : 0.0;
-        if (A.perm && have) A.id_out[base + lane] = A.id_in[src];
-        double2 ahead[kStaged ? M / 2 : 1];                 // (staged, U == 1) the next row, fetched a row ahead
-        if constexpr (kStaged) {
-            if (base < A.np) LpStage<M>::fetch(A.chi_in + src_of(0) * NB, lane, ahead);      // flies during phase 1
+        if (PERM && have) A.id_out[base + lane] = A.id_in[src];
+        if constexpr (kStaged) {                            // (staged, U == 1) the next row is fetched a row ahead
+            if (base < A.np) LpStage<M>::fetch_async(A.chi_in + src_of(0) * NB, sNext[warp], lane);      // flies during phase 1
         }
         lp_chunk_phase1<NB, FUSED>(A, base, lane, px, py, pz, sE, sR, sAC[warp], sNS[warp]);
         for (int j0 = 0; j0 < 32; j0 += U) {
@@ -525,8 +560,8 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
                 const long long sj = src_of(j0 + u), sj1 = src_of((j0 + u + 1) & 31);      // (all lanes shuffle)
                 if (pj < A.np) {
                     if constexpr (kStaged) {
-                        LpStage<M>::place(ahead, sStage[warp], lane, buf[u]);
-                        if (j0 + 1 < 32 && pj + 1 < A.np) LpStage<M>::fetch(A.chi_in + sj1 * NB, lane, ahead);
+                        LpStage<M>::take(sNext[warp], lane, buf[u]);
+                        if (j0 + 1 < 32 && pj + 1 < A.np) LpStage<M>::fetch_async(A.chi_in + sj1 * NB, sNext[warp], lane);
                     } else {
                         lp_load_row<M>(A.chi_in + sj * NB + lane * M, buf[u]);
                     }
@@ -554,11 +589,11 @@ __global__ void __launch_bounds__(kDirectThreads) lp_spectral_direct_kernel(LpSp
             }
             if (cool) {                                     // every row in flight is a cooling row
 #pragma unroll
-                for (int u = 0; u < U; ++u) row[u].setup_cool(tab, ac[u].x, ac[u].y, nsr[u], lane);
+                for (int u = 0; u < U; ++u) row[u].setup_cool(tab, ac[u].x, ac[u].y, nsr[u], lane == G - 1);
                 lp_rows_substeps<true, U, M, G, DIAG>(row, nmin, nmax);
             } else {
 #pragma unroll
-                for (int u = 0; u < U; ++u) row[u].setup(tab, ac[u].x, ac[u].y, nsr[u], lane);
+                for (int u = 0; u < U; ++u) row[u].setup(tab, ac[u].x, ac[u].y, nsr[u], lane == 0, lane == G - 1);
                 lp_rows_substeps<false, U, M, G, DIAG>(row, nmin, nmax);
             }
 #pragma unroll
@@ -745,9 +780,10 @@ struct LpBulkCfg {
 //    chunk's coefficients, applies the substeps and stores the rows.
 // full[slot] / empty[slot] mbarriers (one arrival each) hand the coefficient slots back and forth.
 // Row indices are 32-bit inside the kernel (lp_create limits np to 2^32 - 1); only addresses are 64-bit.
-template <int NB, bool DIAG, bool FUSED>
+template <int NB, bool DIAG, int MODE>
 __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spectral_bulk_kernel(LpSpectralArgs A)
 {
+    constexpr bool FUSED = MODE >= 1, PERM = MODE == 2;
     using C = LpBulkCfg<NB>;
     constexpr int G = C::G, M = C::M, PPW = C::PPW, R = C::R, GPC = C::GPC, S = C::S, RI = C::RI;
     constexpr int NP = C::NP, NR = C::NR, D = C::D;
@@ -794,7 +830,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
         // step re-sorts (A.perm) they are read through the permutation, whose entries are fetched a chunk
         // earlier still, and the ids move with them
         auto chunk_of = [&](uint32_t t) -> uint32_t { return chunk_start(t); };
-        const uint32_t *perm = A.perm;
+        const uint32_t *perm = PERM ? A.perm : nullptr;
         auto own_index = [&](uint32_t t, bool &valid) -> uint32_t {      // index of this lane's particle of chunk t
             valid = t < nblk && chunk_of(t) + lane < np;
             return valid ? chunk_of(t) + lane : 0u;
@@ -861,7 +897,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
     // Re-sort folded into the step: row r of the group comes from row perm[row0 + r] of chi_in -- one bulk copy
     // per row, issued by lane r, all completing on the slot's barrier.  Whole warp calls; `src` = this lane's
     // perm entry for the group (fetched an iteration ahead, so that its latency is not on the issue path).
-    const uint32_t *perm = A.perm;
+    const uint32_t *perm = PERM ? A.perm : nullptr;
     auto perm_entry = [&](uint32_t j) -> uint32_t {      // perm[row0(j) + lane], 0 if there is no such row
         if (j >= ngroups || lane >= R) return 0u;
         const uint32_t r = group_row0(j) + lane;
@@ -938,11 +974,11 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
                     nmin = -lp_group_max<G>(-nmin);
                     if (__all_sync(kFull, cool)) {                  // every row in flight is a cooling row
 #pragma unroll
-                        for (int r = 0; r < RI; ++r) row[r].setup_cool(tab, ac[r].x, ac[r].y, nsr[r], sub);
+                        for (int r = 0; r < RI; ++r) row[r].setup_cool(tab, ac[r].x, ac[r].y, nsr[r], sub == G - 1);
                         lp_rows_substeps<true, RI, M, G, DIAG>(row, nmin, nmax);
                     } else {
 #pragma unroll
-                        for (int r = 0; r < RI; ++r) row[r].setup(tab, ac[r].x, ac[r].y, nsr[r], sub);
+                        for (int r = 0; r < RI; ++r) row[r].setup(tab, ac[r].x, ac[r].y, nsr[r], sub == 0, sub == G - 1);
                         lp_rows_substeps<false, RI, M, G, DIAG>(row, nmin, nmax);
                     }
 #pragma unroll
@@ -999,13 +1035,13 @@ template <class K> int lp_blocks_per_sm(K kernel, int threads, size_t smem)
 // blocks_cache: the context's slot for this variant (0 = not set up yet).  Function attributes are per
 // device and a context lives on one device, so the set-up runs once per context and variant; a context
 // is used by one host thread at a time (lp.h), and cudaFuncSetAttribute itself is thread-safe.
-template <int NB, bool DIAG, bool FUSED>
+template <int NB, bool DIAG, int MODE>
 int launch_variant(const LpSpectralArgs &a, int sm_count, int *blocks_cache, cudaStream_t s)
 {
     const long long nchunks = (a.np + 31) >> 5;
     if constexpr (NB <= LP_BULK_MAX_NB) {
         using C = LpBulkCfg<NB>;
-        auto kernel = lp_spectral_bulk_kernel<NB, DIAG, FUSED>;
+        auto kernel = lp_spectral_bulk_kernel<NB, DIAG, MODE>;
         if (*blocks_cache == 0) {
             if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_TOTAL) != cudaSuccess) return -1;
             if (cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, LP_BULK_CARVEOUT) != cudaSuccess) return -1;
@@ -1017,7 +1053,7 @@ int launch_variant(const LpSpectralArgs &a, int sm_count, int *blocks_cache, cud
         if (blocks < 1) blocks = 1;
         kernel<<<blocks, C::THREADS, C::SMEM_TOTAL, s>>>(a);
     } else {
-        auto kernel = lp_spectral_direct_kernel<NB, DIAG, FUSED>;
+        auto kernel = lp_spectral_direct_kernel<NB, DIAG, MODE>;
         if (*blocks_cache == 0) *blocks_cache = lp_blocks_per_sm(kernel, kDirectThreads, 0);
         const long long want = (nchunks + kDirectWarps - 1) / kDirectWarps;
         const long long cap = (long long)sm_count * *blocks_cache;
@@ -1031,9 +1067,12 @@ int launch_variant(const LpSpectralArgs &a, int sm_count, int *blocks_cache, cud
 template <int NB>
 int launch_nb(const LpSpectralArgs &a, bool diag, bool fused, int sm_count, int *blocks_cache, cudaStream_t s)
 {
-    int *slot = blocks_cache + (diag ? 2 : 0) + (fused ? 1 : 0);
-    if (diag) return fused ? launch_variant<NB, true, true>(a, sm_count, slot, s) : launch_variant<NB, true, false>(a, sm_count, slot, s);
-    return fused ? launch_variant<NB, false, true>(a, sm_count, slot, s) : launch_variant<NB, false, false>(a, sm_count, slot, s);
+    const int mode = fused ? (a.perm ? 2 : 1) : 0;
+    int *slot = blocks_cache + (diag ? 3 : 0) + mode;
+    if (diag) return mode == 2 ? launch_variant<NB, true, 2>(a, sm_count, slot, s)
+                   : mode == 1 ? launch_variant<NB, true, 1>(a, sm_count, slot, s) : launch_variant<NB, true, 0>(a, sm_count, slot, s);
+    return mode == 2 ? launch_variant<NB, false, 2>(a, sm_count, slot, s)
+         : mode == 1 ? launch_variant<NB, false, 1>(a, sm_count, slot, s) : launch_variant<NB, false, 0>(a, sm_count, slot, s);
 }
 
 }  // namespace
