@@ -474,9 +474,10 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
         sms = s0.elapsed_time(s1) / reps
         sbytes = 8 * w.np + 16 * w.nbins * nflag             # r of every particle, flagged rows in and out
-        shock = {"kernel": "lp_shock_kernel<%d>" % w.nbins, "flagged": nflag, "ms": sms,
+        shock = {"kernel": "lp_shock_kernel<%d>" % w.nbins, "bound": "hbm", "flagged": nflag, "ms": sms,
                  "algorithmic_bytes": sbytes, "achieved_gbs": sbytes / (sms * 1e-3) / 1e9,
-                 "flagged_rows_per_s": nflag / (sms * 1e-3)}
+                 "flagged_rows_per_s": nflag / (sms * 1e-3),
+                 "traffic": stored_traffic(w.name + "/shock%g" % args.shock_frac, w.nbins)}
 
     # ---- end to end through lp_step_host: pinned host buffers, H2D + D2H every step
     e2e = None

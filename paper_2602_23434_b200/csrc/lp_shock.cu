@@ -2,11 +2,11 @@
 // of DESIGN.md section 3):
 //   chi_out,i = C ec_i^(2-q) [ sum_{j<i} chi_j ec_j^(q-3) dE_j + (1/2) chi_i ec_i^(q-3) dE_i ],
 //   q = 3r/(r-1) + q_R,   C from number conservation,   ec_i = sqrt(E_i E_{i+1}).
-// The integral of Eq. 7 is a weighted prefix sum over the bins: one warp per flagged row, M = N_b/32
-// contiguous bins per lane, a lane-local running sum plus an exclusive warp scan of the lane totals
-// (SHFL.UP), two warp reductions for the normalisation.  Rows with r <= 1 (or NaN) are not touched and
+// The integral of Eq. 7 is a weighted prefix sum over the bins: a group of G lanes per flagged row, M
+// contiguous bins per lane, a lane-local running sum plus an exclusive scan of the lane totals over the group
+// (SHFL.UP), two group reductions for the normalisation.  Rows with r <= 1 (or NaN) are not touched and
 // cost 8 bytes.  sm_100a.
-#include "lp_internal.h"
+#include "lp_device.cuh"
 
 namespace {
 
@@ -14,63 +14,78 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-    return v;
-}
-
-// Per-lane slice of the bin table for the shock update: M contiguous bins of lane `lane`.
-template <int M>
-struct LpShockTab {
-    double ec[M], lnec[M], de[M];
+// A row is held by G = N_b/M lanes, M contiguous bins per lane (M = 4 up to 128 bins, then N_b/32), so a warp
+// works on 32/G flagged rows at once -- at 64 bins two rows share the warp's instructions, at 16 bins eight.
+template <int NB>
+struct LpShockCfg {
+    static constexpr int M = NB >= 128 ? NB / 32 : 4;
+    static constexpr int G = NB / M;
+    static constexpr int PPW = 32 / G;
 };
 
-// One flagged row, all 32 lanes.  ec^(q-3) = exp((q-3) ln ec) with ln ec tabulated per lane, and
-// ec^(2-q) = 1 / (ec^(q-3) ec): one exp and one division per bin and row instead of two pow (the kernel is
-// bound by this arithmetic, not by HBM); relative error ~ |q-3| ln(ec) ulp ~ 1e-14, far inside the 1e-10
-// parity bound.
+// Per-lane slice of the bin table: the M bins [sub*M, sub*M + M).
 template <int M>
-__device__ __forceinline__ void lp_shock_row(const LpShockTab<M> &tb, double rr, double q_r, double *row,
-                                             bool active, int lane)
+struct LpShockTab {
+    double rec[M], de[M];      // 1/ec_i (ec = geometric bin centre), dE_i
+    double lnec0;              // ln ec of the lane's first bin
+    double dln;                // ln(ec_{i+1}/ec_i): the same for every bin of a log-spaced table
+};
+
+// One row per lane group (all 32 lanes call).  ec^(q-3) is a geometric sequence along the bins of a log-spaced
+// table: one exp for the lane's first bin and one for the ratio replace an exp per bin, and
+// ec^(2-q) = 1/(ec^(q-3) ec) comes from the reciprocal sequence -- two exp and two divisions per lane and row
+// instead of one of each per bin (with those the kernel was bound by this arithmetic, not by HBM).  The table's
+// rounding makes the sequence geometric to ~1e-15 in the exponent and the products accumulate to ~1e-13
+// relative, far inside the 1e-10 parity bound.  Returns whether the row was changed (reading S4).
+template <int M, int G>
+__device__ __forceinline__ bool lp_shock_row(const LpShockTab<M> &tb, double rr, double q_r, double (&c)[M], int sub)
 {
     const double q = __dadd_rn(__ddiv_rn(__dmul_rn(3.0, rr), __dsub_rn(rr, 1.0)), q_r);   // Eq. 8
     const double s3 = q - 3.0;
-    double c[M], term[M], t[M], pw[M];
+    const double rho = exp(s3 * tb.dln), irho = 1.0 / rho;
+    double pw = exp(s3 * tb.lnec0), ipw = 1.0 / pw;                 // ec^(q-3) of the lane's first bin, and 1 / it
+    double term[M], scale[M];
     double total = 0.0, n_in = 0.0;
 #pragma unroll
     for (int i = 0; i < M; ++i) {
-        c[i] = active ? row[i] : 0.0;
-        pw[i] = exp(s3 * tb.lnec[i]);                                       // ec^(q-3)
-        term[i] = c[i] * pw[i] * tb.de[i];
+        term[i] = c[i] * pw * tb.de[i];
+        scale[i] = ipw * tb.rec[i];                                 // ec^(2-q)
         total += term[i];
         n_in = fma(c[i], tb.de[i], n_in);
+        pw *= rho;
+        ipw *= irho;
     }
-    // exclusive scan of the lane totals: what lies in the bins below this lane's
+    // exclusive scan of the lane totals over the row's G lanes: what lies in the bins below this lane's
     double incl = total;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const double u = __shfl_up_sync(kFull, incl, o);
-        if (lane >= o) incl += u;
+    for (int o = 1; o < G; o <<= 1) {
+        const double u = __shfl_up_sync(kFull, incl, o, G);
+        if (sub >= o) incl += u;
     }
-    double below = incl - total;
+    // (not incl - total: the lane's own total can exceed what lies below it by many orders of magnitude, and the
+    // difference would lose exactly the digits the lane's first bins need)
+    double below = __shfl_up_sync(kFull, incl, 1, G);
+    if (sub == 0) below = 0.0;
     double n_out = 0.0;
+    double t[M];
 #pragma unroll
     for (int i = 0; i < M; ++i) {
-        t[i] = (below + 0.5 * term[i]) / (pw[i] * tb.ec[i]);                // ec^(2-q) = 1 / (ec^(q-3) ec)
+        t[i] = (below + 0.5 * term[i]) * scale[i];
         below += term[i];
         n_out = fma(t[i], tb.de[i], n_out);
     }
-    n_in = warp_sum(n_in);
-    n_out = warp_sum(n_out);
-    if (n_out != 0.0 && n_out == n_out) {                                   // else: leave the row (S4)
-        const double norm = n_in / n_out;
-        if (active) {
 #pragma unroll
-            for (int i = 0; i < M; ++i) row[i] = norm * t[i];
-        }
+    for (int o = G / 2; o > 0; o >>= 1) {
+        n_in += __shfl_xor_sync(kFull, n_in, o);
+        n_out += __shfl_xor_sync(kFull, n_out, o);
     }
+    const bool changed = n_out != 0.0 && n_out == n_out;            // else: leave the row (S4)
+    if (changed) {
+        const double norm = n_in / n_out;
+#pragma unroll
+        for (int i = 0; i < M; ++i) c[i] = norm * t[i];
+    }
+    return changed;
 }
 
 template <int NB>
@@ -78,31 +93,59 @@ __global__ void __launch_bounds__(kThreads)
 lp_shock_kernel(const double *__restrict__ tab, const double *__restrict__ r, double q_r,
                 double *__restrict__ chi, long long np)
 {
-    constexpr int M = NB >= 32 ? NB / 32 : 1;          // bins per lane
-    constexpr int LANES = NB >= 32 ? 32 : NB;          // lanes that hold bins (16 bins: half a warp)
-    const int lane = threadIdx.x & 31;
-    const bool active = lane < LANES;
-    const int b0 = active ? lane * M : 0;
+    using C = LpShockCfg<NB>;
+    constexpr int M = C::M, G = C::G, PPW = C::PPW;
+    constexpr bool kStaged = M >= 8;              // rows through the transposing stage buffer (then G = 32, PPW = 1)
+    __shared__ __align__(16) unsigned char sStage[kWarps][kStaged ? LpStage<M>::kBytes : 16];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sub = lane % G, grp = lane / G;
+    const int b0 = sub * M;
 
     LpShockTab<M> tb;
 #pragma unroll
     for (int i = 0; i < M; ++i) {
-        tb.ec[i] = __dsqrt_rn(__dmul_rn(tab[b0 + i], tab[b0 + i + 1]));    // geometric centre
-        tb.lnec[i] = log(tb.ec[i]);
-        tb.de[i] = active ? tab[(NB + 1) + b0 + i] : 0.0;                   // idle lanes (16 bins) weigh nothing
+        const double ec = __dsqrt_rn(__dmul_rn(tab[b0 + i], tab[b0 + i + 1]));      // geometric centre
+        tb.rec[i] = 1.0 / ec;
+        tb.de[i] = tab[(NB + 1) + b0 + i];
+        if (i == 0) tb.lnec0 = log(ec);
     }
+    tb.dln = (log(tab[NB]) - log(tab[0])) / (double)NB;
 
-    // a warp takes 32 consecutive particles at a time: one coalesced read of their r, a ballot of the
-    // flagged ones, then one flagged row after the other -- unflagged particles cost their 8 bytes only
+    // a warp takes 32 consecutive particles at a time: one coalesced read of their r, a ballot of the flagged
+    // ones, then the flagged rows PPW at a time -- unflagged particles cost their 8 bytes only
     const long long gw = ((long long)blockIdx.x * kThreads + threadIdx.x) >> 5;
     const long long nw = ((long long)gridDim.x * kThreads) >> 5;
     for (long long base = gw << 5; base < np; base += nw << 5) {
         const double r_lane = base + lane < np ? r[base + lane] : 0.0;
-        unsigned todo = __ballot_sync(kFull, r_lane > 1.0);                 // r <= 1 or NaN: no shock
-        while (todo) {
-            const int j = __ffs(todo) - 1;
-            todo &= todo - 1;
-            lp_shock_row<M>(tb, __shfl_sync(kFull, r_lane, j), q_r, chi + (base + j) * NB + b0, active, lane);
+        const unsigned todo = __ballot_sync(kFull, r_lane > 1.0);                   // r <= 1 or NaN: no shock
+        const int nflag = __popc(todo);
+        for (int k = 0; k < nflag; k += PPW) {
+            const int idx = k + grp;                                                // this group's flagged row
+            const bool valid = idx < nflag;
+            const int j = valid ? (int)__fns(todo, 0, idx + 1) : 0;                // the idx-th set bit of todo
+            const double rr = __shfl_sync(kFull, r_lane, j);
+            double *row = chi + (base + j) * NB;
+            double c[M];
+            if constexpr (kStaged) {
+                double2 t2[M / 2];
+                LpStage<M>::fetch(row, lane, t2);                                   // (valid is warp-uniform: PPW = 1)
+                LpStage<M>::place(t2, sStage[warp], lane, c);
+            } else {
+#pragma unroll
+                for (int i = 0; i < M; i += 2) {
+                    const double2 v = valid ? *reinterpret_cast<const double2 *>(row + b0 + i) : make_double2(0.0, 0.0);
+                    c[i] = v.x;
+                    c[i + 1] = v.y;
+                }
+            }
+            const bool changed = lp_shock_row<M, G>(tb, valid ? rr : 2.0, q_r, c, sub);
+            if constexpr (kStaged) {
+                if (changed) LpStage<M>::store(row, sStage[warp], lane, c);         // (uniform over the warp)
+            } else if (valid && changed) {
+#pragma unroll
+                for (int i = 0; i < M; i += 2) *reinterpret_cast<double2 *>(row + b0 + i) = make_double2(c[i], c[i + 1]);
+            }
         }
     }
 }

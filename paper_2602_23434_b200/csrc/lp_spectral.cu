@@ -418,77 +418,6 @@ __device__ __forceinline__ int lp_group_max(int n)
     return n;
 }
 
-// Row <-> lane slices through a per-warp staging buffer, for M >= 8 bins per lane.  A lane's slice is M*8
-// bytes of the row, so loading it directly makes every 16-byte load instruction of the warp touch 32
-// different 128-byte lines (measured at M = 16: ~500 L1 wavefronts per row, the kernel's bound after the
-// table fix).  Instead the warp moves the row with fully coalesced 16-byte accesses and transposes in shared
-// memory; slices are padded by 16 bytes so that both sides are free of bank conflicts.
-template <int M>
-struct LpStage {
-    static constexpr int kSliceBytes = M * 8 + 16;                 // padded slice of one lane
-    static constexpr int kBytes = 32 * kSliceBytes;
-    // 16-byte unit e of the row (0 .. 2M*... ) lives at:
-    static __device__ __forceinline__ int unit_offset(int e) { return (e / (M / 2)) * kSliceBytes + (e % (M / 2)) * 16; }
-
-    // the row's coalesced 16-byte pieces into registers (issued early: a row ahead of its use)
-    static __device__ __forceinline__ void fetch(const double *__restrict__ grow, int lane, double2 (&t)[M / 2])
-    {
-#pragma unroll
-        for (int k = 0; k < M / 2; ++k) t[k] = *reinterpret_cast<const double2 *>(grow + 2 * (k * 32 + lane));
-    }
-    // fetched pieces -> this lane's slice
-    static __device__ __forceinline__ void place(const double2 (&t)[M / 2], unsigned char *stage, int lane, double (&v)[M])
-    {
-#pragma unroll
-        for (int k = 0; k < M / 2; ++k) *reinterpret_cast<double2 *>(stage + unit_offset(k * 32 + lane)) = t[k];
-        __syncwarp();
-#pragma unroll
-        for (int j = 0; j < M / 2; ++j) {
-            const double2 u = *reinterpret_cast<const double2 *>(stage + lane * kSliceBytes + j * 16);
-            v[2 * j] = u.x;
-            v[2 * j + 1] = u.y;
-        }
-        __syncwarp();
-    }
-    // The same without registers in between: the row's 16-byte pieces go straight from global memory to their
-    // place in a stage buffer (cp.async, LDGSTS) and are collected by take() once they have landed -- a row can
-    // be fetched a whole row ahead at no register cost.
-    static __device__ __forceinline__ void fetch_async(const double *__restrict__ grow, unsigned char *stage, int lane)
-    {
-#pragma unroll
-        for (int k = 0; k < M / 2; ++k) {
-            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(stage + unit_offset(k * 32 + lane));
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(grow + 2 * (k * 32 + lane)) : "memory");
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    }
-    static __device__ __forceinline__ void take(unsigned char *stage, int lane, double (&v)[M])
-    {
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncwarp();
-#pragma unroll
-        for (int j = 0; j < M / 2; ++j) {
-            const double2 u = *reinterpret_cast<const double2 *>(stage + lane * kSliceBytes + j * 16);
-            v[2 * j] = u.x;
-            v[2 * j + 1] = u.y;
-        }
-        __syncwarp();
-    }
-    static __device__ __forceinline__ void store(double *__restrict__ grow, unsigned char *stage, int lane,
-                                                 const double (&v)[M])
-    {
-#pragma unroll
-        for (int j = 0; j < M / 2; ++j)
-            *reinterpret_cast<double2 *>(stage + lane * kSliceBytes + j * 16) = make_double2(v[2 * j], v[2 * j + 1]);
-        __syncwarp();
-#pragma unroll
-        for (int k = 0; k < M / 2; ++k)
-            *reinterpret_cast<double2 *>(grow + 2 * (k * 32 + lane)) =
-                *reinterpret_cast<const double2 *>(stage + unit_offset(k * 32 + lane));
-        __syncwarp();
-    }
-};
-
 // ------------------------------------------------------------------ direct mover (N_b = 512)
 
 constexpr int kDirectThreads = 128;
