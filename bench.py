@@ -47,6 +47,9 @@ def parse():
     ap.add_argument("--migrate-frac", type=float, default=0.0,
                     help="at the end, time one directional particle exchange (lp_migrate_count/_pack/_unpack, "
                          "PAPER.md:201-214) in which this fraction of the particles leaves through the two x faces")
+    ap.add_argument("--gather", action="store_true",
+                    help="also time the gather alone, direct (lp_interpolate) and through shared-memory tiles "
+                         "(lp_interpolate_tiled), on the state as the timed steps leave it and right after a sort")
     ap.add_argument("--pusher", default="rk2", choices=["rk2", "rk3"],
                     help="with --staged: the two-stage pusher (lp_push) or the three-stage one (lp_push_rk3)")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -500,6 +503,27 @@ def run_ours(args):
                "api": "lp_step_host (pinned host x,y,z,id,chi in and out every step)"}
         del hx, hy, hz, hid, hchi
 
+    # ---- the gather alone: direct against shared-memory tiles (north_star names both)
+    gather = None
+    if args.gather:
+        def time_gather(fn, reps=5):
+            fn()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record()
+            for _ in range(reps):
+                fn()
+            g1.record()
+            torch.cuda.synchronize(dev)
+            return g0.elapsed_time(g1) / reps
+        out7 = torch.empty((7, w.np), dtype=torch.float64, device=dev)
+        direct = lambda: B.lp_interpolate(lp.ctx, out7.data_ptr(), None, lp.stream)
+        tiled = lambda: B.lp_interpolate_tiled(lp.ctx, out7.data_ptr(), lp.stream)
+        gather = {"steps_since_sort": (nstep[0] - 1) % w.sort_every + 1 if w.sort_every else None,
+                  "drifted": {"direct_ms": time_gather(direct), "tiled_ms": time_gather(tiled)}}
+        lp.sort()
+        gather["just_sorted"] = {"direct_ms": time_gather(direct), "tiled_ms": time_gather(tiled)}
+        gather["bytes_out"] = 56 * w.np
+
     # ---- particle exchange (NEXT-3): this rank owns x in [xlo + d, xhi - d) of the periodic box; the leavers of
     # each face come back in through the other one (what the neighbour would send), so the count is unchanged
     migrate = None
@@ -608,6 +632,8 @@ def run_ours(args):
         out["compact"] = compact
     if migrate is not None:
         out["migrate"] = migrate
+    if gather is not None:
+        out["gather"] = gather
     if shock is not None:
         peak_s, _ = measured_peak()
         shock["frac_of_measured_peak"] = shock["achieved_gbs"] / peak_s

@@ -115,6 +115,13 @@ LP_API lp_status lp_set_fields(lp_ctx *ctx, const double *vx, const double *vy, 
  * vx,vy,vz,bx,by,bz,rho (or NULL) and the containing-cell key (k*ny+j)*nx+i [np] (or NULL). */
 LP_API lp_status lp_interpolate(lp_ctx *ctx, double *out7, uint32_t *cell_key, void *stream);
 
+/* The same sampling through shared-memory tiles (the option BASELINE.json's north_star names beside the direct
+ * gather): blocks of 64 consecutive particles load the bounding box of their stencils once and gather from
+ * shared memory; blocks whose box does not fit (set not sorted by cell, or drifted apart) gather directly.
+ * Bit-identical to lp_interpolate.  Kept as a measured alternative: profiles/r02_gather_tile.md has the numbers
+ * that decided for the direct gather in the fused kernels. */
+LP_API lp_status lp_interpolate_tiled(lp_ctx *ctx, double *out7, void *stream);
+
 /* Reorder all particle arrays ascending by (cell key, id); bound arrays hold the result.  Asynchronous,
  * except for the first sort after the ids may have changed (see lp_bind_particles). */
 LP_API lp_status lp_sort(lp_ctx *ctx, void *stream);

@@ -21,7 +21,7 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_measure_fp64_peak", "lp_set_pingpong", "lp_current_particles",
            "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack",
            "lp_capacity", "lp_workspace_bytes_for", "lp_rebind",
-           "lp_bind_energy_grid", "lp_init_energy_grid")
+           "lp_bind_energy_grid", "lp_init_energy_grid", "lp_interpolate_tiled")
 
 
 class LPError(RuntimeError):
@@ -74,6 +74,7 @@ def load():
     lib.lp_bind_diag.argtypes = [vp, dp, dp]
     lib.lp_set_fields.argtypes = [vp] + [dp] * 7 + [vp]
     lib.lp_interpolate.argtypes = [vp, dp, dp, vp]
+    lib.lp_interpolate_tiled.argtypes = [vp, dp, vp]
     lib.lp_sort.argtypes = [vp, vp]
     lib.lp_push.argtypes = [vp, C.c_double, C.c_int, vp]
     lib.lp_spectral_update.argtypes = [vp, C.c_double, vp]
@@ -174,6 +175,10 @@ def lp_set_fields(ctx, vx, vy, vz, bx, by, bz, rho, stream=None):
 
 def lp_interpolate(ctx, out7, cell_key, stream=None):
     _check(ctx, load().lp_interpolate(ctx, out7, cell_key, stream))
+
+
+def lp_interpolate_tiled(ctx, out7, stream=None):
+    _check(ctx, load().lp_interpolate_tiled(ctx, out7, stream))
 
 
 def lp_sort(ctx, stream=None):

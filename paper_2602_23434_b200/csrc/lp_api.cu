@@ -177,6 +177,7 @@ struct lp_ctx {
     // particle exchange in progress (lp_migrate_count -> _pack -> _unpack): 0 none, 1 counted, 2 packed
     int mig_stage = 0;
     long long mig_left = 0, mig_right = 0;
+    bool tile_configured = false;          // lp_interpolate_tile_kernel's shared-memory attribute is set
     bool split_records = false;            // cell records as two 32-byte arrays (dense sets) or one 64-byte array (LpCells)
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
@@ -606,6 +607,18 @@ lp_status lp_interpolate(lp_ctx *ctx, double *out7, uint32_t *cell_key, void *st
     const lp_ctx::Set n = ctx->now();
     return count(ctx, lp_launch_interpolate(ctx->geom, ctx->cells(), n.x, n.y, n.z, ctx->cfg.np, out7, cell_key,
                                             static_cast<cudaStream_t>(stream)), "lp_interpolate_kernel launch");
+}
+
+lp_status lp_interpolate_tiled(lp_ctx *ctx, double *out7, void *stream)
+{
+    lp_status st = need_ready(ctx, true);
+    if (st != LP_OK) return st;
+    if (!out7) return fail(ctx, LP_ERR_INVALID_ARG, "out7 is NULL");
+    if (ctx->cfg.np == 0) return LP_OK;
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const lp_ctx::Set n = ctx->now();
+    return count(ctx, lp_launch_interpolate_tiled(ctx->geom, ctx->cells(), n.x, n.y, n.z, ctx->cfg.np, out7,
+                                                  &ctx->tile_configured, static_cast<cudaStream_t>(stream)), "lp_interpolate_tile_kernel launch");
 }
 
 lp_status lp_sort(lp_ctx *ctx, void *stream)

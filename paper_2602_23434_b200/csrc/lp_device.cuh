@@ -56,7 +56,7 @@ __device__ __forceinline__ void lp_axis(double x, double lo, double inv_dx, int 
     int b = (int)fl;
     i0 = lp_wrap(b, n, periodic);
     if (periodic) i1 = (i0 + 1 == n) ? 0 : i0 + 1;          // floor-mod of b + 1
-    else i1 = min(max(b + 1, 0), n - 1);
+    else i1 = min(max(b + (b != 0x7fffffff), 0), n - 1);   // (the conversion saturates for positions absurdly far out: no overflow)
     w0 = __dsub_rn(1.0, f);
     w1 = f;
 }

@@ -88,6 +88,8 @@ int lp_launch_repack(const double *const f[7], double4 *recA, double4 *recB, uns
                      cudaStream_t s);
 int lp_launch_interpolate(const LpGeom &g, const LpCells &c, const double *x, const double *y,
                           const double *z, long long np, double *out7, uint32_t *key, cudaStream_t s);
+int lp_launch_interpolate_tiled(const LpGeom &g, const LpCells &c, const double *x, const double *y,
+                                const double *z, long long np, double *out7, bool *configured, cudaStream_t s);
 int lp_launch_push0(const LpPushArgs &a, cudaStream_t s);
 int lp_launch_push1(const LpPushArgs &a, cudaStream_t s);
 int lp_launch_push_rk3(const LpPushArgs &a, int stage, cudaStream_t s);     // stage 0, 1, 2 (x0 kept in a.xs)

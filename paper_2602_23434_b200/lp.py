@@ -108,6 +108,12 @@ class LP:
                          key.data_ptr() if want_key else None, self.stream)
         return out7, key
 
+    def interpolate_tiled(self):
+        """lp_interpolate's fields through shared-memory tiles (for sets sorted by cell); same values."""
+        out7 = torch.empty((7, self.cfg.np), dtype=torch.float64, device=self.device)
+        B.lp_interpolate_tiled(self.ctx, out7.data_ptr(), self.stream)
+        return out7
+
     def sort(self):
         B.lp_sort(self.ctx, self.stream)
 

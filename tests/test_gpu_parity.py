@@ -83,6 +83,27 @@ def test_key_non_cubic_grid():
 
 # ------------------------------------------------------------------ a5, a6: push
 
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 0, 0), (1, 0, 1)])
+@pytest.mark.parametrize("np_,n", [(6000 + 3, 12), (70001, 40), (31, 6)])
+def test_interpolate_tiled_bit_exact(periodic, np_, n):
+    """The shared-memory-tile gather gives lp_interpolate's bits: sorted by cell (tiles), then shuffled (the
+    blocks fall back to the direct gather), with far-away particles in one block."""
+    w = small_turbulent(n=n, np_=np_, periodic=periodic)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True)
+    want = orc.gather(prm, f_np, x, y, z)
+    assert np.array_equal(host(lp.interpolate_tiled()), want)            # unsorted: most blocks fall back
+    lp.sort()
+    order = np.argsort(host(lp.id).view(np.uint64)); inv = np.argsort(np.argsort(pid))
+    got = host(lp.interpolate_tiled())[:, order][:, inv]
+    assert np.array_equal(got, want)                                     # sorted: tiles
+    direct, _ = lp.interpolate(want_key=False)
+    assert np.array_equal(host(direct), host(lp.interpolate_tiled()))
+    if np_ > 100:                                                        # a few particles far outside the box
+        lp.x[:5] = torch.tensor([1e3, -1e3, 7.5, 1e12, -3.0], dtype=torch.float64, device=lp.device)
+        direct, _ = lp.interpolate(want_key=False)
+        assert np.array_equal(host(direct), host(lp.interpolate_tiled()), equal_nan=True)
+
+
 @pytest.mark.parametrize("periodic", [(1, 1, 1), (0, 0, 0)])
 def test_push_positions_bit_exact_over_steps(periodic):
     w = small_turbulent(np_=3000 + 11, periodic=periodic)
