@@ -184,7 +184,8 @@ LP_API lp_status lp_set_count(lp_ctx *ctx, int64_t np_new);
  *                      pusher) -- and the two totals.  Synchronises `stream` (the totals size the buffers).
  *   lp_migrate_pack    step 4: the leavers' x, y, z, id and chi row, in ascending index order, into the send
  *                      buffers.  A buffer for n particles is n * lp_migrate_record_bytes bytes, 16-byte
- *                      aligned, laid out as arrays  x[n] | y[n] | z[n] | id[n] | chi[n][nbins];
+ *                      aligned, laid out as arrays  x[n] | y[n] | z[n] | id[n] | chi[n][nbins]  (and, with a
+ *                      bound energy grid, | eng[n][nbins+1]);
  *                      NULL is allowed for a buffer whose total is 0.
  *   lp_migrate_unpack  step 8: the n_from_left particles of from_left, then the n_from_right of from_right
  *                      (same layout, written by the neighbours' lp_migrate_pack): the k-th arrival goes into
@@ -230,10 +231,16 @@ LP_API lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_
  *                        second array of the same size through which a sort moves the rows (NULL: sorts return
  *                        LP_ERR_STATE).  eng = NULL switches back to the fixed bins.
  *   lp_init_energy_grid  rows [first, first + count) <- the fixed table's edges (the grid every particle starts on).
- * Calls that move particles without their grid rows -- lp_compact, lp_migrate_*, lp_rebind, lp_step_host -- and
- * lp_shock_update (its bin centres are the fixed table's) return LP_ERR_UNSUPPORTED while a grid is bound. */
+ *   lp_rebind_energy_grid  after lp_rebind changed the capacity: new arrays of capacity rows; the current particles'
+ *                        rows are copied over on `stream`.  Until then every call that uses the grid returns
+ *                        LP_ERR_STATE when the capacity has outgrown the bound arrays.
+ * The grid rows travel with their particles: lp_sort, lp_compact and lp_migrate_pack / _unpack move them (an
+ * exchange buffer then carries eng[n][nbins+1] behind chi[n][nbins]; lp_migrate_record_bytes says so).
+ * lp_step_host (no host grid argument) and lp_shock_update (its bin centres are the fixed table's) return
+ * LP_ERR_UNSUPPORTED while a grid is bound. */
 LP_API lp_status lp_bind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch);
 LP_API lp_status lp_init_energy_grid(lp_ctx *ctx, int64_t first, int64_t count, void *stream);
+LP_API lp_status lp_rebind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch, void *stream);
 
 /* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
  * spectral update (order of Table 1, without the fluid stages). */

@@ -146,6 +146,7 @@ struct lp_ctx {
     int32_t *nsub_user = nullptr;
     double *lost_user = nullptr;
     double *eng = nullptr, *eng_scratch = nullptr;      // per-particle energy grid (lp_bind_energy_grid): moving-grid mode
+    long long eng_capacity = 0;                         // rows the bound grid arrays hold
     // owned small tables
     double *tab = nullptr;                 // E[nb+1] | dE[nb] | rdE[nb]
     std::vector<double> h_edges, h_widths;
@@ -254,6 +255,14 @@ lp_status need_ready(lp_ctx *c, bool fields)
     return LP_OK;
 }
 
+// a bound energy grid must cover the capacity of the particle arrays (lp_rebind may have outgrown it)
+lp_status grid_ok(lp_ctx *c)
+{
+    if (c->eng && c->eng_capacity < c->capacity)
+        return fail(c, LP_ERR_STATE, "the energy-grid arrays hold fewer rows than the particle arrays (lp_rebind_energy_grid)");
+    return LP_OK;
+}
+
 lp_status not_with_energy_grid(lp_ctx *c, const char *what)
 {
     if (c->eng) return fail(c, LP_ERR_UNSUPPORTED, std::string(what) + " does not move the per-particle energy grid (lp_bind_energy_grid is active)");
@@ -263,6 +272,8 @@ lp_status not_with_energy_grid(lp_ctx *c, const char *what)
 // spectral update on the per-particle moving grid (lp_moving.cu)
 lp_status do_moving(lp_ctx *c, double dt, cudaStream_t s)
 {
+    lp_status gs = grid_ok(c);
+    if (gs != LP_OK) return gs;
     const lp_ctx::Set n = c->now();
     const bool rec = c->timing && c->ev_used + 2 <= c->ev.size();
     if (rec) LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used], s));
@@ -429,6 +440,7 @@ lp_status do_sort(lp_ctx *c, bool in_place, SpectralIO *io, cudaStream_t s)
     const long long np = c->cfg.np;
     if (np == 0) return LP_OK;
     if (c->eng && !c->eng_scratch) return fail(c, LP_ERR_STATE, "a sort needs the eng_scratch array of lp_bind_energy_grid");
+    if (grid_ok(c) != LP_OK) return LP_ERR_STATE;
     uint32_t *perm = nullptr;
     lp_status st = sort_permutation(c, &perm, s);
     if (st != LP_OK) return st;
@@ -698,10 +710,10 @@ lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *st
 {
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
-    if ((st = not_with_energy_grid(ctx, "lp_compact")) != LP_OK) return st;
     if (!np_new) return fail(ctx, LP_ERR_INVALID_ARG, "np_new is NULL");
     *np_new = ctx->cfg.np;
     if (ctx->cfg.np == 0) return LP_OK;
+    if ((st = grid_ok(ctx)) != LP_OK) return st;
     if (!flag && !ctx->status_valid)
         return fail(ctx, LP_ERR_STATE, "no flags given and no outside-box status of the bound particles (lp_push 1 / lp_step first)");
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
@@ -711,7 +723,7 @@ lp_status lp_compact(lp_ctx *ctx, const int32_t *flag, int64_t *np_new, void *st
     st = count(ctx, lp_launch_compact(flag, ctx->cfg.np, ctx->cfg.nbins, ctx->at<uint32_t>(ctx->lay.hist),
                                       ctx->at<uint32_t>(ctx->lay.idx_a), ctx->at<uint32_t>(ctx->lay.idx_b),
                                       ctx->at<uint32_t>(ctx->lay.key), counts, ctx->now().x, ctx->now().y, ctx->now().z,
-                                      ctx->now().id, ctx->now().chi, ctx->sm_count, s), "compaction kernels launch");
+                                      ctx->now().id, ctx->now().chi, ctx->eng, ctx->sm_count, s), "compaction kernels launch");
     if (st != LP_OK) return st;
     LP_CUDA(ctx, cudaMemcpyAsync(h_counts, counts, sizeof h_counts, cudaMemcpyDeviceToHost, s));
     LP_CUDA(ctx, cudaStreamSynchronize(s));
@@ -768,7 +780,6 @@ lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_t bytes
 {
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
-    if ((st = not_with_energy_grid(ctx, "lp_rebind")) != LP_OK) return st;
     if (capacity < ctx->cfg.np || capacity > 0xffffffffll) return fail(ctx, LP_ERR_INVALID_ARG, "capacity below the particle count or >= 2^32");
     if (capacity > 0 && (!x || !y || !z || !id || !chi)) return fail(ctx, LP_ERR_INVALID_ARG, "NULL particle array");
     if (reinterpret_cast<uintptr_t>(chi) % 16) return fail(ctx, LP_ERR_INVALID_ARG, "chi not 16-byte aligned");
@@ -848,7 +859,7 @@ lp_status lp_current_particles(const lp_ctx *ctx, double **x, double **y, double
 lp_status lp_migrate_record_bytes(const lp_ctx *ctx, size_t *bytes)
 {
     if (!ctx || !bytes) return LP_ERR_INVALID_ARG;
-    *bytes = 32 + 8 * (size_t)ctx->cfg.nbins;
+    *bytes = 32 + 8 * (size_t)ctx->cfg.nbins + (ctx->eng ? 8 * ((size_t)ctx->cfg.nbins + 1) : 0);
     return LP_OK;
 }
 
@@ -856,8 +867,8 @@ lp_status lp_migrate_count(lp_ctx *ctx, int axis, double lo, double hi, int64_t 
 {
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
-    if ((st = not_with_energy_grid(ctx, "lp_migrate_count")) != LP_OK) return st;
     if (axis < 0 || axis > 2 || !n_left || !n_right || !(hi > lo)) return fail(ctx, LP_ERR_INVALID_ARG, "bad axis, interval or NULL output");
+    if ((st = grid_ok(ctx)) != LP_OK) return st;
     ctx->mig_stage = 0;
     *n_left = *n_right = 0;
     ctx->mig_left = ctx->mig_right = 0;
@@ -896,7 +907,7 @@ lp_status lp_migrate_pack(lp_ctx *ctx, void *buf_left, void *buf_right, void *st
         LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
         const lp_ctx::Set n = ctx->now();
         st = count(ctx, lp_launch_migrate_pack(ctx->at<unsigned long long>(ctx->lay.partial), nleave, ctx->at<uint32_t>(ctx->lay.idx_b),
-                                               n.x, n.y, n.z, n.id, n.chi, ctx->cfg.nbins, buf_left, buf_right, ctx->sm_count,
+                                               n.x, n.y, n.z, n.id, n.chi, ctx->eng, ctx->cfg.nbins, buf_left, buf_right, ctx->sm_count,
                                                static_cast<cudaStream_t>(stream)), "exchange pack kernel launch");
         if (st != LP_OK) return st;
     }
@@ -920,6 +931,7 @@ lp_status lp_migrate_unpack(lp_ctx *ctx, const void *from_left, int64_t n_from_l
     const long long grown = np + (nin > nholes ? nin - nholes : 0);
     if (grown > ctx->capacity)
         return fail(ctx, LP_ERR_WORKSPACE, "arrivals exceed the capacity of the particle arrays (lp_rebind to grow)");
+    if ((st = grid_ok(ctx)) != LP_OK) return st;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const lp_ctx::Set n = ctx->now();
@@ -928,7 +940,7 @@ lp_status lp_migrate_unpack(lp_ctx *ctx, const void *from_left, int64_t n_from_l
     if (rest) LP_CUDA(ctx, cudaMemsetAsync(flag, 0, (size_t)np * 4, s));
     if (nin > 0 || rest) {
         st = count(ctx, lp_launch_migrate_unpack(from_left, n_from_left, from_right, n_from_right, ctx->at<uint32_t>(ctx->lay.idx_a),
-                                                 nholes, np, n.x, n.y, n.z, n.id, n.chi, ctx->cfg.nbins, rest ? flag : nullptr,
+                                                 nholes, np, n.x, n.y, n.z, n.id, n.chi, ctx->eng, ctx->cfg.nbins, rest ? flag : nullptr,
                                                  ctx->sm_count, s), "exchange unpack kernels launch");
         if (st != LP_OK) return st;
     }
@@ -953,7 +965,23 @@ lp_status lp_bind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch)
     if (eng && ctx->cur != 0) return fail(ctx, LP_ERR_STATE, "bind the energy grid while the state is in the bound arrays");
     ctx->eng = eng;
     ctx->eng_scratch = eng_scratch;
+    ctx->eng_capacity = eng ? ctx->capacity : 0;
     ctx->spectra_done = false;
+    return LP_OK;
+}
+
+lp_status lp_rebind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch, void *stream)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    if (!ctx->eng) return fail(ctx, LP_ERR_STATE, "no energy grid bound (lp_bind_energy_grid)");
+    if (!eng) return fail(ctx, LP_ERR_INVALID_ARG, "eng is NULL");
+    LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    if (ctx->cfg.np > 0 && eng != ctx->eng)
+        LP_CUDA(ctx, cudaMemcpyAsync(eng, ctx->eng, (size_t)ctx->cfg.np * (ctx->cfg.nbins + 1) * 8, cudaMemcpyDeviceToDevice,
+                                     static_cast<cudaStream_t>(stream)));
+    ctx->eng = eng;
+    ctx->eng_scratch = eng_scratch;
+    ctx->eng_capacity = ctx->capacity;
     return LP_OK;
 }
 
@@ -961,7 +989,7 @@ lp_status lp_init_energy_grid(lp_ctx *ctx, int64_t first, int64_t count_, void *
 {
     if (!ctx) return LP_ERR_INVALID_ARG;
     if (!ctx->eng) return fail(ctx, LP_ERR_STATE, "no energy grid bound (lp_bind_energy_grid)");
-    if (first < 0 || count_ < 0 || first + count_ > ctx->capacity) return fail(ctx, LP_ERR_INVALID_ARG, "rows outside the capacity");
+    if (first < 0 || count_ < 0 || first + count_ > ctx->eng_capacity) return fail(ctx, LP_ERR_INVALID_ARG, "rows outside the grid arrays");
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     return count(ctx, lp_launch_moving_init(ctx->tab, ctx->cfg.nbins, ctx->eng, first, count_, static_cast<cudaStream_t>(stream)),
                  "lp_moving_init_kernel launch");

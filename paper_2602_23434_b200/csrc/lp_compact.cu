@@ -118,7 +118,8 @@ lp_holes_fillers_kernel(const int32_t *__restrict__ flag, const uint32_t *__rest
 __global__ void __launch_bounds__(kThreads)
 lp_fill_holes_kernel(const unsigned long long *__restrict__ counts, const uint32_t *__restrict__ hole,
                      const uint32_t *__restrict__ filler, double *__restrict__ x, double *__restrict__ y,
-                     double *__restrict__ z, uint64_t *__restrict__ id, double *__restrict__ chi, int nbins)
+                     double *__restrict__ z, uint64_t *__restrict__ id, double *__restrict__ chi, int nbins,
+                     double *__restrict__ eng /*[np][nbins+1] or NULL*/)
 {
     const long long h = (long long)counts[1];
     const int lane = threadIdx.x & 31;
@@ -130,6 +131,8 @@ lp_fill_holes_kernel(const unsigned long long *__restrict__ counts, const uint32
         const double2 *src = reinterpret_cast<const double2 *>(chi + s * nbins);
         double2 *dst = reinterpret_cast<double2 *>(chi + d * nbins);
         for (int i = lane; i < nbins / 2; i += 32) dst[i] = src[i];
+        if (eng)            // the particle's energy-grid row (8-byte aligned only)
+            for (int i = lane; i <= nbins; i += 32) eng[d * (nbins + 1) + i] = eng[s * (nbins + 1) + i];
     }
 }
 
@@ -142,7 +145,7 @@ size_t lp_compact_block_elems(long long np) { return (size_t)blocks_for(np, kTil
 // counts: 2 x u64 on the device (N_del, H).  Returns kernels launched or -1.
 int lp_launch_compact(const int32_t *flag, long long np, int nbins, uint32_t *blk, uint32_t *rank, uint32_t *hole,
                       uint32_t *filler, unsigned long long *counts, double *x, double *y, double *z, uint64_t *id,
-                      double *chi, int sm_count, cudaStream_t s)
+                      double *chi, double *eng, int sm_count, cudaStream_t s)
 {
     const int nblocks = blocks_for(np, kTile);
     lp_flag_count_kernel<<<nblocks, kThreads, 0, s>>>(flag, np, blk);
@@ -153,6 +156,6 @@ int lp_launch_compact(const int32_t *flag, long long np, int nbins, uint32_t *bl
     const long long cap = (long long)sm_count * 8;
     if (fb > cap) fb = cap;
     if (fb < 1) fb = 1;
-    lp_fill_holes_kernel<<<(int)fb, kThreads, 0, s>>>(counts, hole, filler, x, y, z, id, chi, nbins);
+    lp_fill_holes_kernel<<<(int)fb, kThreads, 0, s>>>(counts, hole, filler, x, y, z, id, chi, nbins, eng);
     return ok() ? 5 : -1;
 }

@@ -107,7 +107,7 @@ int lp_launch_shock(const double *tab, const double *r, double q_r, double *chi,
 size_t lp_compact_block_elems(long long np);
 int lp_launch_compact(const int32_t *flag, long long np, int nbins, uint32_t *blk, uint32_t *rank, uint32_t *hole,
                       uint32_t *filler, unsigned long long *counts, double *x, double *y, double *z, uint64_t *id,
-                      double *chi, int sm_count, cudaStream_t s);
+                      double *chi, double *eng /*or NULL*/, int sm_count, cudaStream_t s);
 
 // particle exchange (lp_migrate.cu); counts = 2 x u64 on the device: n_left, n_right
 size_t lp_migrate_block_elems(long long np);
@@ -116,10 +116,12 @@ int lp_launch_migrate_count(const double *pos, long long np, double lo, double h
                             uint32_t *leaver, cudaStream_t s);
 int lp_launch_migrate_pack(const unsigned long long *counts, long long nleavers, const uint32_t *leaver,
                            const double *x, const double *y, const double *z, const uint64_t *id, const double *chi,
-                           int nbins, void *buf_left, void *buf_right, int sm_count, cudaStream_t s);
+                           const double *eng /*or NULL*/, int nbins, void *buf_left, void *buf_right, int sm_count,
+                           cudaStream_t s);
 int lp_launch_migrate_unpack(const void *in_left, long long n_in_left, const void *in_right, long long n_in_right,
                              const uint32_t *hole, long long nholes, long long np, double *x, double *y, double *z,
-                             uint64_t *id, double *chi, int nbins, int32_t *flag_rest, int sm_count, cudaStream_t s);
+                             uint64_t *id, double *chi, double *eng /*or NULL*/, int nbins, int32_t *flag_rest,
+                             int sm_count, cudaStream_t s);
 
 // sort: fills perm[n] = source index of the n-th particle in (key, id) order.
 struct LpSortBufs {

@@ -8,8 +8,9 @@
 //                     last particle when the holes are used up; holes that stay open are flagged for the
 //                     compaction of lp_compact.cu
 // A send buffer for n particles is laid out as arrays: x[n] | y[n] | z[n] | id[n] | chi[n][nbins]
-// (n * (32 + 8 nbins) bytes, 16-byte aligned base), so both sides of the copy are coalesced and the buffer
-// is what one NCCL send / NVLink peer copy moves.  sm_100a.
+// [| eng[n][nbins+1] when the particles carry an energy grid]  (n * lp_migrate_record_bytes bytes, 16-byte
+// aligned base), so both sides of the copy are coalesced and the buffer is what one NCCL send / NVLink peer copy
+// moves.  sm_100a.
 #include "lp_internal.h"
 
 namespace {
@@ -141,6 +142,7 @@ struct LpMigBuf {           // one send / receive buffer, as arrays
     double *x, *y, *z;
     uint64_t *id;
     double *chi;
+    double *eng;            // [n][nbins + 1] behind chi when the particles carry an energy grid
 };
 
 __device__ __forceinline__ LpMigBuf lp_mig_view(void *base, unsigned long long n, int nbins)
@@ -151,7 +153,7 @@ __device__ __forceinline__ LpMigBuf lp_mig_view(void *base, unsigned long long n
     b.z = b.y + n;
     b.id = reinterpret_cast<uint64_t *>(b.z + n);
     b.chi = reinterpret_cast<double *>(b.id + n);
-    (void)nbins;
+    b.eng = b.chi + n * (unsigned long long)nbins;
     return b;
 }
 
@@ -159,8 +161,8 @@ __device__ __forceinline__ LpMigBuf lp_mig_view(void *base, unsigned long long n
 __global__ void __launch_bounds__(kThreads)
 lp_mig_pack_kernel(const unsigned long long *__restrict__ counts, const uint32_t *__restrict__ leaver,
                    const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
-                   const uint64_t *__restrict__ id, const double *__restrict__ chi, int nbins,
-                   void *buf_left, void *buf_right)
+                   const uint64_t *__restrict__ id, const double *__restrict__ chi, const double *__restrict__ eng,
+                   int nbins, void *buf_left, void *buf_right)
 {
     const unsigned long long nl = counts[0], nr = counts[1];
     const LpMigBuf L = lp_mig_view(buf_left, nl, nbins), R = lp_mig_view(buf_right, nr, nbins);
@@ -176,6 +178,8 @@ lp_mig_pack_kernel(const unsigned long long *__restrict__ counts, const uint32_t
         const double2 *src = reinterpret_cast<const double2 *>(chi + s * nbins);
         double2 *dst = reinterpret_cast<double2 *>(B.chi + d * nbins);
         for (int i = lane; i < nbins / 2; i += 32) dst[i] = src[i];
+        if (eng)
+            for (int i = lane; i <= nbins; i += 32) B.eng[d * (nbins + 1) + i] = eng[s * (nbins + 1) + i];
     }
 }
 
@@ -184,7 +188,7 @@ __global__ void __launch_bounds__(kThreads)
 lp_mig_unpack_kernel(const void *in_left, long long n_in_left, const void *in_right, long long n_in_right,
                      const uint32_t *__restrict__ hole, long long nholes, long long np,
                      double *__restrict__ x, double *__restrict__ y, double *__restrict__ z,
-                     uint64_t *__restrict__ id, double *__restrict__ chi, int nbins)
+                     uint64_t *__restrict__ id, double *__restrict__ chi, double *__restrict__ eng, int nbins)
 {
     const LpMigBuf L = lp_mig_view(const_cast<void *>(in_left), (unsigned long long)n_in_left, nbins);
     const LpMigBuf R = lp_mig_view(const_cast<void *>(in_right), (unsigned long long)n_in_right, nbins);
@@ -200,6 +204,8 @@ lp_mig_unpack_kernel(const void *in_left, long long n_in_left, const void *in_ri
         const double2 *src = reinterpret_cast<const double2 *>(B.chi + s * nbins);
         double2 *dst = reinterpret_cast<double2 *>(chi + d * nbins);
         for (int i = lane; i < nbins / 2; i += 32) dst[i] = src[i];
+        if (eng)
+            for (int i = lane; i <= nbins; i += 32) eng[d * (nbins + 1) + i] = B.eng[s * (nbins + 1) + i];
     }
 }
 
@@ -230,19 +236,20 @@ int lp_launch_migrate_count(const double *pos, long long np, double lo, double h
 
 int lp_launch_migrate_pack(const unsigned long long *counts, long long nleavers, const uint32_t *leaver,
                            const double *x, const double *y, const double *z, const uint64_t *id, const double *chi,
-                           int nbins, void *buf_left, void *buf_right, int sm_count, cudaStream_t s)
+                           const double *eng, int nbins, void *buf_left, void *buf_right, int sm_count, cudaStream_t s)
 {
     long long blocks = (nleavers + kWarps - 1) / kWarps;
     const long long cap = (long long)sm_count * 8;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
-    lp_mig_pack_kernel<<<(int)blocks, kThreads, 0, s>>>(counts, leaver, x, y, z, id, chi, nbins, buf_left, buf_right);
+    lp_mig_pack_kernel<<<(int)blocks, kThreads, 0, s>>>(counts, leaver, x, y, z, id, chi, eng, nbins, buf_left, buf_right);
     return ok() ? 1 : -1;
 }
 
 int lp_launch_migrate_unpack(const void *in_left, long long n_in_left, const void *in_right, long long n_in_right,
                              const uint32_t *hole, long long nholes, long long np, double *x, double *y, double *z,
-                             uint64_t *id, double *chi, int nbins, int32_t *flag_rest, int sm_count, cudaStream_t s)
+                             uint64_t *id, double *chi, double *eng, int nbins, int32_t *flag_rest, int sm_count,
+                             cudaStream_t s)
 {
     int launches = 0;
     const long long nin = n_in_left + n_in_right;
@@ -251,7 +258,7 @@ int lp_launch_migrate_unpack(const void *in_left, long long n_in_left, const voi
         const long long cap = (long long)sm_count * 8;
         if (blocks > cap) blocks = cap;
         lp_mig_unpack_kernel<<<(int)blocks, kThreads, 0, s>>>(in_left, n_in_left, in_right, n_in_right, hole, nholes,
-                                                             np, x, y, z, id, chi, nbins);
+                                                             np, x, y, z, id, chi, eng, nbins);
         ++launches;
     }
     if (nin < nholes && flag_rest) {

@@ -20,6 +20,7 @@ class LP:
         self._bound = None            # the caller-side tensors x, y, z, id, chi (the bound arrays)
         self.capacity = cfg.np
         self.nsub = self.lost = None
+        self.eng = self._eng_scratch = None
         self._fields = None
 
     def _alloc_workspace(self, nbytes):
@@ -168,6 +169,13 @@ class LP:
         self.nsub = self.lost = None
         if any(had):
             self.bind_diag(*had)
+        if getattr(self, "eng", None) is not None:           # the energy grid follows: new arrays, rows copied over
+            shape = (capacity, nb + 1)
+            eng = torch.empty(shape, dtype=torch.float64, device=self.device)
+            scr = torch.empty(shape, dtype=torch.float64, device=self.device) if self._eng_scratch is not None else None
+            B.lp_rebind_energy_grid(self.ctx, eng.data_ptr(), scr.data_ptr() if scr is not None else None, self.stream)
+            self._retired = self._retired + (self.eng, self._eng_scratch)
+            self.eng, self._eng_scratch = eng, scr
 
     def reserve(self, n_new, e=18):
         """Room for n_new more particles behind the current ones (Listing 2's Reserve): when the capacity does

@@ -103,10 +103,13 @@ def test_moving_grid_synchrotron_law_and_unsupported_calls():
     eng = host(lp.eng)
     assert np.allclose(eng, (E / (1.0 + cr * E * dt * 100))[None, :], rtol=1e-12, atol=0)
     with pytest.raises(B.LPError) as e:
-        lp.compact(torch.zeros(w.np, dtype=torch.int32, device=lp.device))
+        lp.shock_update(torch.full((w.np,), 2.0, dtype=torch.float64, device=lp.device))
     assert e.value.status == B.LP_ERR_UNSUPPORTED
-    with pytest.raises(B.LPError):
-        lp.migrate_count(0, -1.0, 0.0)
+    hx = torch.zeros(w.np, dtype=torch.float64).pin_memory()
+    with pytest.raises(B.LPError) as e:
+        lp.step_host(dt, hx, hx, hx, torch.zeros(w.np, dtype=torch.int64).pin_memory(),
+                     torch.zeros((w.np, w.nbins), dtype=torch.float64).pin_memory())
+    assert e.value.status == B.LP_ERR_UNSUPPORTED
     lp.unbind_energy_grid()
     lp.step(dt)                                  # back on the fixed bins
     assert lp.diag()["max_substeps"] >= 1
@@ -123,3 +126,51 @@ def test_sort_without_scratch_is_refused():
     with pytest.raises(B.LPError) as e:
         lp.sort()
     assert e.value.status == B.LP_ERR_STATE
+
+
+def test_grid_rows_travel_with_their_particles():
+    """Compaction, the exchange and growth move the energy-grid rows with the particles: the oracle's
+    orc_compact / orc_migrate_* are run on rows that are chi and eng side by side (they move "every parameter"
+    of a particle, whatever its width)."""
+    rng = np.random.default_rng(9)
+    n, nb = 3000, 32
+    w = I.workload(3).scaled(n=12, np=n, nbins=nb, sort_every=0)
+    lp, prm, f_np, st = setup(w)
+    for _ in range(2):                                   # give every particle its own grid
+        lp.step(w.dt)
+        st = oracle_step(prm, f_np, st, w.dt, False)
+    check(lp, st)
+    x, y, z, pid, chi, eng = st
+    wide = np.concatenate([chi, eng], axis=1)            # [n][2 nb + 1]
+
+    def split(rows):
+        return rows[:, :nb], rows[:, nb:]
+
+    # deletion with hole filling
+    flag = (rng.uniform(size=n) < 0.3).astype(np.int32)
+    n1 = lp.compact(torch.from_numpy(flag).to(lp.device))
+    x, y, z, pid, wide = orc.compact(flag, x, y, z, pid, wide)
+    chi, eng = split(wide)
+    check(lp, [x, y, z, pid, chi, eng])
+    assert n1 == x.shape[0]
+
+    # one directional exchange: this rank owns x in [-1, 0.2); what leaves comes back as "arrivals" from the
+    # other side with shifted ids (a stand-in for the neighbour)
+    nl, nr = lp.migrate_count(0, -1.0, 0.2)
+    assert B.lp_migrate_record_bytes(lp.ctx) == 32 + 8 * nb + 8 * (nb + 1)
+    bl, br = lp.migrate_pack(nl, nr)
+    dest, holes, left, right = orc.migrate_pack(0, -1.0, 0.2, -1.0, 1.0, 1, x, y, z, pid, wide)
+    assert (nl, nr) == (left[0].shape[0], right[0].shape[0]) and nr > 0
+    raw = br.cpu().numpy()[: nr * (32 + 8 * nb + 8 * (nb + 1))]
+    d = raw.view(np.float64)
+    assert np.array_equal(d[:nr], right[0]) and np.array_equal(raw.view(np.uint64)[3 * nr:4 * nr], right[3])
+    assert_chi_close(d[4 * nr:4 * nr + nr * nb].reshape(nr, nb), right[4][:, :nb])       # (spectra: 1e-10, not bits)
+    assert_chi_close(d[4 * nr + nr * nb:].reshape(nr, nb + 1), right[4][:, nb:], what="eng")
+    lp.reserve(nr, e=8)                                  # grow between pack and unpack: the grid follows
+    n2 = lp.migrate_unpack(br, nr, bl, nl)               # the leavers come back in (right buffer first)
+    x, y, z, pid, wide = orc.migrate_unpack(holes, right, left, x, y, z, pid, wide)
+    chi, eng = split(wide)
+    assert n2 == x.shape[0]
+    check(lp, [x, y, z, pid, chi, eng])
+    lp.step(w.dt)                                        # and the moving-grid update goes on
+    check(lp, oracle_step(prm, f_np, [x, y, z, pid, chi, eng], w.dt, False))
