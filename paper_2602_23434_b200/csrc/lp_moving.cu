@@ -63,8 +63,11 @@ __device__ __forceinline__ double2 lp_moving_coef(const LpMovingArgs &A, long lo
     return make_double2(alpha, beta);
 }
 
+// Resident blocks per SM: six at N_b <= 64 (84 registers; the per-particle phase is a larger share of a short
+// row and needs more blocks to hide behind), four above (measured: 64 bins 0.806 -> 0.828 of the copy bandwidth
+// with six, 128 / 256 bins 0.89 / 0.90 -> 0.875 / 0.865; eight blocks or eight rows in flight lose everywhere).
 template <int NB>
-__global__ void __launch_bounds__(kThreads) lp_moving_kernel(LpMovingArgs A)
+__global__ void __launch_bounds__(kThreads, NB <= 64 ? 6 : 4) lp_moving_kernel(LpMovingArgs A)
 {
     constexpr int G = NB < 32 ? NB : 32;         // lanes per row
     constexpr int PPW = 32 / G;                  // rows a warp holds side by side
