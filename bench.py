@@ -581,14 +581,14 @@ def run_ours(args):
     state_bytes = (32 if staged else 48) * w.np
     if args.energy_grid:        # moving grid: chi and the N_b + 1 edges in and out; x, y, z, rho_old in
         rows_bytes = 16 * (2 * w.nbins + 1) * w.np
-        state_bytes = 32 * w.np
+        state_bytes = (32 if staged else 48) * w.np
     grid_bytes = 56 * min(w.n ** 3, 8 * w.np)
     alg_bytes = rows_bytes + state_bytes + grid_bytes
     spec_avg_ms = spec_ms / max(spec_n, 1)
     achieved = alg_bytes / (spec_avg_ms * 1e-3) / 1e9 if spec_n else None
     kname = "lp_spectral_%s_kernel<%d,0,%d>" % ("bulk" if w.nbins <= 256 else "direct", w.nbins, 0 if staged else 1)
     if args.energy_grid:
-        kname = "lp_moving_kernel<%d>" % w.nbins
+        kname = "lp_moving_kernel<%d,%d>" % (w.nbins, 0 if staged else 1)
     # The secondary bound ("report both fractions"): fp64 arithmetic.  Algorithmic flops of a row:
     # per bin and substep the donor-cell update is 3 multiply-adds (6 flop), plus 12 flop per bin once for the
     # edge velocities and the update coefficients; the substep total is the kernel's own count (lp_get_diag).

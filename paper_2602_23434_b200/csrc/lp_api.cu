@@ -270,14 +270,15 @@ lp_status not_with_energy_grid(lp_ctx *c, const char *what)
 }
 
 // spectral update on the per-particle moving grid (lp_moving.cu)
-lp_status do_moving(lp_ctx *c, double dt, cudaStream_t s)
+lp_status do_moving(lp_ctx *c, double dt, bool fused, cudaStream_t s)
 {
     lp_status gs = grid_ok(c);
     if (gs != LP_OK) return gs;
     const lp_ctx::Set n = c->now();
     const bool rec = c->timing && c->ev_used + 2 <= c->ev.size();
     if (rec) LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used], s));
-    lp_status st = count(c, lp_launch_moving(c->geom, c->cells(), n.x, n.y, n.z, c->at<double>(c->lay.rho_old), c->eng, n.chi,
+    lp_status st = count(c, lp_launch_moving(c->geom, c->cells(), n.x, n.y, n.z, c->at<double>(c->lay.rho_old),
+                                             c->at<int32_t>(c->lay.status), fused, c->eng, n.chi,
                                              c->at<int32_t>(c->lay.nsub), c->nsub_user, c->cfg.np, c->cfg.nbins, dt,
                                              c->cfg.kappa, c->cfg.u_rad, c->sm_count, s), "lp_moving_kernel launch");
     if (rec) {
@@ -287,6 +288,7 @@ lp_status do_moving(lp_ctx *c, double dt, cudaStream_t s)
     if (st == LP_OK) {
         c->spectra_done = true;
         c->stage0_done = false; c->rk3_next = 0; c->push_done = false;
+        if (fused) { c->status_valid = true; c->mig_stage = 0; }
     }
     return st;
 }
@@ -690,7 +692,7 @@ lp_status lp_spectral_update(lp_ctx *ctx, double dt, void *stream)
         return fail(ctx, LP_ERR_STATE, "lp_spectral_update needs the push finished (lp_push stage 1 / lp_push_rk3 stage 2)");
     if (ctx->cfg.np == 0) return LP_OK;
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    if (ctx->eng) return do_moving(ctx, dt, static_cast<cudaStream_t>(stream));
+    if (ctx->eng) return do_moving(ctx, dt, false, static_cast<cudaStream_t>(stream));
     return do_spectral(ctx, dt, io_in_place(ctx), false, static_cast<cudaStream_t>(stream));
 }
 
@@ -1005,14 +1007,9 @@ lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const bool sort_now = ctx->cfg.sort_every > 0 && (ctx->steps - 1) % ctx->cfg.sort_every == 0;
     if (ctx->eng) {
-        // moving energy grid: the staged kernels in a row (sort, push 0, push 1, moving-grid update)
+        // moving energy grid: sort when due, then one kernel that does both push stages and the grid update
         if (sort_now && (st = do_sort(ctx, true, nullptr, s)) != LP_OK) return st;
-        LpPushArgs a = push_args(ctx, dt);
-        if ((st = count(ctx, lp_launch_push0(a, s), "lp_push0_kernel launch")) != LP_OK) return st;
-        if ((st = count(ctx, lp_launch_push1(a, s), "lp_push1_kernel launch")) != LP_OK) return st;
-        ctx->status_valid = true;
-        ctx->mig_stage = 0;
-        return do_moving(ctx, dt, s);
+        return do_moving(ctx, dt, true, s);
     }
     SpectralIO io = io_in_place(ctx);
     bool flip = false;

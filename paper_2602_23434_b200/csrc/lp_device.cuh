@@ -197,6 +197,71 @@ __device__ __forceinline__ double lp_wrap_pos(double x, double lo, double hi, do
     return x >= hi ? lo : x;
 }
 
+// The per-particle part every spectral kernel starts with: [FUSED: the two push stages a5, a6 (same arithmetic as
+// lp_push0/1_kernel), run on the same thread so that k1, x*, rho_old never leave registers;
+// x^{n+1} and the outside-box status are written], then the gathers at x^{n+1} and the coefficients a7:
+// dtau = dt/gamma_g, c_r (Eq. 4), a = (1/3) div_mu u^mu through continuity
+// (PAPER.md:105).  Not FUSED: (px, py, pz) is x^{n+1} and rho_old comes from push stage 0.
+template <bool FUSED>
+__device__ __forceinline__ void lp_particle_coefficients(const LpGeom &g, const LpCells &cells, double dt, double kappa,
+                                                         double u_rad, double *x, double *y, double *z, int32_t *status,
+                                                         const double *rho_old_in, long long p, double px, double py,
+                                                         double pz, double &a, double &cr, double &dtau)
+{
+    LpStencil st;
+    LpCornersA ka;
+    LpCornersB kb;
+    double rho_old;
+    double qa[4], qb[3];
+    if (FUSED) {
+        lp_stencil(g, px, py, pz, st);
+        ka.load(cells, st);
+        // B is gathered last, at x^{n+1}, whose cells are these or their neighbours.  With split record arrays
+        // start the B halves of the four x-lower corners on their way from DRAM to L2 now (every prefetch is an
+        // L1 request, and eight cost more than they save); in a 64-byte record the B half arrives in L2 with A.
+        if (cells.stride == 1) {
+#pragma unroll
+            for (int n = 0; n < 8; n += 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(cells.recB + st.c[n]));
+        }
+        ka.gather4(st, qa);                                 // k1 = v(x^n), rho_old = rho(x^n)
+        rho_old = qa[3];
+        lp_stencil(g, __dadd_rn(px, __dmul_rn(dt, qa[0])), __dadd_rn(py, __dmul_rn(dt, qa[1])),
+                   __dadd_rn(pz, __dmul_rn(dt, qa[2])), st);
+        double k2[3];
+        ka.update(cells, st);
+        ka.gather3(st, k2);
+        const double hdt = __dmul_rn(0.5, dt);
+        double pos[3] = { px, py, pz };
+        int stt = 0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            double xn = __dadd_rn(pos[d], __dmul_rn(hdt, __dadd_rn(qa[d], k2[d])));
+            if (g.per[d]) xn = lp_wrap_pos(xn, g.xlo[d], g.xhi[d], g.len[d]);
+            else if (xn < g.xlo[d] || xn >= g.xhi[d]) stt |= (1 << d);
+            pos[d] = xn;
+        }
+        px = pos[0]; py = pos[1]; pz = pos[2];
+        __stcs(x + p, px); __stcs(y + p, py); __stcs(z + p, pz);
+        __stcs(status + p, stt);
+        lp_stencil(g, px, py, pz, st);
+        ka.update(cells, st);
+    } else {
+        rho_old = rho_old_in[p];
+        lp_stencil(g, px, py, pz, st);
+        ka.load(cells, st);
+    }
+    ka.gather4(st, qa);
+    kb.load(cells, st);       // (issued after A is consumed: holding both record sets spills registers)
+    kb.gather3(st, qb);
+    // gamma_g, dtau, c_r (Eq. 4), a (continuity)
+    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(qa[0], qa[0]), __dmul_rn(qa[1], qa[1])), __dmul_rn(qa[2], qa[2]));
+    const double b2 = __dadd_rn(__dadd_rn(__dmul_rn(qb[0], qb[0]), __dmul_rn(qb[1], qb[1])), __dmul_rn(qb[2], qb[2]));
+    const double gam = __ddiv_rn(1.0, __dsqrt_rn(__dsub_rn(1.0, v2)));
+    dtau = __ddiv_rn(dt, gam);
+    cr = __dmul_rn(kappa, __dadd_rn(__dmul_rn(0.5, b2), u_rad));
+    a = __ddiv_rn(-log(__ddiv_rn(qa[3], rho_old)), __dmul_rn(3.0, dtau));
+}
+
 // Row <-> lane slices through a per-warp staging buffer, for M >= 8 bins per lane.  A lane's slice is M*8
 // bytes of the row, so loading it directly makes every 16-byte load instruction of the warp touch 32
 // different 128-byte lines (measured at M = 16: ~500 L1 wavefronts per row, the kernel's bound after the

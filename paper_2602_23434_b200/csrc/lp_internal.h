@@ -156,9 +156,10 @@ int lp_launch_permute_rows(const uint32_t *perm, const double *src, double *dst,
 int lp_launch_max_u64(const uint64_t *v, long long np, unsigned long long *out, cudaStream_t s);
 
 // moving energy grid (lp_moving.cu)
-int lp_launch_moving(const LpGeom &g, const LpCells &cells, const double *x, const double *y, const double *z,
-                     const double *rho_old, double *eng, double *chi, int32_t *nsub_ws, int32_t *nsub_user, long long np,
-                     int nbins, double dt, double kappa, double u_rad, int sm_count, cudaStream_t s);
+// fused: the kernel also does both push stages (x^n in x, y, z; x^{n+1} and status written), rho_old unused
+int lp_launch_moving(const LpGeom &g, const LpCells &cells, double *x, double *y, double *z, const double *rho_old,
+                     int32_t *status, bool fused, double *eng, double *chi, int32_t *nsub_ws, int32_t *nsub_user,
+                     long long np, int nbins, double dt, double kappa, double u_rad, int sm_count, cudaStream_t s);
 int lp_launch_moving_init(const double *tab, int nbins, double *eng, long long first, long long count, cudaStream_t s);
 int lp_launch_permute_rows8(const uint32_t *perm, const double *src, double *dst, long long np, int len, cudaStream_t s);
 

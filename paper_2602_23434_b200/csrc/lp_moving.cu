@@ -9,6 +9,7 @@
 // pure stream of 16 (2 N_b + 1) bytes per particle behind a per-particle phase (gather, coefficients) that is
 // the same as the fixed-grid kernel's (lp_spectral.cu).
 //
+// Staged (lp_spectral_update) or fused with the two push stages (lp_step), like the fixed-grid kernel.
 // A block takes 128 particles at a time: phase 1 with one thread per particle leaves (alpha, beta) in shared
 // memory, then its four warps stream the 128 rows, RI rows per warp in flight.  Several blocks are resident
 // per SM, so the latency-bound phase of one overlaps the stream of the others.  sm_100a.
@@ -23,8 +24,9 @@ constexpr int kWarps = kThreads / 32;
 struct LpMovingArgs {
     LpGeom g;
     LpCells cells;
-    const double *x, *y, *z;     // x^{n+1}
-    const double *rho_old;       // from push stage 0
+    double *x, *y, *z;           // staged: x^{n+1} (read only); fused: x^n in, x^{n+1} out
+    const double *rho_old;       // staged: from push stage 0
+    int32_t *status;             // fused: outside-box flags [np]
     double *eng;                 // [np][nbins + 1] in/out
     double *chi;                 // [np][nbins] in/out
     int32_t *nsub_ws;            // [np]: 1 (one exact step per particle)
@@ -33,29 +35,14 @@ struct LpMovingArgs {
     double dt, kappa, u_rad;
 };
 
-// per-particle phase: (alpha, beta) of the step  (a7 of DESIGN.md section 1, then reading E2)
+// per-particle phase: [FUSED: push stages a5, a6,] coefficients a7, then (alpha, beta) of the step (reading E2)
+template <bool FUSED>
 __device__ __forceinline__ double2 lp_moving_coef(const LpMovingArgs &A, long long p)
 {
     const double px = A.x[p], py = A.y[p], pz = A.z[p];
-    LpStencil st;
-    lp_stencil(A.g, px, py, pz, st);
-    double qa[4], qb[3];
-    {
-        LpCornersA ka;
-        ka.load(A.cells, st);
-        ka.gather4(st, qa);
-    }
-    {
-        LpCornersB kb;
-        kb.load(A.cells, st);
-        kb.gather3(st, qb);
-    }
-    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(qa[0], qa[0]), __dmul_rn(qa[1], qa[1])), __dmul_rn(qa[2], qa[2]));
-    const double b2 = __dadd_rn(__dadd_rn(__dmul_rn(qb[0], qb[0]), __dmul_rn(qb[1], qb[1])), __dmul_rn(qb[2], qb[2]));
-    const double gam = __ddiv_rn(1.0, __dsqrt_rn(__dsub_rn(1.0, v2)));
-    const double dtau = __ddiv_rn(A.dt, gam);
-    const double cr = __dmul_rn(A.kappa, __dadd_rn(__dmul_rn(0.5, b2), A.u_rad));
-    const double a = __ddiv_rn(-log(__ddiv_rn(qa[3], A.rho_old[p])), __dmul_rn(3.0, dtau));
+    double a, cr, dtau;
+    lp_particle_coefficients<FUSED>(A.g, A.cells, A.dt, A.kappa, A.u_rad, A.x, A.y, A.z, A.status, A.rho_old, p, px, py, pz,
+                                    a, cr, dtau);
     const double s = __dmul_rn(a, dtau);
     const double alpha = exp(-s);
     const double crt = __dmul_rn(cr, dtau);
@@ -63,11 +50,13 @@ __device__ __forceinline__ double2 lp_moving_coef(const LpMovingArgs &A, long lo
     return make_double2(alpha, beta);
 }
 
-// Resident blocks per SM: six at N_b <= 64 (84 registers; the per-particle phase is a larger share of a short
-// row and needs more blocks to hide behind), four above (measured: 64 bins 0.806 -> 0.828 of the copy bandwidth
-// with six, 128 / 256 bins 0.89 / 0.90 -> 0.875 / 0.865; eight blocks or eight rows in flight lose everywhere).
-template <int NB>
-__global__ void __launch_bounds__(kThreads, NB <= 64 ? 6 : 4) lp_moving_kernel(LpMovingArgs A)
+// Resident blocks per SM, staged kernel: six at N_b <= 64 (84 registers; the per-particle phase is a larger share
+// of a short row and needs more blocks to hide behind), four above (measured: 64 bins 0.806 -> 0.828 of the copy
+// bandwidth with six, 128 / 256 bins 0.89 / 0.90 -> 0.875 / 0.865; eight blocks or eight rows in flight lose
+// everywhere).  The fused kernel (push stages in the per-particle phase: three stencils, the corner records kept
+// in registers between them) gets four.
+template <int NB, bool FUSED>
+__global__ void __launch_bounds__(kThreads, (NB <= 64 && !FUSED) ? 6 : 4) lp_moving_kernel(LpMovingArgs A)
 {
     constexpr int G = NB < 32 ? NB : 32;         // lanes per row
     constexpr int PPW = 32 / G;                  // rows a warp holds side by side
@@ -87,7 +76,7 @@ __global__ void __launch_bounds__(kThreads, NB <= 64 ? 6 : 4) lp_moving_kernel(L
             const long long p = base + threadIdx.x;
             double2 ab = make_double2(1.0, 0.0);
             if (p < A.np) {
-                ab = lp_moving_coef(A, p);
+                ab = lp_moving_coef<FUSED>(A, p);
                 __stcs(A.nsub_ws + p, 1);
                 if (A.nsub_user) __stcs(A.nsub_user + p, 1);
             }
@@ -168,41 +157,48 @@ lp_permute_rows8_kernel(const uint32_t *__restrict__ perm, const double *__restr
     }
 }
 
-template <int NB>
-int launch(const LpMovingArgs &a, int sm_count, cudaStream_t s)
+template <int NB, bool FUSED>
+int launch_mode(const LpMovingArgs &a, int sm_count, cudaStream_t s)
 {
     int per_sm = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_moving_kernel<NB>, kThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_moving_kernel<NB, FUSED>, kThreads, 0);
     if (per_sm < 1) per_sm = 1;
     const long long want = (a.np + kThreads - 1) / kThreads;
     const long long cap = (long long)sm_count * per_sm;
     int blocks = (int)(want < cap ? want : cap);
     if (blocks < 1) blocks = 1;
-    lp_moving_kernel<NB><<<blocks, kThreads, 0, s>>>(a);
+    lp_moving_kernel<NB, FUSED><<<blocks, kThreads, 0, s>>>(a);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+template <int NB>
+int launch(const LpMovingArgs &a, bool fused, int sm_count, cudaStream_t s)
+{
+    return fused ? launch_mode<NB, true>(a, sm_count, s) : launch_mode<NB, false>(a, sm_count, s);
 }
 
 }  // namespace
 
-int lp_launch_moving(const LpGeom &g, const LpCells &cells, const double *x, const double *y, const double *z,
-                     const double *rho_old, double *eng, double *chi, int32_t *nsub_ws, int32_t *nsub_user, long long np,
-                     int nbins, double dt, double kappa, double u_rad, int sm_count, cudaStream_t s)
+int lp_launch_moving(const LpGeom &g, const LpCells &cells, double *x, double *y, double *z, const double *rho_old,
+                     int32_t *status, bool fused, double *eng, double *chi, int32_t *nsub_ws, int32_t *nsub_user,
+                     long long np, int nbins, double dt, double kappa, double u_rad, int sm_count, cudaStream_t s)
 {
     LpMovingArgs a;
     a.g = g; a.cells = cells;
     a.x = x; a.y = y; a.z = z;
     a.rho_old = rho_old;
+    a.status = status;
     a.eng = eng; a.chi = chi;
     a.nsub_ws = nsub_ws; a.nsub_user = nsub_user;
     a.np = np;
     a.dt = dt; a.kappa = kappa; a.u_rad = u_rad;
     switch (nbins) {
-    case 16:  return launch<16>(a, sm_count, s);
-    case 32:  return launch<32>(a, sm_count, s);
-    case 64:  return launch<64>(a, sm_count, s);
-    case 128: return launch<128>(a, sm_count, s);
-    case 256: return launch<256>(a, sm_count, s);
-    case 512: return launch<512>(a, sm_count, s);
+    case 16:  return launch<16>(a, fused, sm_count, s);
+    case 32:  return launch<32>(a, fused, sm_count, s);
+    case 64:  return launch<64>(a, fused, sm_count, s);
+    case 128: return launch<128>(a, fused, sm_count, s);
+    case 256: return launch<256>(a, fused, sm_count, s);
+    case 512: return launch<512>(a, fused, sm_count, s);
     default:  return -1;
     }
 }

@@ -46,58 +46,9 @@ template <int NB, bool FUSED>
 __device__ __forceinline__ void lp_phase1(const LpSpectralArgs &A, long long p, double px, double py, double pz,
                                           const double *sE, const double *sR, LpCoef &c, int &ns_signed)
 {
-    LpStencil st;
-    LpCornersA ka;
-    LpCornersB kb;
-    double rho_old;
-    double qa[4], qb[3];
-    if (FUSED) {
-        lp_stencil(A.g, px, py, pz, st);
-        ka.load(A.cells, st);
-        // B is gathered last, at x^{n+1}, whose cells are these or their neighbours.  With split record arrays
-        // start the B halves of the four x-lower corners on their way from DRAM to L2 now (every prefetch is an
-        // L1 request, and eight cost more than they save); in a 64-byte record the B half arrives in L2 with A.
-        if (A.cells.stride == 1) {
-#pragma unroll
-            for (int n = 0; n < 8; n += 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.cells.recB + st.c[n]));
-        }
-        ka.gather4(st, qa);                                 // k1 = v(x^n), rho_old = rho(x^n)
-        rho_old = qa[3];
-        lp_stencil(A.g, __dadd_rn(px, __dmul_rn(A.dt, qa[0])), __dadd_rn(py, __dmul_rn(A.dt, qa[1])),
-                   __dadd_rn(pz, __dmul_rn(A.dt, qa[2])), st);
-        double k2[3];
-        ka.update(A.cells, st);
-        ka.gather3(st, k2);
-        const double hdt = __dmul_rn(0.5, A.dt);
-        double pos[3] = { px, py, pz };
-        int stt = 0;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            double xn = __dadd_rn(pos[d], __dmul_rn(hdt, __dadd_rn(qa[d], k2[d])));
-            if (A.g.per[d]) xn = lp_wrap_pos(xn, A.g.xlo[d], A.g.xhi[d], A.g.len[d]);
-            else if (xn < A.g.xlo[d] || xn >= A.g.xhi[d]) stt |= (1 << d);
-            pos[d] = xn;
-        }
-        px = pos[0]; py = pos[1]; pz = pos[2];
-        __stcs(A.x + p, px); __stcs(A.y + p, py); __stcs(A.z + p, pz);
-        __stcs(A.status + p, stt);
-        lp_stencil(A.g, px, py, pz, st);
-        ka.update(A.cells, st);
-    } else {
-        rho_old = A.rho_old[p];
-        lp_stencil(A.g, px, py, pz, st);
-        ka.load(A.cells, st);
-    }
-    ka.gather4(st, qa);
-    kb.load(A.cells, st);       // (issued after A is consumed: holding both record sets spills registers)
-    kb.gather3(st, qb);
-    // gamma_g, dtau, c_r (Eq. 4), a (continuity)
-    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(qa[0], qa[0]), __dmul_rn(qa[1], qa[1])), __dmul_rn(qa[2], qa[2]));
-    const double b2 = __dadd_rn(__dadd_rn(__dmul_rn(qb[0], qb[0]), __dmul_rn(qb[1], qb[1])), __dmul_rn(qb[2], qb[2]));
-    const double gam = __ddiv_rn(1.0, __dsqrt_rn(__dsub_rn(1.0, v2)));
-    const double dtau = __ddiv_rn(A.dt, gam);
-    const double cr = __dmul_rn(A.kappa, __dadd_rn(__dmul_rn(0.5, b2), A.u_rad));
-    const double a = __ddiv_rn(-log(__ddiv_rn(qa[3], rho_old)), __dmul_rn(3.0, dtau));
+    double a, cr, dtau;
+    lp_particle_coefficients<FUSED>(A.g, A.cells, A.dt, A.kappa, A.u_rad, A.x, A.y, A.z, A.status, A.rho_old, p, px, py, pz,
+                                    a, cr, dtau);
 
     // lambda = max_i outflow_i.  On the library's log-spaced table the maximum sits in the first or the
     // last bin up to the rounding noise of E/dE (LpLamCand::margin, >= 1e-12), so those two bins decide n_sub
