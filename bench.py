@@ -375,7 +375,7 @@ def run_ours(args):
         # time-dependent fields (reading R18): the sets for every step boundary are made before the timed
         # region, lp_set_fields (the repack kernel) runs inside it, as in the paper's step
         import lp_inputs as I
-        field_sets = [I.make_fields(w, t=k * dt, device=dev) for k in range(total_steps + 1)]
+        field_sets = [I.make_fields(w, t=k * dt, device=dev) for k in range(total_steps + 2)]      # (+1: the histogram step)
         field_at = lambda k: field_sets[k]
 
     def barrier():
@@ -459,6 +459,17 @@ def run_ours(args):
                "median_value": aggregate_rate(world, w.np, args.steps, med[0] * 1e-3),
                "dominant_kernel_ms": [p_[1] / max(p_[2], 1) for p_ in passes],
                "clocks_after_first_pass": clocks2}
+
+    # ---- n_sub histogram of one more step; binding n_sub alone keeps the kernel instantiation
+    nsub_hist = None
+    if not args.energy_grid:
+        lp.bind_diag(nsub=True, lost=False)
+        one_step()
+        ns = lp.nsub[: w.np].abs().to(torch.int64)
+        edges = [1, 2, 3, 5, 9, 17, 33, 65, 129, 1 << 30]
+        counts = [int(((ns >= lo) & (ns < hi)).sum().item()) for lo, hi in zip(edges[:-1], edges[1:])]
+        nsub_hist = {"bins": ["1", "2", "3-4", "5-8", "9-16", "17-32", "33-64", "65-128", ">128"], "particles": counts}
+        lp.bind_diag(nsub=False, lost=False)
 
     # ---- shock-crossing update (NEXT-1), timed alone on the resident state
     shock = None
@@ -630,7 +641,7 @@ def run_ours(args):
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
            "parity_checked": parity, "repeats": repeats,
            "diag": {"mean_substeps": d["sum_substeps"] / max(1, d["np"]), "max_substeps": d["max_substeps"],
-                    "sorts_total": d["sorts"]}}
+                    "sorts_total": d["sorts"], "nsub_histogram": nsub_hist}}
     if compact is not None:
         out["compact"] = compact
     if migrate is not None:
