@@ -226,8 +226,8 @@ LP_API lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_
  * keeps its number, chi_i' = chi_i dE_i / dE_i': exact for frozen coefficients, no CFL limit, no substeps, no
  * numerical diffusion, nothing lost through the ends.
  *   lp_bind_energy_grid  eng [capacity][nbins+1] (device, caller-owned, updated in place) switches the context to the
- *                        moving grid: lp_spectral_update and lp_step use it (lp_step then runs the staged kernels in a
- *                        row), n_sub reads 1, lp_get_diag's number uses the particle's own widths.  eng_scratch: a
+ *                        moving grid: lp_spectral_update and lp_step use it (lp_step stays one fused kernel; a re-sort
+ *                        step permutes the rows in a pass of its own), n_sub reads 1, lp_get_diag's number uses the particle's own widths.  eng_scratch: a
  *                        second array of the same size through which a sort moves the rows (NULL: sorts return
  *                        LP_ERR_STATE).  eng = NULL switches back to the fixed bins.
  *   lp_init_energy_grid  rows [first, first + count) <- the fixed table's edges (the grid every particle starts on).
