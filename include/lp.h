@@ -226,8 +226,7 @@ LP_API lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_
  * keeps its number, chi_i' = chi_i dE_i / dE_i': exact for frozen coefficients, no CFL limit, no substeps, no
  * numerical diffusion, nothing lost through the ends.
  *   lp_bind_energy_grid  eng [capacity][nbins+1] (device, caller-owned, updated in place) switches the context to the
- *                        moving grid: lp_spectral_update and lp_step use it (lp_step stays one fused kernel; a re-sort
- *                        step permutes the rows in a pass of its own), n_sub reads 1, lp_get_diag's number uses the particle's own widths.  eng_scratch: a
+ *                        moving grid: lp_spectral_update and lp_step use it (lp_step stays one fused kernel), n_sub reads 1, lp_get_diag's number uses the particle's own widths.  eng_scratch: a
  *                        second array of the same size through which a sort moves the rows (NULL: sorts return
  *                        LP_ERR_STATE).  eng = NULL switches back to the fixed bins.
  *   lp_init_energy_grid  rows [first, first + count) <- the fixed table's edges (the grid every particle starts on).
@@ -241,6 +240,10 @@ LP_API lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_
 LP_API lp_status lp_bind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch);
 LP_API lp_status lp_init_energy_grid(lp_ctx *ctx, int64_t first, int64_t count, void *stream);
 LP_API lp_status lp_rebind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch, void *stream);
+/* Where the grid lives now: with ping-pong buffers (lp_set_pingpong) a re-sort writes the rows in the new order into
+ * eng_scratch and the two arrays change roles instead of being copied (in lp_step the permutation is then folded
+ * into the fused kernel, as for the fixed bins); without ping-pong it is always the array bound as eng. */
+LP_API lp_status lp_current_energy_grid(const lp_ctx *ctx, double **eng);
 
 /* One whole step with frozen fields: [sort every sort_every steps] -> push 0 -> push 1 ->
  * spectral update (order of Table 1, without the fluid stages). */

@@ -21,7 +21,8 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_measure_fp64_peak", "lp_set_pingpong", "lp_current_particles",
            "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack",
            "lp_capacity", "lp_workspace_bytes_for", "lp_rebind",
-           "lp_bind_energy_grid", "lp_init_energy_grid", "lp_rebind_energy_grid", "lp_interpolate_tiled")
+           "lp_bind_energy_grid", "lp_init_energy_grid", "lp_rebind_energy_grid", "lp_current_energy_grid",
+           "lp_interpolate_tiled")
 
 
 class LPError(RuntimeError):
@@ -97,6 +98,7 @@ def load():
     lib.lp_bind_energy_grid.argtypes = [vp, dp, dp]
     lib.lp_init_energy_grid.argtypes = [vp, C.c_int64, C.c_int64, vp]
     lib.lp_rebind_energy_grid.argtypes = [vp, dp, dp, vp]
+    lib.lp_current_energy_grid.argtypes = [vp, C.POINTER(C.c_void_p)]
     lib.lp_capacity.argtypes = [vp, C.POINTER(C.c_int64)]
     lib.lp_workspace_bytes_for.argtypes = [vp, C.c_int64, C.POINTER(C.c_size_t)]
     lib.lp_rebind.argtypes = [vp, C.c_int64, dp, C.c_size_t, dp, dp, dp, dp, dp, vp]
@@ -252,6 +254,12 @@ def lp_init_energy_grid(ctx, first, count, stream=None):
 
 def lp_rebind_energy_grid(ctx, eng, eng_scratch=None, stream=None):
     _check(ctx, load().lp_rebind_energy_grid(ctx, eng, eng_scratch, stream))
+
+
+def lp_current_energy_grid(ctx):
+    p = C.c_void_p()
+    _check(ctx, load().lp_current_energy_grid(ctx, C.byref(p)))
+    return p.value or 0
 
 
 def lp_capacity(ctx):

@@ -2,6 +2,7 @@
 // Host code only; every step of the path runs in the kernels of lp_particles.cu, lp_spectral.cu
 // and lp_sort.cu.  No CPU fallback exists.
 #include <algorithm>
+#include <utility>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -147,6 +148,8 @@ struct lp_ctx {
     double *lost_user = nullptr;
     double *eng = nullptr, *eng_scratch = nullptr;      // per-particle energy grid (lp_bind_energy_grid): moving-grid mode
     long long eng_capacity = 0;                         // rows the bound grid arrays hold
+    bool eng_swapped = false;                           // (ping-pong) eng / eng_scratch have changed roles: the grid lives in
+                                                        // the array bound as scratch
     // owned small tables
     double *tab = nullptr;                 // E[nb+1] | dE[nb] | rdE[nb]
     std::vector<double> h_edges, h_widths;
@@ -270,17 +273,22 @@ lp_status not_with_energy_grid(lp_ctx *c, const char *what)
 }
 
 // spectral update on the per-particle moving grid (lp_moving.cu)
-lp_status do_moving(lp_ctx *c, double dt, bool fused, cudaStream_t s)
+lp_status do_moving(lp_ctx *c, double dt, bool fused, cudaStream_t s, const uint32_t *perm = nullptr)
 {
     lp_status gs = grid_ok(c);
     if (gs != LP_OK) return gs;
     const lp_ctx::Set n = c->now();
+    LpMovingIO io{ n.x, n.y, n.z, c->eng, n.chi, n.x, n.y, n.z, c->eng, n.chi, nullptr, nullptr, nullptr };
+    if (perm) {                         // re-sort folded into the step: read the current homes, write the other ones
+        const lp_ctx::Set o = c->other();
+        io = LpMovingIO{ n.x, n.y, n.z, c->eng, n.chi, o.x, o.y, o.z, c->eng_scratch, o.chi, perm, n.id, o.id };
+    }
     const bool rec = c->timing && c->ev_used + 2 <= c->ev.size();
     if (rec) LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used], s));
-    lp_status st = count(c, lp_launch_moving(c->geom, c->cells(), n.x, n.y, n.z, c->at<double>(c->lay.rho_old),
-                                             c->at<int32_t>(c->lay.status), fused, c->eng, n.chi,
-                                             c->at<int32_t>(c->lay.nsub), c->nsub_user, c->cfg.np, c->cfg.nbins, dt,
-                                             c->cfg.kappa, c->cfg.u_rad, c->sm_count, s), "lp_moving_kernel launch");
+    lp_status st = count(c, lp_launch_moving(c->geom, c->cells(), io, c->at<double>(c->lay.rho_old),
+                                             c->at<int32_t>(c->lay.status), fused, c->at<int32_t>(c->lay.nsub), c->nsub_user,
+                                             c->cfg.np, c->cfg.nbins, dt, c->cfg.kappa, c->cfg.u_rad, c->sm_count, s),
+                         "lp_moving_kernel launch");
     if (rec) {
         LP_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], s));
         c->ev_used += 2;
@@ -289,6 +297,11 @@ lp_status do_moving(lp_ctx *c, double dt, bool fused, cudaStream_t s)
         c->spectra_done = true;
         c->stage0_done = false; c->rk3_next = 0; c->push_done = false;
         if (fused) { c->status_valid = true; c->mig_stage = 0; }
+        if (perm) {                     // the state now lives in the other homes
+            c->cur ^= 1;
+            std::swap(c->eng, c->eng_scratch);
+            c->eng_swapped = !c->eng_swapped;
+        }
     }
     return st;
 }
@@ -449,7 +462,12 @@ lp_status do_sort(lp_ctx *c, bool in_place, SpectralIO *io, cudaStream_t s)
     if (c->eng) {                       // the energy-grid rows follow their particles (through the scratch and back)
         const int len = c->cfg.nbins + 1;
         if ((st = count(c, lp_launch_permute_rows8(perm, c->eng, c->eng_scratch, np, len, s), "permute launch")) != LP_OK) return st;
-        LP_CUDA(c, cudaMemcpyAsync(c->eng, c->eng_scratch, (size_t)np * len * 8, cudaMemcpyDeviceToDevice, s));
+        if (c->pingpong) {              // the scratch becomes the grid's home (lp_current_energy_grid)
+            std::swap(c->eng, c->eng_scratch);
+            c->eng_swapped = !c->eng_swapped;
+        } else {
+            LP_CUDA(c, cudaMemcpyAsync(c->eng, c->eng_scratch, (size_t)np * len * 8, cudaMemcpyDeviceToDevice, s));
+        }
     }
     const lp_ctx::Set n = c->now();
     lp_ctx::Set o = c->other();
@@ -840,6 +858,14 @@ lp_status lp_set_pingpong(lp_ctx *ctx, int enable, void *stream)
         LP_CUDA(ctx, cudaMemcpyAsync(b.id, n.id, np * 8, cudaMemcpyDeviceToDevice, s));
         LP_CUDA(ctx, cudaMemcpyAsync(b.chi, n.chi, np * (size_t)ctx->cfg.nbins * 8, cudaMemcpyDeviceToDevice, s));
     }
+    if (!enable && ctx->eng && ctx->eng_swapped) {           // the grid goes home to the array bound as eng
+        LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+        if (ctx->cfg.np > 0)
+            LP_CUDA(ctx, cudaMemcpyAsync(ctx->eng_scratch, ctx->eng, (size_t)ctx->cfg.np * (ctx->cfg.nbins + 1) * 8,
+                                         cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
+        std::swap(ctx->eng, ctx->eng_scratch);
+        ctx->eng_swapped = false;
+    }
     if (!enable) ctx->cur = 0;
     ctx->pingpong = enable != 0;
     return LP_OK;
@@ -967,8 +993,16 @@ lp_status lp_bind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch)
     if (eng && ctx->cur != 0) return fail(ctx, LP_ERR_STATE, "bind the energy grid while the state is in the bound arrays");
     ctx->eng = eng;
     ctx->eng_scratch = eng_scratch;
+    ctx->eng_swapped = false;
     ctx->eng_capacity = eng ? ctx->capacity : 0;
     ctx->spectra_done = false;
+    return LP_OK;
+}
+
+lp_status lp_current_energy_grid(const lp_ctx *ctx, double **eng)
+{
+    if (!ctx || !eng) return LP_ERR_INVALID_ARG;
+    *eng = ctx->eng;
     return LP_OK;
 }
 
@@ -983,6 +1017,7 @@ lp_status lp_rebind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch, v
                                      static_cast<cudaStream_t>(stream)));
     ctx->eng = eng;
     ctx->eng_scratch = eng_scratch;
+    ctx->eng_swapped = false;
     ctx->eng_capacity = ctx->capacity;
     return LP_OK;
 }
@@ -1007,7 +1042,15 @@ lp_status lp_step(lp_ctx *ctx, double dt, void *stream)
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const bool sort_now = ctx->cfg.sort_every > 0 && (ctx->steps - 1) % ctx->cfg.sort_every == 0;
     if (ctx->eng) {
-        // moving energy grid: sort when due, then one kernel that does both push stages and the grid update
+        // moving energy grid: one kernel that does both push stages and the grid update; on a re-sort step with
+        // ping-pong buffers it also reads everything through the permutation (else the rows are permuted first)
+        if (sort_now && ctx->pingpong && ctx->eng_scratch) {
+            if ((st = grid_ok(ctx)) != LP_OK) return st;
+            uint32_t *perm = nullptr;
+            if ((st = sort_permutation(ctx, &perm, s)) != LP_OK) return st;
+            sort_invalidates(ctx);
+            return do_moving(ctx, dt, true, s, perm);
+        }
         if (sort_now && (st = do_sort(ctx, true, nullptr, s)) != LP_OK) return st;
         return do_moving(ctx, dt, true, s);
     }

@@ -156,10 +156,19 @@ int lp_launch_permute_rows(const uint32_t *perm, const double *src, double *dst,
 int lp_launch_max_u64(const uint64_t *v, long long np, unsigned long long *out, cudaStream_t s);
 
 // moving energy grid (lp_moving.cu)
-// fused: the kernel also does both push stages (x^n in x, y, z; x^{n+1} and status written), rho_old unused
-int lp_launch_moving(const LpGeom &g, const LpCells &cells, double *x, double *y, double *z, const double *rho_old,
-                     int32_t *status, bool fused, double *eng, double *chi, int32_t *nsub_ws, int32_t *nsub_user,
-                     long long np, int nbins, double dt, double kappa, double u_rad, int sm_count, cudaStream_t s);
+// fused: the kernel also does both push stages (x^n read, x^{n+1} and status written), rho_old unused.
+// io.perm != NULL (fused only): the step re-sorts -- everything is read at perm[p] of the *_in arrays and written
+// at p of the others.
+struct LpMovingIO {
+    const double *xin, *yin, *zin, *eng_in, *chi_in;
+    double *x, *y, *z, *eng, *chi;
+    const uint32_t *perm;
+    const uint64_t *id_in;
+    uint64_t *id_out;
+};
+int lp_launch_moving(const LpGeom &g, const LpCells &cells, const LpMovingIO &io, const double *rho_old, int32_t *status,
+                     bool fused, int32_t *nsub_ws, int32_t *nsub_user, long long np, int nbins, double dt, double kappa,
+                     double u_rad, int sm_count, cudaStream_t s);
 int lp_launch_moving_init(const double *tab, int nbins, double *eng, long long first, long long count, cudaStream_t s);
 int lp_launch_permute_rows8(const uint32_t *perm, const double *src, double *dst, long long np, int len, cudaStream_t s);
 

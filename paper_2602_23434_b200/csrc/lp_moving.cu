@@ -24,11 +24,19 @@ constexpr int kWarps = kThreads / 32;
 struct LpMovingArgs {
     LpGeom g;
     LpCells cells;
-    double *x, *y, *z;           // staged: x^{n+1} (read only); fused: x^n in, x^{n+1} out
+    double *x, *y, *z;           // staged: x^{n+1} (read only); fused: x^{n+1} out
+    const double *xin, *yin, *zin;   // positions read (== x, y, z unless the step re-sorts)
+    // Re-sort folded into the fused step (as in lp_spectral.cu): particle p of the new order is the one stored at
+    // perm[p] of xin.., id_in, eng_in, chi_in; everything is written at p of the other buffer set.
+    const uint32_t *perm;        // or NULL
+    const uint64_t *id_in;
+    uint64_t *id_out;
     const double *rho_old;       // staged: from push stage 0
     int32_t *status;             // fused: outside-box flags [np]
-    double *eng;                 // [np][nbins + 1] in/out
-    double *chi;                 // [np][nbins] in/out
+    const double *eng_in;        // [np][nbins + 1]
+    double *eng;                 // [np][nbins + 1] out (== eng_in unless the step re-sorts)
+    const double *chi_in;        // [np][nbins]
+    double *chi;                 // [np][nbins] out
     int32_t *nsub_ws;            // [np]: 1 (one exact step per particle)
     int32_t *nsub_user;          // or NULL
     long long np;
@@ -37,9 +45,8 @@ struct LpMovingArgs {
 
 // per-particle phase: [FUSED: push stages a5, a6,] coefficients a7, then (alpha, beta) of the step (reading E2)
 template <bool FUSED>
-__device__ __forceinline__ double2 lp_moving_coef(const LpMovingArgs &A, long long p)
+__device__ __forceinline__ double2 lp_moving_coef(const LpMovingArgs &A, long long p, double px, double py, double pz)
 {
-    const double px = A.x[p], py = A.y[p], pz = A.z[p];
     double a, cr, dtau;
     lp_particle_coefficients<FUSED>(A.g, A.cells, A.dt, A.kappa, A.u_rad, A.x, A.y, A.z, A.status, A.rho_old, p, px, py, pz,
                                     a, cr, dtau);
@@ -55,9 +62,11 @@ __device__ __forceinline__ double2 lp_moving_coef(const LpMovingArgs &A, long lo
 // bandwidth with six, 128 / 256 bins 0.89 / 0.90 -> 0.875 / 0.865; eight blocks or eight rows in flight lose
 // everywhere).  The fused kernel (push stages in the per-particle phase: three stencils, the corner records kept
 // in registers between them) gets four.
-template <int NB, bool FUSED>
-__global__ void __launch_bounds__(kThreads, (NB <= 64 && !FUSED) ? 6 : 4) lp_moving_kernel(LpMovingArgs A)
+// MODE: 0 staged (lp_spectral_update), 1 fused step, 2 fused step that re-sorts (reads through A.perm).
+template <int NB, int MODE>
+__global__ void __launch_bounds__(kThreads, (NB <= 64 && MODE == 0) ? 6 : 4) lp_moving_kernel(LpMovingArgs A)
 {
+    constexpr bool FUSED = MODE >= 1, PERM = MODE == 2;
     constexpr int G = NB < 32 ? NB : 32;         // lanes per row
     constexpr int PPW = 32 / G;                  // rows a warp holds side by side
     constexpr int M = NB / G;                    // bins per lane: bin sub + G j
@@ -66,6 +75,7 @@ __global__ void __launch_bounds__(kThreads, (NB <= 64 && !FUSED) ? 6 : 4) lp_mov
     static_assert(32 % ROWS == 0 || ROWS <= 32, "rows per trip");
 
     __shared__ double2 sAB[kThreads];
+    __shared__ uint32_t sSrc[PERM ? kThreads : 1];          // source row of every particle of the group
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sub = lane % G, grp = lane / G;
     const long long ngroups = (A.np + kThreads - 1) / kThreads;
@@ -76,7 +86,12 @@ __global__ void __launch_bounds__(kThreads, (NB <= 64 && !FUSED) ? 6 : 4) lp_mov
             const long long p = base + threadIdx.x;
             double2 ab = make_double2(1.0, 0.0);
             if (p < A.np) {
-                ab = lp_moving_coef<FUSED>(A, p);
+                const size_t src = PERM ? (size_t)A.perm[p] : (size_t)p;
+                if (PERM) {
+                    sSrc[threadIdx.x] = (uint32_t)src;
+                    A.id_out[p] = A.id_in[src];
+                }
+                ab = lp_moving_coef<FUSED>(A, p, A.xin[src], A.yin[src], A.zin[src]);
                 __stcs(A.nsub_ws + p, 1);
                 if (A.nsub_user) __stcs(A.nsub_user + p, 1);
             }
@@ -95,8 +110,9 @@ __global__ void __launch_bounds__(kThreads, (NB <= 64 && !FUSED) ? 6 : 4) lp_mov
                 row[u] = base + rl;
                 have[u] = row[u] < A.np;
                 ab[u] = sAB[rl];
-                const double *er = A.eng + row[u] * (NB + 1);
-                const double *cp = A.chi + row[u] * NB;
+                const long long srow = (PERM && have[u]) ? (long long)sSrc[rl] : row[u];
+                const double *er = A.eng_in + srow * (NB + 1);
+                const double *cp = A.chi_in + srow * NB;
 #pragma unroll
                 for (int j = 0; j < M; ++j) {
                     e[u][j] = have[u] ? __ldcs(er + sub + G * j) : 1.0;
@@ -157,38 +173,42 @@ lp_permute_rows8_kernel(const uint32_t *__restrict__ perm, const double *__restr
     }
 }
 
-template <int NB, bool FUSED>
+template <int NB, int MODE>
 int launch_mode(const LpMovingArgs &a, int sm_count, cudaStream_t s)
 {
     int per_sm = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_moving_kernel<NB, FUSED>, kThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_moving_kernel<NB, MODE>, kThreads, 0);
     if (per_sm < 1) per_sm = 1;
     const long long want = (a.np + kThreads - 1) / kThreads;
     const long long cap = (long long)sm_count * per_sm;
     int blocks = (int)(want < cap ? want : cap);
     if (blocks < 1) blocks = 1;
-    lp_moving_kernel<NB, FUSED><<<blocks, kThreads, 0, s>>>(a);
+    lp_moving_kernel<NB, MODE><<<blocks, kThreads, 0, s>>>(a);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
 template <int NB>
 int launch(const LpMovingArgs &a, bool fused, int sm_count, cudaStream_t s)
 {
-    return fused ? launch_mode<NB, true>(a, sm_count, s) : launch_mode<NB, false>(a, sm_count, s);
+    if (!fused) return launch_mode<NB, 0>(a, sm_count, s);
+    return a.perm ? launch_mode<NB, 2>(a, sm_count, s) : launch_mode<NB, 1>(a, sm_count, s);
 }
 
 }  // namespace
 
-int lp_launch_moving(const LpGeom &g, const LpCells &cells, double *x, double *y, double *z, const double *rho_old,
-                     int32_t *status, bool fused, double *eng, double *chi, int32_t *nsub_ws, int32_t *nsub_user,
-                     long long np, int nbins, double dt, double kappa, double u_rad, int sm_count, cudaStream_t s)
+int lp_launch_moving(const LpGeom &g, const LpCells &cells, const LpMovingIO &io, const double *rho_old, int32_t *status,
+                     bool fused, int32_t *nsub_ws, int32_t *nsub_user, long long np, int nbins, double dt, double kappa,
+                     double u_rad, int sm_count, cudaStream_t s)
 {
     LpMovingArgs a;
     a.g = g; a.cells = cells;
-    a.x = x; a.y = y; a.z = z;
+    a.x = io.x; a.y = io.y; a.z = io.z;
+    a.xin = io.xin; a.yin = io.yin; a.zin = io.zin;
+    a.perm = io.perm; a.id_in = io.id_in; a.id_out = io.id_out;
     a.rho_old = rho_old;
     a.status = status;
-    a.eng = eng; a.chi = chi;
+    a.eng_in = io.eng_in; a.eng = io.eng;
+    a.chi_in = io.chi_in; a.chi = io.chi;
     a.nsub_ws = nsub_ws; a.nsub_user = nsub_user;
     a.np = np;
     a.dt = dt; a.kappa = kappa; a.u_rad = u_rad;

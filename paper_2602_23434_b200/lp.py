@@ -20,7 +20,7 @@ class LP:
         self._bound = None            # the caller-side tensors x, y, z, id, chi (the bound arrays)
         self.capacity = cfg.np
         self.nsub = self.lost = None
-        self.eng = self._eng_scratch = None
+        self._eng = self._eng_scratch = None
         self._fields = None
 
     def _alloc_workspace(self, nbytes):
@@ -142,16 +142,24 @@ class LP:
         """Switch to the moving energy grid: allocates eng [capacity][nbins+1] (and the scratch a sort needs),
         starts every particle on the fixed table's edges."""
         shape = (self.capacity, self.cfg.nbins + 1)
-        self.eng = torch.empty(shape, dtype=torch.float64, device=self.device)
+        self._eng = torch.empty(shape, dtype=torch.float64, device=self.device)
         self._eng_scratch = torch.empty(shape, dtype=torch.float64, device=self.device) if sortable else None
-        B.lp_bind_energy_grid(self.ctx, self.eng.data_ptr(), self._eng_scratch.data_ptr() if sortable else None)
+        B.lp_bind_energy_grid(self.ctx, self._eng.data_ptr(), self._eng_scratch.data_ptr() if sortable else None)
         if init:
             B.lp_init_energy_grid(self.ctx, 0, self.capacity, self.stream)
-        return self.eng
+        return self._eng
+
+    @property
+    def eng(self):
+        """The tensor that holds the energy grid now (with ping-pong buffers a re-sort swaps it with the scratch)."""
+        if self._eng is None:
+            return None
+        ptr = B.lp_current_energy_grid(self.ctx)
+        return self._eng if ptr == self._eng.data_ptr() else self._eng_scratch
 
     def unbind_energy_grid(self):
         B.lp_bind_energy_grid(self.ctx, None, None)
-        self.eng = self._eng_scratch = None
+        self._eng = self._eng_scratch = None
 
     # ---- chunked growth (PAPER.md:176-184 Listing 1; Reserve() / Shrink() of Listing 2)
     def _rebind(self, capacity):
@@ -169,13 +177,13 @@ class LP:
         self.nsub = self.lost = None
         if any(had):
             self.bind_diag(*had)
-        if getattr(self, "eng", None) is not None:           # the energy grid follows: new arrays, rows copied over
+        if self._eng is not None:                            # the energy grid follows: new arrays, rows copied over
             shape = (capacity, nb + 1)
             eng = torch.empty(shape, dtype=torch.float64, device=self.device)
             scr = torch.empty(shape, dtype=torch.float64, device=self.device) if self._eng_scratch is not None else None
             B.lp_rebind_energy_grid(self.ctx, eng.data_ptr(), scr.data_ptr() if scr is not None else None, self.stream)
-            self._retired = self._retired + (self.eng, self._eng_scratch)
-            self.eng, self._eng_scratch = eng, scr
+            self._retired = self._retired + (self._eng, self._eng_scratch)
+            self._eng, self._eng_scratch = eng, scr
 
     def reserve(self, n_new, e=18):
         """Room for n_new more particles behind the current ones (Listing 2's Reserve): when the capacity does

@@ -88,7 +88,14 @@ def test_moving_grid_lp_step_with_resort(nbins, np_, pingpong):
     check(lp, st)
     lp.sort()
     perm = orc.sort_perm(orc.cell_key(prm, *st[:3]), st[3])
-    check(lp, [a[perm] for a in st])
+    st = [a[perm] for a in st]
+    check(lp, st)
+    if pingpong:                                         # leaving ping-pong brings state and grid home
+        lp.set_pingpong(False)
+        assert lp.eng.data_ptr() == lp._eng.data_ptr() and lp.x.data_ptr() == lp._bound[0].data_ptr()
+        check(lp, st)
+        lp.step(w.dt)                                    # step 6: no re-sort due
+        check(lp, oracle_step(prm, f_np, st, w.dt, False))
 
 
 def test_moving_grid_synchrotron_law_and_unsupported_calls():
