@@ -132,3 +132,38 @@ def test_exchange_state_errors_and_capacity():
     lp.sort()
     with pytest.raises(B.LPError):
         lp.migrate_pack(nl, nr)
+
+
+@pytest.mark.parametrize("n,lo,hi", [(0, -1.0, 0.0), (1, 0.5, 1.0), (1, -1.0, 1.0), (37, 0.999, 1.0), (4097, -1.0, 1.0)])
+def test_exchange_degenerate_sets(n, lo, hi):
+    """No particles, one particle, (almost) everybody leaving, nobody leaving: counts, buffers and the state after
+    an exchange in which nothing arrives follow the oracle."""
+    rng = np.random.default_rng(n)
+    nb, cap = 16, max(n, 1)
+    cfg = P.make_config(4, 4, 4, (-1.0,) * 3, (1.0,) * 3, (1, 1, 1), cap, nb, 1.0, 1e6)
+    lp = P.LP(cfg)
+    pos = rng.uniform(-1, 0.99, size=(cap, 3)); pid = np.arange(cap, dtype=np.uint64) + np.uint64(7)
+    chi = rng.uniform(size=(cap, nb))
+    lp.bind_particles(pos[:, 0], pos[:, 1], pos[:, 2], pid, chi)
+    lp.set_count(n)
+    st = tuple(a[:n].copy() for a in (pos[:, 0], pos[:, 1], pos[:, 2], pid, chi))
+    dest, holes, left, right = orc.migrate_pack(0, lo, hi, -1.0, 1.0, 1, *st)
+    nl, nr = lp.migrate_count(0, lo, hi)
+    assert (nl, nr) == (left[0].shape[0], right[0].shape[0])
+    bl, br = lp.migrate_pack(nl, nr)
+    for got, want in ((decode(bl, nl, nb), left), (decode(br, nr, nb), right)):
+        for g, w_ in zip(got, want):
+            assert np.array_equal(g, w_)
+    n_new = lp.migrate_unpack(None, 0, None, 0)
+    want = orc.migrate_unpack(holes, None, None, *st)
+    assert n_new == want[0].shape[0] == n - nl - nr
+    torch.cuda.synchronize()
+    for g, w_ in zip(gpu_state(lp), want):
+        assert np.array_equal(g, w_)
+    if nl + nr:                                             # everything that left comes back in: the count is restored
+        assert lp.migrate_count(0, -1.0, 1.0) == (0, 0)
+        lp.migrate_pack(0, 0)
+        assert lp.migrate_unpack(bl, nl, br, nr) == n
+        back = orc.migrate_unpack(np.zeros(0, dtype=np.int64), left, right, *want)
+        for g, w_ in zip(gpu_state(lp), back):
+            assert np.array_equal(g, w_)
