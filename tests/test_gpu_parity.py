@@ -540,3 +540,43 @@ def test_random_small_configurations(seed):
     assert_chi_close(host(lp.chi), chi)
     d = lp.diag()
     assert d["n_outside"] == int((st != 0).sum()) and d["np"] == np_
+
+
+# ------------------------------------------------------------------ several contexts at once
+
+def test_two_contexts_from_two_host_threads():
+    """lp.h: a context is used by one host thread at a time, but several contexts may run concurrently from
+    different threads (they share no mutable state).  Two threads, each with its own context, bin count and
+    stream, step at the same time; both must give the oracle's result."""
+    import threading
+    cases = [small_turbulent(np_=5000 + 3, nbins=64, sort_every=2), small_turbulent(np_=3000 + 1, nbins=256, sort_every=1, seed=99)]
+    pairs = [setup_pair(w, shuffle_ids=True, diag="nsub", pingpong=(i == 1)) for i, w in enumerate(cases)]
+    errors = []
+    torch.cuda.synchronize()            # the set-up ran on the default stream
+
+    def work(i):
+        try:
+            lp, w = pairs[i][0], cases[i]
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                for _ in range(6):
+                    lp.step(w.dt)
+                stream.synchronize()
+        except Exception as e:          # noqa: BLE001 -- reported by the main thread
+            errors.append((i, e))
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    torch.cuda.synchronize()
+    for (lp, prm, f_np, x, y, z, pid, chi), w in zip(pairs, cases):
+        for s in range(6):
+            if s % w.sort_every == 0:
+                x, y, z, pid, chi, _, _ = oracle_sort_state(prm, x, y, z, pid, chi)
+            x, y, z, chi, nsub, lost, st = orc.step(prm, f_np, x, y, z, w.dt, chi, nthreads=8)
+        assert np.array_equal(host(lp.id).view(np.uint64), pid) and np.array_equal(host(lp.x), x)
+        assert_nsub_equal(host(lp.nsub), nsub)
+        assert_chi_close(host(lp.chi), chi)
