@@ -36,8 +36,12 @@
  * flow, the closed form Eq. 10 and homologous flow for the pusher;
  * the analytic synchrotron-cooled power law, the adiabatic rho^{1/3} law, a
  * scale-invariance product formula, the loss steady state, number conservation,
- * positivity and hand-worked N_b = 2, 3 cases for the spectral update.
- * No function here is "parity unpinned".
+ * positivity and hand-worked N_b = 2, 3 cases for the spectral update; hand-worked fractions, a closed
+ * form and the paper's slope for the shock update; hand-worked cases and invariants for the compaction; the
+ * cubic Taylor factor for the third-order pusher; a hand-worked two-rank case, the owner by brute force and
+ * "everybody at home after three sweeps" for the exchange; hand-worked values, an independent ODE
+ * integration, the synchrotron and rho^(1/3) laws and exact bin means of a cooled power law for the moving
+ * energy grid.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
