@@ -393,6 +393,20 @@ void orc_shock_update(int32_t nbins, const double *E, const double *dE, int64_t 
     for (int64_t p = 0; p < np; ++p) orc_shock_row(nbins, E, dE, r[p], q_r, chi + p * nbins);
 }
 
+/* the same with a per-particle energy grid (moving grid, readings E1-E4): row p is discretised on its own
+ * edges eng[p][0..nbins], so its bin centres and widths are its own; orc_shock_row is written for any edges */
+void orc_shock_update_grid(int32_t nbins, int64_t np, const double *eng /*[np][nbins+1]*/, const double *r,
+                           double q_r, double *chi /*[np][nbins] in/out*/)
+{
+    double *dE = (double *)malloc((size_t)nbins * sizeof(double));
+    for (int64_t p = 0; p < np; ++p) {
+        const double *E = eng + p * (nbins + 1);
+        for (int i = 0; i < nbins; ++i) dE[i] = E[i + 1] - E[i];
+        orc_shock_row(nbins, E, dE, r[p], q_r, chi + p * nbins);
+    }
+    free(dE);
+}
+
 /* ---------------------------------------------------------------- deletion + hole filling (NEXT-2) */
 
 /* The paper's compaction, step by step:

@@ -197,6 +197,17 @@ def shock_update(E, dE, r, q_r, chi):
     return chi
 
 
+def shock_update_grid(eng, r, q_r, chi):
+    """Eq. 7-8 on every row, each on its own edges eng [np][nbins+1]; returns the new chi."""
+    eng = np.ascontiguousarray(eng, dtype=np.float64); r, pr = _d(r)
+    chi = np.array(chi, dtype=np.float64, order="C")
+    f = lib().orc_shock_update_grid
+    f.restype = None
+    dp = C.POINTER(C.c_double)
+    f(C.c_int32(chi.shape[1]), C.c_int64(chi.shape[0]), eng.ctypes.data_as(dp), pr, C.c_double(q_r), chi.ctypes.data_as(dp))
+    return chi
+
+
 def compact(flag, x, y, z, pid, chi):
     """The paper's delete-and-fill compaction; returns (x, y, z, id, chi) cut to the new count."""
     flag = np.ascontiguousarray(flag, dtype=np.int32)

@@ -91,3 +91,25 @@ def test_shock_update_applies_row_by_row():
     for p in range(7):
         row, _ = orc.shock_row(E, dE, r[p], 0.0, chi[p])
         assert np.array_equal(out[p], row)
+
+
+def test_shock_on_per_particle_grids_is_the_row_update_on_each_grid():
+    """orc_shock_update_grid: every row on its own edges.  A particle whose grid is the fixed table must give
+    orc_shock_update's row; a grid scaled by a factor s gives the same chi / s on the scaled bins (Eq. 7 is
+    homogeneous in the energy: the update commutes with a rescaling of the energy axis); number is conserved."""
+    nb = 32
+    E, dE, Ec = orc.bin_table(nb, 1.0, 1e6)
+    rng = np.random.default_rng(4)
+    chi = rng.uniform(0.5, 1.5, size=(3, nb)) * Ec[None, :] ** -2.3
+    s = 0.37
+    eng = np.stack([E, s * E, E])
+    chi_in = chi.copy(); chi_in[1] = chi[0] / s           # the same particle as row 0 on a scaled energy axis
+    r = np.array([3.0, 3.0, 1.0])
+    out = orc.shock_update_grid(eng, r, 0.1, chi_in)
+    want0 = orc.shock_update(E, dE, r[:1], 0.1, chi[:1])[0]
+    assert np.allclose(out[0], want0, rtol=1e-14, atol=0)
+    assert np.allclose(out[1] * s, out[0], rtol=1e-12, atol=0)
+    assert np.array_equal(out[2], chi_in[2])                # r = 1: untouched
+    for p in range(2):
+        w = np.diff(eng[p])
+        assert np.isclose((out[p] * w).sum(), (chi_in[p] * w).sum(), rtol=1e-13)
