@@ -235,8 +235,8 @@ LP_API lp_status lp_rebind(lp_ctx *ctx, int64_t capacity, void *workspace, size_
  *                        LP_ERR_STATE when the capacity has outgrown the bound arrays.
  * The grid rows travel with their particles: lp_sort, lp_compact and lp_migrate_pack / _unpack move them (an
  * exchange buffer then carries eng[n][nbins+1] behind chi[n][nbins]; lp_migrate_record_bytes says so).
- * lp_step_host (no host grid argument) and lp_shock_update (its bin centres are the fixed table's) return
- * LP_ERR_UNSUPPORTED while a grid is bound. */
+ * lp_shock_update takes every row's centres and widths from its own grid.  lp_step_host (no host grid argument)
+ * returns LP_ERR_UNSUPPORTED while a grid is bound. */
 LP_API lp_status lp_bind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch);
 LP_API lp_status lp_init_energy_grid(lp_ctx *ctx, int64_t first, int64_t count, void *stream);
 LP_API lp_status lp_rebind_energy_grid(lp_ctx *ctx, double *eng, double *eng_scratch, void *stream);

@@ -718,11 +718,11 @@ lp_status lp_shock_update(lp_ctx *ctx, const double *r, double q_r, void *stream
 {
     lp_status st = need_ready(ctx, false);
     if (st != LP_OK) return st;
-    if ((st = not_with_energy_grid(ctx, "lp_shock_update")) != LP_OK) return st;
+    if ((st = grid_ok(ctx)) != LP_OK) return st;
     if (ctx->cfg.np == 0) return LP_OK;
     if (!r) return fail(ctx, LP_ERR_INVALID_ARG, "r is NULL");
     LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    return count(ctx, lp_launch_shock(ctx->tab, r, q_r, ctx->now().chi, ctx->cfg.np, ctx->cfg.nbins, ctx->sm_count,
+    return count(ctx, lp_launch_shock(ctx->tab, ctx->eng, r, q_r, ctx->now().chi, ctx->cfg.np, ctx->cfg.nbins, ctx->sm_count,
                                       static_cast<cudaStream_t>(stream)), "lp_shock_kernel launch");
 }
 

@@ -100,8 +100,9 @@ int lp_launch_spectral(const LpSpectralArgs &a, int nbins, bool diag, bool fused
                        cudaStream_t s);
 
 // shock-crossing update of the flagged rows (lp_shock.cu); r [np] device, r <= 1 = untouched
-int lp_launch_shock(const double *tab, const double *r, double q_r, double *chi, long long np, int nbins,
-                    int sm_count, cudaStream_t s);
+// eng != NULL: every row on its own edges eng[p][0..nbins] (moving energy grid) instead of the table's
+int lp_launch_shock(const double *tab, const double *eng, const double *r, double q_r, double *chi, long long np,
+                    int nbins, int sm_count, cudaStream_t s);
 
 // deletion with hole filling (lp_compact.cu); counts = 2 x u64 on the device: N_del, number of holes
 size_t lp_compact_block_elems(long long np);

@@ -88,6 +88,96 @@ __device__ __forceinline__ bool lp_shock_row(const LpShockTab<M> &tb, double rr,
     return changed;
 }
 
+// The same on a per-particle energy grid (moving grid): the row's own edges e[0..M] (e[M] = the next lane's first
+// edge or the top edge) give its centres and widths; nothing is geometric any more, so ec^(q-3) costs a log and an
+// exp per bin.
+template <int M, int G>
+__device__ __forceinline__ bool lp_shock_row_grid(const double (&e)[M + 1], double rr, double q_r, double (&c)[M], int sub)
+{
+    const double q = __dadd_rn(__ddiv_rn(__dmul_rn(3.0, rr), __dsub_rn(rr, 1.0)), q_r);   // Eq. 8
+    const double s3 = q - 3.0;
+    double term[M], scale[M], de[M];
+    double total = 0.0, n_in = 0.0;
+#pragma unroll
+    for (int i = 0; i < M; ++i) {
+        const double ec = __dsqrt_rn(__dmul_rn(e[i], e[i + 1]));
+        de[i] = __dsub_rn(e[i + 1], e[i]);
+        const double pw = exp(s3 * log(ec));
+        term[i] = c[i] * pw * de[i];
+        scale[i] = 1.0 / (pw * ec);
+        total += term[i];
+        n_in = fma(c[i], de[i], n_in);
+    }
+    double incl = total;
+#pragma unroll
+    for (int o = 1; o < G; o <<= 1) {
+        const double u = __shfl_up_sync(kFull, incl, o, G);
+        if (sub >= o) incl += u;
+    }
+    double below = __shfl_up_sync(kFull, incl, 1, G);
+    if (sub == 0) below = 0.0;
+    double n_out = 0.0;
+    double t[M];
+#pragma unroll
+    for (int i = 0; i < M; ++i) {
+        t[i] = (below + 0.5 * term[i]) * scale[i];
+        below += term[i];
+        n_out = fma(t[i], de[i], n_out);
+    }
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) {
+        n_in += __shfl_xor_sync(kFull, n_in, o);
+        n_out += __shfl_xor_sync(kFull, n_out, o);
+    }
+    const bool changed = n_out != 0.0 && n_out == n_out;
+    if (changed) {
+        const double norm = n_in / n_out;
+#pragma unroll
+        for (int i = 0; i < M; ++i) c[i] = norm * t[i];
+    }
+    return changed;
+}
+
+// one lane group per flagged row, plain 8-byte accesses (grid rows are 8-byte aligned only)
+template <int NB>
+__global__ void __launch_bounds__(kThreads)
+lp_shock_grid_kernel(const double *__restrict__ eng, const double *__restrict__ r, double q_r,
+                     double *__restrict__ chi, long long np)
+{
+    using C = LpShockCfg<NB>;
+    constexpr int M = C::M, G = C::G, PPW = C::PPW;
+    const int lane = threadIdx.x & 31;
+    const int sub = lane % G, grp = lane / G;
+    const int b0 = sub * M;
+    const long long gw = ((long long)blockIdx.x * kThreads + threadIdx.x) >> 5;
+    const long long nw = ((long long)gridDim.x * kThreads) >> 5;
+    for (long long base = gw << 5; base < np; base += nw << 5) {
+        const double r_lane = base + lane < np ? r[base + lane] : 0.0;
+        const unsigned todo = __ballot_sync(kFull, r_lane > 1.0);
+        const int nflag = __popc(todo);
+        for (int k = 0; k < nflag; k += PPW) {
+            const int idx = k + grp;
+            const bool valid = idx < nflag;
+            const int j = valid ? (int)__fns(todo, 0, idx + 1) : 0;
+            const double rr = __shfl_sync(kFull, r_lane, j);
+            double *row = chi + (base + j) * NB + b0;
+            const double *er = eng + (base + j) * (NB + 1) + b0;
+            double c[M], e[M + 1];
+#pragma unroll
+            for (int i = 0; i < M; ++i) {
+                c[i] = valid ? row[i] : 0.0;
+                e[i] = valid ? er[i] : 1.0 + i;
+            }
+            e[M] = valid ? er[M] : 1.0 + M;
+            const bool changed = lp_shock_row_grid<M, G>(e, valid ? rr : 2.0, q_r, c, sub);
+            if (valid && changed) {
+#pragma unroll
+                for (int i = 0; i < M; ++i) row[i] = c[i];
+            }
+        }
+    }
+}
+
 template <int NB>
 __global__ void __launch_bounds__(kThreads)
 lp_shock_kernel(const double *__restrict__ tab, const double *__restrict__ r, double q_r,
@@ -151,28 +241,30 @@ lp_shock_kernel(const double *__restrict__ tab, const double *__restrict__ r, do
 }
 
 template <int NB>
-int launch(const double *tab, const double *r, double q_r, double *chi, long long np, int sm_count, cudaStream_t s)
+int launch(const double *tab, const double *eng, const double *r, double q_r, double *chi, long long np, int sm_count,
+           cudaStream_t s)
 {
     long long blocks = (np + kWarps * 32 - 1) / (kWarps * 32);          // a warp takes 32 particles per trip
     const long long cap = (long long)sm_count * 8;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
-    lp_shock_kernel<NB><<<(int)blocks, kThreads, 0, s>>>(tab, r, q_r, chi, np);
+    if (eng) lp_shock_grid_kernel<NB><<<(int)blocks, kThreads, 0, s>>>(eng, r, q_r, chi, np);
+    else lp_shock_kernel<NB><<<(int)blocks, kThreads, 0, s>>>(tab, r, q_r, chi, np);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
 }  // namespace
 
-int lp_launch_shock(const double *tab, const double *r, double q_r, double *chi, long long np, int nbins,
-                    int sm_count, cudaStream_t s)
+int lp_launch_shock(const double *tab, const double *eng, const double *r, double q_r, double *chi, long long np,
+                    int nbins, int sm_count, cudaStream_t s)
 {
     switch (nbins) {
-    case 16:  return launch<16>(tab, r, q_r, chi, np, sm_count, s);
-    case 32:  return launch<32>(tab, r, q_r, chi, np, sm_count, s);
-    case 64:  return launch<64>(tab, r, q_r, chi, np, sm_count, s);
-    case 128: return launch<128>(tab, r, q_r, chi, np, sm_count, s);
-    case 256: return launch<256>(tab, r, q_r, chi, np, sm_count, s);
-    case 512: return launch<512>(tab, r, q_r, chi, np, sm_count, s);
+    case 16:  return launch<16>(tab, eng, r, q_r, chi, np, sm_count, s);
+    case 32:  return launch<32>(tab, eng, r, q_r, chi, np, sm_count, s);
+    case 64:  return launch<64>(tab, eng, r, q_r, chi, np, sm_count, s);
+    case 128: return launch<128>(tab, eng, r, q_r, chi, np, sm_count, s);
+    case 256: return launch<256>(tab, eng, r, q_r, chi, np, sm_count, s);
+    case 512: return launch<512>(tab, eng, r, q_r, chi, np, sm_count, s);
     default:  return -1;
     }
 }

@@ -109,9 +109,6 @@ def test_moving_grid_synchrotron_law_and_unsupported_calls():
         lp.step(dt)
     eng = host(lp.eng)
     assert np.allclose(eng, (E / (1.0 + cr * E * dt * 100))[None, :], rtol=1e-12, atol=0)
-    with pytest.raises(B.LPError) as e:
-        lp.shock_update(torch.full((w.np,), 2.0, dtype=torch.float64, device=lp.device))
-    assert e.value.status == B.LP_ERR_UNSUPPORTED
     hx = torch.zeros(w.np, dtype=torch.float64).pin_memory()
     with pytest.raises(B.LPError) as e:
         lp.step_host(dt, hx, hx, hx, torch.zeros(w.np, dtype=torch.int64).pin_memory(),
@@ -181,3 +178,25 @@ def test_grid_rows_travel_with_their_particles():
     check(lp, [x, y, z, pid, chi, eng])
     lp.step(w.dt)                                        # and the moving-grid update goes on
     check(lp, oracle_step(prm, f_np, [x, y, z, pid, chi, eng], w.dt, False))
+
+
+@pytest.mark.parametrize("nbins", [16, 64, 128, 512])
+def test_shock_update_on_the_moving_grid(nbins):
+    """lp_shock_update with a bound grid: every flagged row on its own edges, against orc_shock_update_grid."""
+    w = I.workload(3).scaled(n=12, np=1500 + 7, nbins=nbins, sort_every=0)
+    lp, prm, f_np, st = setup(w)
+    for _ in range(3):                                   # grids that differ from particle to particle
+        lp.step(w.dt)
+        st = oracle_step(prm, f_np, st, w.dt, False)
+    rng = np.random.default_rng(nbins)
+    r = np.where(rng.uniform(size=w.np) < 0.6, rng.uniform(1.5, 4.0, size=w.np), 1.0)
+    r[::53] = np.nan
+    lp.shock_update(torch.from_numpy(r).to(lp.device), 0.05)
+    before = st[4].copy()
+    st[4] = orc.shock_update_grid(st[5], r, 0.05, st[4])
+    check(lp, st)
+    untouched = ~(r > 1.0)
+    got = host(lp.chi)
+    assert_chi_close(got[untouched], before[untouched])
+    wdt = np.diff(host(lp.eng), axis=1)
+    assert np.allclose((got * wdt).sum(axis=1), (before * np.diff(st[5], axis=1)).sum(axis=1), rtol=1e-12, atol=0)
