@@ -587,19 +587,23 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #ifndef LP_BULK_WARPS
 #define LP_BULK_WARPS 16        // warps per block (one block per SM)
 #endif
-// particle warps per block by bin count (the rest are row warps): the per-particle phase costs the
-// same at every N_b, the row phase grows with N_b
+// particle warps per block by bin count (the rest are row warps): the per-particle phase costs the same at every
+// N_b, the row phase grows with N_b.  Swept in round 2 on workloads 3-5 (fraction of the copy bandwidth):
+//   16 bins  8 / 10 / 11 / 12 particle warps: 0.664 / 0.708 / 0.712 / 0.707      32 bins  8 / 9 / 10 / 11: 0.754 / 0.760 / 0.766 / 0.760
+//   64 bins  workload 4: 4 / 6 / 7 / 8 / 10: 0.677 / 0.838 / 0.859 / 0.836 / 0.706;  workload 5: 0.665 / 0.804 / 0.813 / 0.759 / 0.744
+//   128 bins 3 / 4 / 5 / 6: workload 3 0.818 / 0.922 / 0.944 / 0.871, workload 4 at 128 bins 0.804 / 0.877 / 0.861 / 0.809
+//   256 bins 3 / 4 / 5 / 6: 0.839 / 0.828 / 0.811 / 0.780
 #ifndef LP_BULK_NP16
-#define LP_BULK_NP16 8
+#define LP_BULK_NP16 10
 #endif
 #ifndef LP_BULK_NP32
-#define LP_BULK_NP32 8
+#define LP_BULK_NP32 10
 #endif
 #ifndef LP_BULK_NP64
-#define LP_BULK_NP64 8
+#define LP_BULK_NP64 7
 #endif
 #ifndef LP_BULK_NP256
-#define LP_BULK_NP256 4
+#define LP_BULK_NP256 3
 #endif
 #ifndef LP_BULK_NP128
 #define LP_BULK_NP128 4
