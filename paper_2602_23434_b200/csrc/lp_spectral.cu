@@ -645,7 +645,7 @@ struct LpBulkCfg {
     static constexpr int THREADS = (NP + NR) * 32;
     static constexpr size_t SMEM_RING = (size_t)NR * S * SLOT_BYTES;
     static constexpr size_t SMEM_TAB = ((size_t)(2 * NB + 2) * 8 + 127) / 128 * 128;
-    static constexpr size_t SMEM_COEF = (size_t)D * 32 * (sizeof(double2) + sizeof(int));
+    static constexpr size_t SMEM_COEF = (size_t)D * 32 * (sizeof(double2) + sizeof(int)) + (size_t)D * 2 * sizeof(uint32_t);
     static constexpr size_t SMEM_BAR = ((size_t)(NR * S + 2 * D) * 8 + 127) / 128 * 128;
     static constexpr size_t SMEM_TOTAL = SMEM_RING + SMEM_TAB + SMEM_COEF + SMEM_BAR + 128;
     static constexpr int RI_WANT = (LP_BULK_RI * PPW <= R) ? LP_BULK_RI : R / PPW;
@@ -678,11 +678,19 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
     double *sR = sE + (NB + 2);
     double2 *sAC = reinterpret_cast<double2 *>(sm + C::SMEM_RING + C::SMEM_TAB);
     int *sNS = reinterpret_cast<int *>(sAC + D * 32);
+    // Which chunk a coefficient slot holds (sTag) and which chunk was last consumed from it (sDone).  An mbarrier
+    // wait only knows the parity of a phase: a warp that gets two phases ahead of a slot's barrier would pass the
+    // wait on the phase before last.  With 8 + 8 or 4 + 12 warps and 32 slots that cannot happen (a slot's chunks
+    // all belong to one particle warp and one row warp); with 7 + 9, 10 + 6, 3 + 13 it can, so every wait is
+    // confirmed against the chunk number and repeated if the slot is not there yet.
+    volatile uint32_t *sTag = reinterpret_cast<volatile uint32_t *>(sNS + D * 32);
+    volatile uint32_t *sDone = sTag + D;
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(sm + C::SMEM_RING + C::SMEM_TAB + C::SMEM_COEF);
     // bars: [NR*S] ring slots | [D] coefficient slot full | [D] coefficient slot empty
 
     for (int i = threadIdx.x; i <= NB; i += C::THREADS) sE[i] = A.tab[i];
     for (int i = threadIdx.x; i < NB; i += C::THREADS) sR[i] = A.tab[(NB + 1) + NB + i];
+    for (int i = threadIdx.x; i < 2 * D; i += C::THREADS) sTag[i] = 0xffffffffu;
     if (threadIdx.x == 0) {
         for (int i = 0; i < NR * S + 2 * D; ++i) lp_mbar_init(lp_smem_u32(bars + i), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -744,9 +752,15 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
                 if (perm) __stcs(A.id_out + p1, __ldcs(A.id_in + p));
             }
             if (perm && v2) q1 = perm[p2];
-            if (use >= 1) lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u);
+            if (use >= 1) {                 // the slot's previous chunk (t - D) has been consumed
+                lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u);
+                while (sDone[cs] != t - D) { __nanosleep(64); lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u); }
+            }
             lp_chunk_phase1<NB, FUSED>(A, (long long)base, lane, px, py, pz, sE, sR, sAC + cs * 32, sNS + cs * 32);
-            if (lane == 0) lp_mbar_arrive(full_u32 + 8 * cs);      // (lp_chunk_phase1 ends with __syncwarp)
+            if (lane == 0) {                // (lp_chunk_phase1 ends with __syncwarp)
+                sTag[cs] = t;
+                lp_mbar_arrive(full_u32 + 8 * cs);
+            }
         }
         return;
     }
@@ -821,6 +835,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
         const uint32_t base = chunk_base(k);
         const int nchunk = (int)(np - base < 32u ? np - base : 32u);      // rows of this chunk
         lp_mbar_wait(full_u32 + 8 * cs, use & 1u);                         // the chunk's coefficients
+        while (sTag[cs] != t) { __nanosleep(64); lp_mbar_wait(full_u32 + 8 * cs, use & 1u); }
         const double2 *my_ac = sAC + cs * 32;
         const int *my_ns = sNS + cs * 32;
 #pragma unroll 1
@@ -902,7 +917,10 @@ __global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spect
             if (++slot == S) { slot = 0; parity ^= 1u; }
         }
         __syncwarp();                                                     // every lane is done with the slot
-        if (lane == 0) lp_mbar_arrive(empty_u32 + 8 * cs);
+        if (lane == 0) {
+            sDone[cs] = t;
+            lp_mbar_arrive(empty_u32 + 8 * cs);
+        }
     }
     if (lane == 0) lp_bulk_wait_all();
 }
