@@ -608,6 +608,24 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #ifndef LP_BULK_NP128
 #define LP_BULK_NP128 4
 #endif
+// the staged kernel (lp_spectral_update: one stencil per particle instead of three) needs fewer of them; same sweep,
+// workload-4 size: 64 bins 5 / 6 / 7 / 8: 3.25 / 3.23 / 3.39 / 3.48 ms; 128 bins 2 / 3 / 4 / 5: 6.93 / 5.90 / 6.28 / 6.39 ms;
+// workload 5: 16 bins 6 / 8 / 10 / 12: 0.660 / 0.611 / 0.682 / 0.682 ms; 256 bins 2 / 3 / 4: 3.38 / 3.48 / 3.53 ms
+#ifndef LP_BULK_NPS16
+#define LP_BULK_NPS16 8
+#endif
+#ifndef LP_BULK_NPS32
+#define LP_BULK_NPS32 8
+#endif
+#ifndef LP_BULK_NPS64
+#define LP_BULK_NPS64 6
+#endif
+#ifndef LP_BULK_NPS128
+#define LP_BULK_NPS128 3
+#endif
+#ifndef LP_BULK_NPS256
+#define LP_BULK_NPS256 2
+#endif
 #ifndef LP_BULK_L2HINT
 #define LP_BULK_L2HINT 1        // row loads and stores of N_b <= 128 carry an L2 evict-first policy (rows are touched
                                 // once per step, grid records by many particles); measured +2 % (64 bins) to +8 %
@@ -629,7 +647,7 @@ __device__ __forceinline__ void lp_fence_async_smem() { asm volatile("fence.prox
 #define LP_BULK_GROUP 1         // consecutive chunks dealt to a block at a time (power of two)
 #endif
 
-template <int NB>
+template <int NB, bool FUSED>
 struct LpBulkCfg {
     static constexpr int M = (NB / 32 > LP_BULK_M) ? NB / 32 : LP_BULK_M;   // bins per lane
     static constexpr int G = NB / M;                              // lanes per row
@@ -639,7 +657,8 @@ struct LpBulkCfg {
     static constexpr int R = SLOT_BYTES / ROW_BYTES;              // rows per slot
     static constexpr int GPC = 32 / R;                            // slots ("groups") per chunk of 32 rows
     static constexpr int S = LP_BULK_DEPTH;                       // ring depth per row warp
-    static constexpr int NP = NB <= 16 ? LP_BULK_NP16 : NB == 32 ? LP_BULK_NP32 : NB == 64 ? LP_BULK_NP64 : NB == 128 ? LP_BULK_NP128 : LP_BULK_NP256;
+    static constexpr int NP = FUSED ? (NB <= 16 ? LP_BULK_NP16 : NB == 32 ? LP_BULK_NP32 : NB == 64 ? LP_BULK_NP64 : NB == 128 ? LP_BULK_NP128 : LP_BULK_NP256)
+                                    : (NB <= 16 ? LP_BULK_NPS16 : NB == 32 ? LP_BULK_NPS32 : NB == 64 ? LP_BULK_NPS64 : NB == 128 ? LP_BULK_NPS128 : LP_BULK_NPS256);
     static constexpr int NR = LP_BULK_WARPS - NP;                 // particle warps, row warps
     static constexpr int D = LP_BULK_COEF_DEPTH;                  // coefficient ring, in chunks
     static constexpr int THREADS = (NP + NR) * 32;
@@ -665,10 +684,10 @@ struct LpBulkCfg {
 // full[slot] / empty[slot] mbarriers (one arrival each) hand the coefficient slots back and forth.
 // Row indices are 32-bit inside the kernel (lp_create limits np to 2^32 - 1); only addresses are 64-bit.
 template <int NB, bool DIAG, int MODE>
-__global__ void __launch_bounds__(LpBulkCfg<NB>::THREADS, LP_BULK_MINB) lp_spectral_bulk_kernel(LpSpectralArgs A)
+__global__ void __launch_bounds__(LpBulkCfg<NB, (MODE >= 1)>::THREADS, LP_BULK_MINB) lp_spectral_bulk_kernel(LpSpectralArgs A)
 {
     constexpr bool FUSED = MODE >= 1, PERM = MODE == 2;
-    using C = LpBulkCfg<NB>;
+    using C = LpBulkCfg<NB, (MODE >= 1)>;
     constexpr int G = C::G, M = C::M, PPW = C::PPW, R = C::R, GPC = C::GPC, S = C::S, RI = C::RI;
     constexpr int NP = C::NP, NR = C::NR, D = C::D;
 
@@ -942,7 +961,7 @@ int launch_variant(const LpSpectralArgs &a, int sm_count, int *blocks_cache, cud
 {
     const long long nchunks = (a.np + 31) >> 5;
     if constexpr (NB <= LP_BULK_MAX_NB) {
-        using C = LpBulkCfg<NB>;
+        using C = LpBulkCfg<NB, (MODE >= 1)>;
         auto kernel = lp_spectral_bulk_kernel<NB, DIAG, MODE>;
         if (*blocks_cache == 0) {
             if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_TOTAL) != cudaSuccess) return -1;
