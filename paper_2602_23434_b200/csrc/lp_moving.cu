@@ -61,7 +61,9 @@ __device__ __forceinline__ double2 lp_moving_coef(const LpMovingArgs &A, long lo
 // of a short row and needs more blocks to hide behind), four above (measured: 64 bins 0.806 -> 0.828 of the copy
 // bandwidth with six, 128 / 256 bins 0.89 / 0.90 -> 0.875 / 0.865; eight blocks or eight rows in flight lose
 // everywhere).  The fused kernel (push stages in the per-particle phase: three stencils, the corner records kept
-// in registers between them) gets four.
+// in registers between them) gets four.  A warp-specialised variant (one particle warp working a group ahead of
+// three row warps, a block barrier per group) was measured slower: 0.74 instead of 0.79 at 64 bins, 0.52 instead
+// of 0.72 at 16.
 // MODE: 0 staged (lp_spectral_update), 1 fused step, 2 fused step that re-sorts (reads through A.perm).
 template <int NB, int MODE>
 __global__ void __launch_bounds__(kThreads, (NB <= 64 && MODE == 0) ? 6 : 4) lp_moving_kernel(LpMovingArgs A)
