@@ -276,6 +276,35 @@ LP_API lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, do
 /* Aggregate diagnostics; synchronises `stream`. */
 LP_API lp_status lp_get_diag(lp_ctx *ctx, lp_diag *out /*host*/, void *stream);
 
+/* The particle number  sum_p sum_i chi[p][i] * widths[i]  (the `number` of lp_diag: what Eq. 2 / Eq. 6 conserve,
+ * PAPER.md:87, 107) for callers that cannot allocate device memory -- and this call allocates none: no cudaMalloc,
+ * no cudaFree, no workspace, no context (lp_create uploads a table with cudaMalloc, and lp_get_diag wants the
+ * multi-GB workspace of the whole step).  Meant for a conservation monitor inside a host code that gave all device
+ * memory to its own arena at start-up, for a diagnostic fired while other streams run (cudaMalloc / cudaFree
+ * stall the whole device), and for code that sits where the allocating runtime calls are forbidden.
+ *   device   CUDA ordinal the pointers live on (made current for the call, the previous one restored)
+ *   chi      device [np][nbins] doubles, particle-major, 8-byte aligned, read only
+ *   widths   device [nbins] doubles: the dE_i of lp_get_bins, copied to the device by the caller
+ *   number   device [1] double, written on `stream`; the caller reads it after synchronising (0 for np = 0)
+ *   err      host buffer for a one-line reason when the status is not LP_OK (there is no context to hold
+ *            one), or NULL; err_len its size
+ * The scratch -- one partial sum per 2048 rows -- is a 64 KiB array compiled into the library, resident on every GPU
+ * that loads liblp_b200.so for the life of the process.  Hence the limits: np <= LP_NUMBER_STATIC_MAX_NP rows
+ * (2^24: workload 4 of BASELINE.json; sum larger sets slice by slice) and nbins <= LP_NUMBER_STATIC_MAX_NBINS;
+ * beyond them LP_ERR_UNSUPPORTED with the reason in err, nothing launched.
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress, which may make the driver load
+ * the library's code on that device): make that first call during set-up, before any stream capture and before
+ * the phase in which the device must not be disturbed.  Later calls only enqueue two kernels on `stream`.
+ * All calls on one device share the array: two calls whose kernels can overlap on the GPU (different streams, no
+ * event between them) race on it and both results are garbage; calls on one stream, or ordered by events, are
+ * safe.  Nothing in the array has to start at zero and nothing of a previous call is read.  The sum order
+ * depends on (np, nbins) only, so the result is bitwise reproducible across GPUs and runs; it agrees with
+ * lp_get_diag's number to rounding, not bit for bit. */
+#define LP_NUMBER_STATIC_MAX_NP    ((int64_t)1 << 24)
+#define LP_NUMBER_STATIC_MAX_NBINS 512
+LP_API lp_status lp_number_static(int device, const double *chi, const double *widths, int32_t nbins, int64_t np,
+                                  double *number, void *stream, char *err /*host*/, size_t err_len);
+
 /* Number of kernel launches the library has enqueued so far on this context. */
 LP_API lp_status lp_launch_count(const lp_ctx *ctx, int64_t *out /*host*/);
 

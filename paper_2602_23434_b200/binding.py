@@ -22,7 +22,7 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack",
            "lp_capacity", "lp_workspace_bytes_for", "lp_rebind",
            "lp_bind_energy_grid", "lp_init_energy_grid", "lp_rebind_energy_grid", "lp_current_energy_grid",
-           "lp_interpolate_tiled")
+           "lp_interpolate_tiled", "lp_number_static")
 
 
 class LPError(RuntimeError):
@@ -106,6 +106,7 @@ def load():
     lib.lp_migrate_count.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int64), C.POINTER(C.c_int64), vp]
     lib.lp_migrate_pack.argtypes = [vp, dp, dp, vp]
     lib.lp_migrate_unpack.argtypes = [vp, dp, C.c_int64, dp, C.c_int64, C.POINTER(C.c_int64), vp]
+    lib.lp_number_static.argtypes = [C.c_int, dp, dp, C.c_int32, C.c_int64, dp, vp, C.c_char_p, C.c_size_t]
     for name in EXPORTS:
         if name != "lp_last_error":
             getattr(lib, name).restype = C.c_int
@@ -331,6 +332,15 @@ def lp_measure_fp64_peak(device=0):
     if st != LP_OK:
         raise LPError(st)
     return out.value
+
+
+def lp_number_static(device, chi_ptr, widths_ptr, nbins, np_, number_ptr, stream=None):
+    """The allocation-free particle number (include/lp.h): device pointers in, one double written at number_ptr on
+    `stream`.  Needs no context; the reason of a refusal comes back in the exception."""
+    err = C.create_string_buffer(256)
+    st = load().lp_number_static(int(device), chi_ptr, widths_ptr, int(nbins), int(np_), number_ptr, stream, err, len(err))
+    if st != LP_OK:
+        raise LPError(st, err.value.decode())
 
 
 def lp_get_bins(ctx, nbins):

@@ -158,3 +158,17 @@ def test_set_count_stays_within_capacity():
         assert lib.lp_set_count(ctx, C.c_int64(0)) == B.LP_OK
     finally:
         lib.lp_destroy(ctx)
+
+
+def test_number_static_refuses_oversize_without_touching_the_gpu():
+    """lp_number_static (the allocation-free entry point) checks its sizes before any CUDA call: the refusal and
+    its reason can be had on a box without a GPU."""
+    with pytest.raises(B.LPError) as e:
+        B.lp_number_static(0, 8, 8, 64, (1 << 24) + 1, 8, None)
+    assert e.value.status == B.LP_ERR_UNSUPPORTED and "static scratch" in str(e.value)
+    with pytest.raises(B.LPError) as e:
+        B.lp_number_static(0, 8, 8, 0, 10, 8, None)
+    assert e.value.status == B.LP_ERR_UNSUPPORTED
+    with pytest.raises(B.LPError) as e:
+        B.lp_number_static(-1, 8, 8, 64, 10, 8, None)
+    assert e.value.status == B.LP_ERR_INVALID_ARG
