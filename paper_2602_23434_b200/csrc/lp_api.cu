@@ -934,7 +934,7 @@ lp_status lp_migrate_pack(lp_ctx *ctx, void *buf_left, void *buf_right, void *st
     if (nleave > 0) {
         LP_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
         const lp_ctx::Set n = ctx->now();
-        st = count(ctx, lp_launch_migrate_pack(ctx->at<unsigned long long>(ctx->lay.partial), nleave, ctx->at<uint32_t>(ctx->lay.idx_b),
+        st = count(ctx, lp_launch_migrate_pack(ctx->mig_left, ctx->mig_right, ctx->at<uint32_t>(ctx->lay.idx_b),
                                                n.x, n.y, n.z, n.id, n.chi, ctx->eng, ctx->cfg.nbins, buf_left, buf_right, ctx->sm_count,
                                                static_cast<cudaStream_t>(stream)), "exchange pack kernel launch");
         if (st != LP_OK) return st;

@@ -115,7 +115,7 @@ size_t lp_migrate_block_elems(long long np);
 int lp_launch_migrate_count(const double *pos, long long np, double lo, double hi, double len, int periodic,
                             uint32_t *dest, unsigned long long *blk, unsigned long long *counts, uint32_t *hole,
                             uint32_t *leaver, cudaStream_t s);
-int lp_launch_migrate_pack(const unsigned long long *counts, long long nleavers, const uint32_t *leaver,
+int lp_launch_migrate_pack(long long n_left, long long n_right, const uint32_t *leaver,
                            const double *x, const double *y, const double *z, const uint64_t *id, const double *chi,
                            const double *eng /*or NULL*/, int nbins, void *buf_left, void *buf_right, int sm_count,
                            cudaStream_t s);

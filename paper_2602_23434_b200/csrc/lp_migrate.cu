@@ -159,12 +159,13 @@ __device__ __forceinline__ LpMigBuf lp_mig_view(void *base, unsigned long long n
 
 // step 4: a warp per leaver
 __global__ void __launch_bounds__(kThreads)
-lp_mig_pack_kernel(const unsigned long long *__restrict__ counts, const uint32_t *__restrict__ leaver,
+lp_mig_pack_kernel(unsigned long long nl, unsigned long long nr, const uint32_t *__restrict__ leaver,
                    const double *__restrict__ x, const double *__restrict__ y, const double *__restrict__ z,
                    const uint64_t *__restrict__ id, const double *__restrict__ chi, const double *__restrict__ eng,
                    int nbins, void *buf_left, void *buf_right)
 {
-    const unsigned long long nl = counts[0], nr = counts[1];
+    // (nl, nr by value: the host holds them since lp_migrate_count synchronised for them, and the device copy sits in
+    // scratch that lp_get_diag may overwrite between count and pack)
     const LpMigBuf L = lp_mig_view(buf_left, nl, nbins), R = lp_mig_view(buf_right, nr, nbins);
     const int lane = threadIdx.x & 31;
     const long long gw = ((long long)blockIdx.x * kThreads + threadIdx.x) >> 5;
@@ -234,15 +235,15 @@ int lp_launch_migrate_count(const double *pos, long long np, double lo, double h
     return ok() ? 3 : -1;
 }
 
-int lp_launch_migrate_pack(const unsigned long long *counts, long long nleavers, const uint32_t *leaver,
+int lp_launch_migrate_pack(long long n_left, long long n_right, const uint32_t *leaver,
                            const double *x, const double *y, const double *z, const uint64_t *id, const double *chi,
                            const double *eng, int nbins, void *buf_left, void *buf_right, int sm_count, cudaStream_t s)
 {
-    long long blocks = (nleavers + kWarps - 1) / kWarps;
+    long long blocks = (n_left + n_right + kWarps - 1) / kWarps;
     const long long cap = (long long)sm_count * 8;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
-    lp_mig_pack_kernel<<<(int)blocks, kThreads, 0, s>>>(counts, leaver, x, y, z, id, chi, eng, nbins, buf_left, buf_right);
+    lp_mig_pack_kernel<<<(int)blocks, kThreads, 0, s>>>((unsigned long long)n_left, (unsigned long long)n_right, leaver, x, y, z, id, chi, eng, nbins, buf_left, buf_right);
     return ok() ? 1 : -1;
 }
 

@@ -167,3 +167,29 @@ def test_exchange_degenerate_sets(n, lo, hi):
         back = orc.migrate_unpack(np.zeros(0, dtype=np.int64), left, right, *want)
         for g, w_ in zip(gpu_state(lp), back):
             assert np.array_equal(g, w_)
+
+
+def test_diag_between_count_and_pack_leaves_the_exchange_alone():
+    """lp.h allows any call that moves no particle between lp_migrate_count and lp_migrate_pack.  lp_get_diag is
+    one, and its per-block partial sums used to land on the device copy of the leaver totals that the pack kernel
+    read (round-2 advisor finding): count -> diag -> pack -> unpack must give the oracle's buffers and state."""
+    rng = np.random.default_rng(17)
+    nb = 32
+    lp, st = make_rank([-1, -1, -1], [0, 1, 1], 3000 + 11, nb, 3200, rng, 5, -1.0, 1.0, 0.5)
+    dest, holes, left, right = orc.migrate_pack(0, -1.0, 0.0, -1.0, 1.0, 1, *st)
+    nl, nr = lp.migrate_count(0, -1.0, 0.0)
+    assert (nl, nr) == (left[0].shape[0], right[0].shape[0]) and nl > 0 and nr > 0
+    d = lp.diag()                                           # writes fp64 partial sums into the shared scratch
+    assert d["np"] == 3000 + 11 and d["number"] > 0
+    bl, br = lp.migrate_pack(nl, nr)
+    torch.cuda.synchronize()
+    for got, want in ((decode(bl, nl, nb), left), (decode(br, nr, nb), right)):
+        for g, w_ in zip(got, want):
+            assert np.array_equal(g, w_)
+    lp.diag()
+    n_new = lp.migrate_unpack(br, nr, bl, nl)               # the leavers come back in, right buffer first
+    want = orc.migrate_unpack(holes, right, left, *st)
+    assert n_new == want[0].shape[0] == 3000 + 11
+    torch.cuda.synchronize()
+    for g, w_ in zip(gpu_state(lp), want):
+        assert np.array_equal(g, w_)
