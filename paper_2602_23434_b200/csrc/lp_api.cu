@@ -1136,6 +1136,7 @@ lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *h
     LP_CUDA(ctx, cudaMemcpyAsync(n.y, hy, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
     LP_CUDA(ctx, cudaMemcpyAsync(n.z, hz, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
     LP_CUDA(ctx, cudaMemcpyAsync(n.id, hid, np * 8, cudaMemcpyHostToDevice, ctx->s_in));
+    ctx->id_bits_stale = true;                          // as in the whole-array branch: these may be other ids
     ++ctx->steps;
     for (int b = 0; b < kBatches; ++b) {
         const size_t p0 = (size_t)b * per;

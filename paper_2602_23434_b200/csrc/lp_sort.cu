@@ -283,7 +283,16 @@ lp_cell_rank_kernel(const uint32_t *__restrict__ key, const uint32_t *__restrict
     if (n > 1) {
         if (n > (uint32_t)kMaxSeg) { *overflow = 1u; return; }
         const uint64_t mine = id[p];
-        for (uint32_t j = 0; j < n; ++j) r += seg_id[o + j] < mine ? 1u : 0u;
+        uint32_t same = 0;
+        for (uint32_t j = 0; j < n; ++j) {
+            const uint64_t other = seg_id[o + j];
+            r += other < mine ? 1u : 0u;
+            same += other == mine ? 1u : 0u;
+        }
+        // ids are unique by contract (lp.h).  Two equal ids in one cell would get the same rank, write one slot of
+        // perm twice and leave another stale: hand such a set to the radix passes instead, which are stable (equal
+        // (key, id) pairs stay in index order) -- a caller's bug then costs time, not a particle.
+        if (same > 1) { *overflow = 1u; return; }
     }
     perm[o + r] = (uint32_t)p;
 }

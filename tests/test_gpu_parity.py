@@ -484,12 +484,15 @@ def test_nsub_when_cfl_ratio_is_next_to_an_integer(nbins, diag):
 
 # ------------------------------------------------------------------ a2 after injection: ids wider than any bound id
 
+@pytest.mark.parametrize("np_", [6000, 30000])
 @pytest.mark.parametrize("pingpong", [False, True])
-def test_sort_after_compaction_and_injection_of_wider_ids(pingpong):
+def test_sort_after_compaction_and_injection_of_wider_ids(pingpong, np_):
     """The number of radix passes over the ids must follow the ids that are there when the sort runs, not
     those bound at the start: delete some particles, inject new ones with ids far above every earlier id
-    (more significant bits), raise the count, sort -- the order must be the oracle's (key, id) order."""
-    w = small_turbulent(n=6, np_=6000, nbins=16)
+    (more significant bits), raise the count, sort -- the order must be the oracle's (key, id) order.
+    6000 particles on 216 cells stay inside the counting sort (at most 64 per cell); 30000 put about 139 in
+    every cell, so the sort falls back to the radix passes, the one consumer of the measured id width."""
+    w = small_turbulent(n=6, np_=np_, nbins=16)
     lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, pingpong=pingpong)
     lp.sort()                                                     # a sort with the narrow ids first
     x, y, z, pid, chi, _, _ = oracle_sort_state(prm, x, y, z, pid, chi)
@@ -511,6 +514,33 @@ def test_sort_after_compaction_and_injection_of_wider_ids(pingpong):
     sx, sy, sz, sid, schi, skey, perm = oracle_sort_state(prm, x, y, z, pid, chi)
     assert np.array_equal(host(lp.id).view(np.uint64), sid)
     assert np.array_equal(host(lp.x), sx) and np.array_equal(host(lp.chi), schi)
+
+
+@pytest.mark.parametrize("pingpong", [False, True])
+def test_sort_with_duplicate_ids_loses_no_particle(pingpong):
+    """Ids are unique by contract, but a caller's bug (an uninitialised tail after lp_set_count) must not cost a
+    particle: with equal ids inside one cell the rank-counting sort used to write one slot of the permutation twice
+    (round-2 advisor finding).  Such a set now goes through the stable radix passes: the result is ordered by
+    (key, id) and is a permutation of what went in -- the order among equal pairs is not unique and not compared."""
+    w = small_turbulent(n=6, np_=5000 + 1, nbins=16)
+    lp, prm, f_np, x, y, z, pid, chi = setup_pair(w, shuffle_ids=True, pingpong=pingpong)
+    key = orc.cell_key(prm, x, y, z)
+    order = np.argsort(key, kind="stable")
+    pid = pid.copy()
+    for a, b in zip(order[:-1:7], order[1::7]):              # neighbours in key order: mostly the same cell
+        if key[a] == key[b]:
+            pid[b] = pid[a]
+    assert len(np.unique(pid)) < w.np - 100
+    chi[:, 0] = np.arange(w.np)                               # a tag that tells the rows apart
+    lp.bind_particles(x, y, z, pid, chi)
+    lp.sort()
+    gid = host(lp.id).view(np.uint64); gx = host(lp.x); gchi = host(lp.chi)
+    src = gchi[:, 0].astype(np.int64)
+    assert np.array_equal(np.sort(src), np.arange(w.np))     # a permutation: nobody twice, nobody lost
+    assert np.array_equal(gid, pid[src]) and np.array_equal(gx, x[src]) and np.array_equal(gchi, chi[src])
+    gkey = key[src].astype(np.uint64)
+    pairs = list(zip(gkey.tolist(), gid.tolist()))
+    assert pairs == sorted(pairs)
 
 
 # ------------------------------------------------------------------ seeded random configurations
