@@ -702,6 +702,12 @@ __global__ void __launch_bounds__(LpBulkCfg<NB, (MODE >= 1)>::THREADS, LP_BULK_M
     // wait on the phase before last.  With 8 + 8 or 4 + 12 warps and 32 slots that cannot happen (a slot's chunks
     // all belong to one particle warp and one row warp); with 7 + 9, 10 + 6, 3 + 13 it can, so every wait is
     // confirmed against the chunk number and repeated if the slot is not there yet.
+    // Ordering.  A wait that passed on the right phase is an acquire paired with the other side's releasing arrive.
+    // A wait that passed on a stale phase is not, and the confirmation loop may then leave through the tag alone.  So
+    // the tag itself carries the ordering: the writer's lane 0 (behind the __syncwarp that orders the other lanes'
+    // sAC / sNS accesses before it) fences and then stores the tag; the reader loads the tag and then fences -- the
+    // release and acquire patterns of the PTX memory model on a relaxed (volatile) word.  Whoever reads tag == t
+    // therefore sees the slot's coefficients of chunk t (sTag), resp. is past the last read of them (sDone).
     volatile uint32_t *sTag = reinterpret_cast<volatile uint32_t *>(sNS + D * 32);
     volatile uint32_t *sDone = sTag + D;
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(sm + C::SMEM_RING + C::SMEM_TAB + C::SMEM_COEF);
@@ -774,9 +780,11 @@ __global__ void __launch_bounds__(LpBulkCfg<NB, (MODE >= 1)>::THREADS, LP_BULK_M
             if (use >= 1) {                 // the slot's previous chunk (t - D) has been consumed
                 lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u);
                 while (sDone[cs] != t - D) { __nanosleep(64); lp_mbar_wait(empty_u32 + 8 * cs, (use - 1) & 1u); }
+                __threadfence_block();      // acquire side of sDone
             }
             lp_chunk_phase1<NB, FUSED>(A, (long long)base, lane, px, py, pz, sE, sR, sAC + cs * 32, sNS + cs * 32);
             if (lane == 0) {                // (lp_chunk_phase1 ends with __syncwarp)
+                __threadfence_block();      // release side of sTag
                 sTag[cs] = t;
                 lp_mbar_arrive(full_u32 + 8 * cs);
             }
@@ -855,6 +863,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB, (MODE >= 1)>::THREADS, LP_BULK_M
         const int nchunk = (int)(np - base < 32u ? np - base : 32u);      // rows of this chunk
         lp_mbar_wait(full_u32 + 8 * cs, use & 1u);                         // the chunk's coefficients
         while (sTag[cs] != t) { __nanosleep(64); lp_mbar_wait(full_u32 + 8 * cs, use & 1u); }
+        __threadfence_block();              // acquire side of sTag
         const double2 *my_ac = sAC + cs * 32;
         const int *my_ns = sNS + cs * 32;
 #pragma unroll 1
@@ -937,6 +946,7 @@ __global__ void __launch_bounds__(LpBulkCfg<NB, (MODE >= 1)>::THREADS, LP_BULK_M
         }
         __syncwarp();                                                     // every lane is done with the slot
         if (lane == 0) {
+            __threadfence_block();          // release side of sDone
             sDone[cs] = t;
             lp_mbar_arrive(empty_u32 + 8 * cs);
         }
