@@ -57,12 +57,15 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--repeats", type=int, default=5,
-                    help="timed passes of --steps in all (SURVEY.md 8(d): median of 5); `value` is the first one")
+                    help="timed passes of --steps in all (SURVEY.md 8(d): median of 5); `value` is the median pass")
     ap.add_argument("--no-pingpong", action="store_true",
                     help="keep the state in the bound arrays across re-sorts (permute pass + copies) instead of "
                          "lp_set_pingpong (re-sort folded into the fused kernel)")
     ap.add_argument("--energy-grid", action="store_true",
                     help="per-particle moving energy grid (lp_bind_energy_grid, NEXT-5) instead of the fixed bins")
+    ap.add_argument("--no-sweep", action="store_true",
+                    help="leave out the `sweep` key (the other BASELINE.json configs, run after the main line of the "
+                         "default workload-4 invocation)")
     ap.add_argument("--no-parity", action="store_true", help="skip the oracle check of the timed state")
     ap.add_argument("--parity-sample", type=int, default=2048)
     return ap.parse_args()
@@ -74,6 +77,30 @@ def measured_peak():
         return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def fp64_peak(device):
+    """(TFLOP/s, clock record): the device's fp64 FMA rate from bench_fp64_peak.cu (independent DFMA chains, 8 per
+    thread, 512 threads x 4 blocks per SM, best of three), built here with nvcc when missing or stale, with the SM
+    clock sampled while it runs.  A bench-side helper: the product library does not carry it."""
+    import ctypes
+    import subprocess
+    src, lib = os.path.join(ROOT, "bench_fp64_peak.cu"), os.path.join(ROOT, "bench_fp64_peak.so")
+    if not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+        tmp = lib + ".tmp%d" % os.getpid()
+        subprocess.run(["/usr/local/cuda/bin/nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-shared",
+                        "-Xcompiler", "-fPIC", "-o", tmp, src], check=True, capture_output=True)
+        os.replace(tmp, lib)
+    fn = ctypes.CDLL(lib).bench_fp64_peak
+    fn.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+    out = ctypes.c_double()
+    sampler = ClockSampler(device)
+    sampler.start()
+    st = fn(int(device), ctypes.byref(out))
+    clocks = sampler.stop()
+    if st != 0:
+        raise RuntimeError("bench_fp64_peak failed (%d)" % st)
+    return out.value, clocks
 
 
 def stored_traffic(wname, nbins, staged=False):
@@ -284,12 +311,13 @@ def parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_rows_fn, dt, n
 
 # ------------------------------------------------------------------------------- inputs
 
-def make_inputs(w, device):
-    """fields on `device`, u_rad, positions/ids (numpy) and a function building chi rows."""
+def make_inputs(w, device, fields=None):
+    """fields on `device` (made here unless handed in), u_rad, positions/ids (numpy) and a function building chi rows."""
     import numpy as np
     import torch
     import lp_inputs as I
-    fields = I.make_fields(w, device=device)
+    if fields is None:
+        fields = I.make_fields(w, device=device)
     u_rad = w.u_rad_frac * I.mean_magnetic_energy(fields) if w.u_rad_frac > 0 else 0.0
     x, y, z, pid = I.make_particles(w, shuffle_ids=True)
     row = I.make_spectrum(w.scaled(np=1), jitter=False)[0]
@@ -303,6 +331,147 @@ def make_inputs(w, device):
 
     chi_host.rows = lambda sel: amp[sel, None] * row[None, :]
     return fields, u_rad, x, y, z, pid, chi_host, chi_device
+
+
+def make_stepper(lp, w, dt, staged, field_at, pusher="rk2"):
+    """one_step() advances the state by one step through the API the run is about (fused lp_step, or the staged
+    calls with the fields re-set between the stages); nstep[0] counts the steps taken."""
+    nstep = [0]
+
+    def one_step():
+        k = nstep[0]
+        nstep[0] += 1
+        if not staged:
+            lp.step(dt)
+            return
+        if w.sort_every and k % w.sort_every == 0:
+            lp.sort()
+        if field_at is not None:
+            lp.set_fields(field_at(k))
+        if pusher == "rk3":
+            for stage in range(3):
+                if stage == 1 and field_at is not None:
+                    lp.set_fields(field_at(k + 1))
+                lp.push_rk3(dt, stage)
+        else:
+            lp.push(dt, 0)
+            if field_at is not None:
+                lp.set_fields(field_at(k + 1))
+            lp.push(dt, 1)
+        lp.spectral_update(dt)
+
+    return one_step, nstep
+
+
+def algorithmic_bytes(w, staged, moving=False):
+    """Algorithmic bytes of one launch of the dominant kernel:
+      rows: chi in and out, 16 N_b per particle (moving grid: chi and the N_b + 1 edges in and out);
+      state: fused lp_step x,y,z in and out (48); staged lp_spectral_update x,y,z and rho_old in (32);
+      grid: the (vx,vy,vz,rho,bx,by,bz) of every distinct cell the gathers touch, once: 56 B x
+            min(cells, 8 corners x particles) -- the three gathers of the fused kernel share their cells."""
+    rows = 16 * (2 * w.nbins + 1) * w.np if moving else 16 * w.nbins * w.np
+    state = (32 if staged else 48) * w.np
+    grid = 56 * min(w.n ** 3, 8 * w.np)
+    return rows, state, grid
+
+
+def algorithmic_flops(w, sum_substeps, moving=False):
+    """fp64 flops of one launch: per bin and substep the donor-cell update is 3 multiply-adds (6 flop), plus 12 flop
+    per bin once for the edge velocities and the update coefficients (moving grid: 16 per bin, no substeps)."""
+    if moving:
+        return 16.0 * w.nbins * w.np
+    return 6.0 * w.nbins * sum_substeps + 12.0 * w.nbins * w.np
+
+
+def sweep_point(P, index, nbins, dev, local, peak, alu_peak, cache, nsample=512):
+    """One entry of the `sweep` key: BASELINE.json configs[index - 1] (at `nbins` bins for the sweep of configs[4]) for
+    its own number of steps after 3 warm-up steps, timed like the main line (CUDA events around the steps, the
+    dominant kernel through lp_timing), then a seeded sample of the timed state replayed by the oracle."""
+    import torch
+    import lp_inputs as I
+    B = P.binding
+    w = I.workload(index)
+    if nbins:
+        w = w.scaled(nbins=nbins)
+    dt = step_dt(w)
+    staged = w.field_kind == "homologous"
+    warm, steps = 3, w.steps
+    key = (w.index, w.n, w.seed)
+    if cache.get("key") != key:                 # the fields depend on the grid and the seed, not on the bin count
+        cache.clear()
+        torch.cuda.empty_cache()
+        cache["key"] = key
+        cache["fields"] = I.make_fields(w, device=dev)
+        cache["np"] = None
+    fields, u_rad, x, y, z, pid, chi_host, chi_device = make_inputs(w, dev, fields=cache["fields"])
+    lp = P.LP(P.config_from_workload(w, u_rad=u_rad, device=local))
+    lp.set_fields(fields)
+    lp.bind_particles(x, y, z, pid, chi_device())
+    lp.set_pingpong(True)
+    field_at = None
+    if staged:
+        field_sets = [I.make_fields(w, t=k * dt, device=dev) for k in range(warm + steps + 1)]
+        field_at = lambda k: field_sets[k]
+    one_step, nstep = make_stepper(lp, w, dt, staged, field_at)
+    for _ in range(warm):
+        one_step()
+    torch.cuda.synchronize(dev)
+    B.lp_timing_enable(lp.ctx, steps)
+    sampler = ClockSampler(local)
+    sampler.start()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(steps):
+        one_step()
+    t1.record()
+    torch.cuda.synchronize(dev)
+    clocks = sampler.stop()
+    ms = t0.elapsed_time(t1)
+    sp_ms, sp_n = B.lp_timing_read(lp.ctx)
+    B.lp_timing_enable(lp.ctx, 0)
+    d = lp.diag()
+    if field_at is None:
+        if cache.get("np") is None:
+            cache["np"] = [f.cpu().numpy() for f in fields]
+        fnp = cache["np"]
+        fields_for_step = lambda k: (fnp, fnp)
+    else:
+        fields_for_step = lambda k: tuple([f.cpu().numpy() for f in field_at(k + j)] for j in (0, 1))
+    parity = parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_host.rows, dt, nstep[0], nsample, dev)
+    rows_b, state_b, grid_b = algorithmic_bytes(w, staged)
+    alg = rows_b + state_b + grid_b
+    k_ms = sp_ms / max(sp_n, 1)
+    ach = alg / (k_ms * 1e-3) / 1e9 if sp_n else None
+    traffic = stored_traffic(w.name, w.nbins, staged)
+    flops = algorithmic_flops(w, d["sum_substeps"])
+    out = {"workload": "configs[%d] %s" % (w.index - 1, w.name), "grid": "%d^3" % w.n, "particles": w.np,
+           "nbins": w.nbins, "api": "staged, fields re-set between the stages" if staged else "fused lp_step",
+           "steps": steps, "warmup": warm, "ms_per_step": ms / steps,
+           "value": w.np * steps / (ms * 1e-3), "kernel_ms": k_ms, "achieved": ach,
+           "frac": (ach / peak) if ach else None, "whole_step_frac": alg / (ms / steps * 1e-3) / 1e9 / peak,
+           "alu_frac": (flops / (k_ms * 1e-3) / 1e12 / alu_peak) if (alu_peak and sp_n) else None,
+           "mean_substeps": d["sum_substeps"] / max(1, d["np"]),
+           "traffic_over_algorithmic": (traffic / alg) if traffic else None,
+           "parity_checked": {k: parity[k] for k in ("particles", "steps", "max_rel", "positions_bit_exact", "ok")},
+           "clocks": clocks}
+    lp.close()
+    return out
+
+
+def run_sweep(P, dev, local, peak, alu_peak):
+    """The configurations of BASELINE.json the main line is not quoted on: configs[0], [1], [2] and the bin sweep of
+    configs[4] (the GB/s-vs-bins curve), each for its own step count, in this process.  Workloads 1 and 2 are
+    parity cases at sizes (1 024 and 65 536 particles) where a launch is latency, not bandwidth: their fractions
+    are reported for completeness, the bound applies to configs[2]-[4]."""
+    cache = {}
+    out = []
+    for index, nbins in ((1, 0), (2, 0), (3, 0), (5, 16), (5, 32), (5, 64), (5, 128), (5, 256), (5, 512)):
+        try:
+            out.append(sweep_point(P, index, nbins, dev, local, peak, alu_peak, cache))
+        except Exception as e:          # noqa: BLE001 -- one failed point must not cost the main line
+            out.append({"workload": "configs[%d]" % (index - 1), "nbins": nbins, "error": repr(e)})
+    cache.clear()
+    return out
 
 
 # ------------------------------------------------------------------------------- arms
@@ -383,29 +552,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    nstep = [0]
-
-    def one_step():
-        k = nstep[0]
-        nstep[0] += 1
-        if not staged:
-            lp.step(dt)
-            return
-        if w.sort_every and k % w.sort_every == 0:
-            lp.sort()
-        if field_at is not None:
-            lp.set_fields(field_at(k))
-        if args.pusher == "rk3":
-            for stage in range(3):
-                if stage == 1 and field_at is not None:
-                    lp.set_fields(field_at(k + 1))
-                lp.push_rk3(dt, stage)
-        else:
-            lp.push(dt, 0)
-            if field_at is not None:
-                lp.set_fields(field_at(k + 1))
-            lp.push(dt, 1)
-        lp.spectral_update(dt)
+    one_step, nstep = make_stepper(lp, w, dt, staged, field_at, args.pusher)
 
     def timed_pass():
         B.lp_timing_enable(lp.ctx, args.steps)
@@ -424,14 +571,31 @@ def run_ours(args):
     for _ in range(args.warmup):
         one_step()
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    ms, launches, spec_ms, spec_n = timed_pass()           # the K steps `value` is quoted on
-    clocks = sampler.stop()
+    # ---- `repeats` passes of the same K steps, each with its own clock record.  `value`, `ms_per_step`, `roofline`
+    # and `clocks` are those of the MEDIAN pass (SURVEY.md 8(d) "median of 5 repeats"): the first pass runs at the
+    # boost clock, later ones under the power cap, and the kernel follows the SM clock.
+    passes = []
+    for _ in range(max(1, args.repeats)):
+        sampler = ClockSampler(local)
+        sampler.start()
+        m, ln, sm_, sn_ = timed_pass()
+        passes.append({"ms": m, "launches": ln, "spec_ms": sm_, "spec_n": sn_, "clocks": sampler.stop()})
+    B.lp_timing_enable(lp.ctx, 0)
+    order = sorted(range(len(passes)), key=lambda i: passes[i]["ms"])
+    quoted = order[(len(order) - 1) // 2] if len(order) % 2 == 0 else order[len(order) // 2]
+    q = passes[quoted]
+    ms, launches, spec_ms, spec_n, clocks = q["ms"], q["launches"], q["spec_ms"], q["spec_n"], q["clocks"]
     d = lp.diag()
     value = aggregate_rate(world, w.np, args.steps, ms * 1e-3)
+    repeats = {"passes": len(passes), "steps_per_pass": args.steps, "quoted_pass": quoted,
+               "quoted": "median of the passes by time (value, ms_per_step, roofline, clocks are this pass's)",
+               "ms_per_step": [p_["ms"] / args.steps for p_ in passes],
+               "value": [aggregate_rate(world, w.np, args.steps, p_["ms"] * 1e-3) for p_ in passes],
+               "dominant_kernel_ms": [p_["spec_ms"] / max(p_["spec_n"], 1) for p_ in passes],
+               "clocks": [p_["clocks"] for p_ in passes]}
 
-    # ---- the timed state against the oracle (rank 0 of a single-GPU run; the oracle is test infrastructure)
+    # ---- the timed state (after every pass) against the oracle (rank 0 of a single-GPU run; the oracle is test
+    # infrastructure)
     parity = None
     fields_np = None
     if world == 1 and not args.no_parity and args.pusher == "rk2":
@@ -442,23 +606,6 @@ def run_ours(args):
             fields_for_step = lambda k: tuple([f.cpu().numpy() for f in field_at(k + j)] for j in (0, 1))
         parity = parity_check(lp, w, fields_for_step, u_rad, x, y, z, pid, chi_host.rows, dt, nstep[0],
                               args.parity_sample, dev, moving=args.energy_grid)
-
-    # ---- further passes of the same K steps: median of all (SURVEY.md 8(d) "median of 5 repeats")
-    passes = [(ms, spec_ms, spec_n)]
-    sampler2 = ClockSampler(local)
-    sampler2.start()
-    for _ in range(max(1, args.repeats) - 1):
-        m, _, sm_, sn_ = timed_pass()
-        passes.append((m, sm_, sn_))
-    clocks2 = sampler2.stop()
-    B.lp_timing_enable(lp.ctx, 0)
-    med = sorted(passes)[len(passes) // 2]
-    repeats = {"passes": len(passes), "steps_per_pass": args.steps,
-               "ms_per_step": [p_[0] / args.steps for p_ in passes],
-               "median_ms_per_step": med[0] / args.steps,
-               "median_value": aggregate_rate(world, w.np, args.steps, med[0] * 1e-3),
-               "dominant_kernel_ms": [p_[1] / max(p_[2], 1) for p_ in passes],
-               "clocks_after_first_pass": clocks2}
 
     # ---- n_sub histogram of one more step; binding n_sub alone keeps the kernel instantiation
     nsub_hist = None
@@ -583,17 +730,7 @@ def run_ours(args):
     if rank != 0:
         return
     peak, peak_src = measured_peak()
-    # Algorithmic bytes of one launch of the dominant kernel:
-    #   rows: chi in and out, 16 N_b per particle;
-    #   state: fused lp_step x,y,z in and out (48); staged lp_spectral_update x,y,z and rho_old in (32);
-    #   grid: the (vx,vy,vz,rho,bx,by,bz) of every distinct cell the gathers touch, once: 56 B x
-    #         min(cells, 8 corners x particles) -- the three gathers of the fused kernel share their cells.
-    rows_bytes = 16 * w.nbins * w.np
-    state_bytes = (32 if staged else 48) * w.np
-    if args.energy_grid:        # moving grid: chi and the N_b + 1 edges in and out; x, y, z, rho_old in
-        rows_bytes = 16 * (2 * w.nbins + 1) * w.np
-        state_bytes = (32 if staged else 48) * w.np
-    grid_bytes = 56 * min(w.n ** 3, 8 * w.np)
+    rows_bytes, state_bytes, grid_bytes = algorithmic_bytes(w, staged, args.energy_grid)
     alg_bytes = rows_bytes + state_bytes + grid_bytes
     spec_avg_ms = spec_ms / max(spec_n, 1)
     achieved = alg_bytes / (spec_avg_ms * 1e-3) / 1e9 if spec_n else None
@@ -603,17 +740,17 @@ def run_ours(args):
     # The secondary bound ("report both fractions"): fp64 arithmetic.  Algorithmic flops of a row:
     # per bin and substep the donor-cell update is 3 multiply-adds (6 flop), plus 12 flop per bin once for the
     # edge velocities and the update coefficients; the substep total is the kernel's own count (lp_get_diag).
-    # Peak: the device's fp64 FMA rate measured now by the library (lp_measure_fp64_peak, independent DFMA chains).
+    # Peak: the device's fp64 FMA rate measured now by bench_fp64_peak.cu (independent DFMA chains), with its clocks.
     alu = None
+    alu_peak = None
     try:
-        alu_peak = B.lp_measure_fp64_peak(local)
-        flops = 6.0 * w.nbins * d["sum_substeps"] + 12.0 * w.nbins * w.np
-        if args.energy_grid:    # per bin: t = 1 + beta e, e' = alpha e / t (a division ~ 10 flop), chi' = chi t t_up / alpha
-            flops = 16.0 * w.nbins * w.np
+        alu_peak, alu_clocks = fp64_peak(local)
+        flops = algorithmic_flops(w, d["sum_substeps"], args.energy_grid)
         alu_ach = flops / (spec_avg_ms * 1e-3) / 1e12 if spec_n else None
         alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s (fp64)",
                "frac": (alu_ach / alu_peak) if alu_ach else None,
-               "peak_source": "measured now: lp_measure_fp64_peak (8 DFMA chains/thread, 512 threads x 4 blocks/SM, best of 3)",
+               "peak_source": "measured now: bench_fp64_peak.cu (8 DFMA chains/thread, 512 threads x 4 blocks/SM, best of 3)",
+               "peak_clocks": alu_clocks,
                "algorithmic_flops_per_launch": flops,
                "flop_per_byte": flops / alg_bytes}
     except Exception as e:          # noqa: BLE001 -- the line is still valid without the secondary bound
@@ -656,6 +793,14 @@ def run_ours(args):
         if fields_np is None:
             fields_np = [f.cpu().numpy() for f in fields]
         out["cpu_baseline"] = cpu_baseline(w, fields_np, u_rad, x, y, z, pid, chi_host, dt, args.cpu_seconds)
+    default_run = (args.workload == 4 and not (args.nbins or args.np or args.grid) and args.sort_every < 0
+                   and not staged and not args.energy_grid and args.pusher == "rk2")
+    if world == 1 and default_run and not args.no_sweep:
+        # the other configurations of BASELINE.json (configs[0]-[2] and the bin sweep of configs[4]) in the same line
+        lp.close()
+        del lp, fields, fields_np
+        torch.cuda.empty_cache()
+        out["sweep"] = run_sweep(P, dev, local, peak, alu_peak)
     print(json.dumps(out), flush=True)
     if dist is not None:
         dist.barrier()

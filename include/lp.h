@@ -315,12 +315,6 @@ LP_API lp_status lp_launch_count(const lp_ctx *ctx, int64_t *out /*host*/);
 LP_API lp_status lp_timing_enable(lp_ctx *ctx, int max_records);
 LP_API lp_status lp_timing_read(lp_ctx *ctx, double *spectral_ms_sum /*host*/, int32_t *n_records /*host*/);
 
-/* fp64 FMA rate of `device` in TFLOP/s (2 flop per DFMA), measured with a kernel of independent dependent-FMA
- * chains (8 per thread, 512 threads x 4 blocks per SM, best of three): the denominator of the arithmetic
- * roofline bench.py prints beside the HBM one for the bin counts whose rows take many substeps.  Needs no
- * context; allocates and frees 8 B per thread; synchronises the device. */
-LP_API lp_status lp_measure_fp64_peak(int device, double *tflops /*host*/);
-
 /* Copy the library's bin table to host arrays: edges [nbins+1], widths [nbins] (either may be NULL). */
 LP_API lp_status lp_get_bins(const lp_ctx *ctx, double *edges /*host*/, double *widths /*host*/);
 

@@ -18,7 +18,7 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_bind_particles", "lp_bind_diag", "lp_set_fields", "lp_interpolate", "lp_sort", "lp_push",
            "lp_spectral_update", "lp_step", "lp_step_host", "lp_get_diag", "lp_launch_count", "lp_get_bins",
            "lp_timing_enable", "lp_timing_read", "lp_get_cfl_bins", "lp_shock_update", "lp_compact", "lp_push_rk3", "lp_chunked_capacity", "lp_set_count",
-           "lp_measure_fp64_peak", "lp_set_pingpong", "lp_current_particles",
+           "lp_set_pingpong", "lp_current_particles",
            "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack",
            "lp_capacity", "lp_workspace_bytes_for", "lp_rebind",
            "lp_bind_energy_grid", "lp_init_energy_grid", "lp_rebind_energy_grid", "lp_current_energy_grid",
@@ -92,7 +92,6 @@ def load():
     lib.lp_timing_enable.argtypes = [vp, C.c_int]
     lib.lp_get_cfl_bins.argtypes = [vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.lp_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
-    lib.lp_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
     lib.lp_set_pingpong.argtypes = [vp, C.c_int, vp]
     lib.lp_current_particles.argtypes = [vp] + [C.POINTER(C.c_void_p)] * 5
     lib.lp_bind_energy_grid.argtypes = [vp, dp, dp]
@@ -324,14 +323,6 @@ def lp_timing_read(ctx):
     ms = C.c_double(); n = C.c_int32()
     _check(ctx, load().lp_timing_read(ctx, C.byref(ms), C.byref(n)))
     return ms.value, n.value
-
-
-def lp_measure_fp64_peak(device=0):
-    out = C.c_double()
-    st = load().lp_measure_fp64_peak(int(device), C.byref(out))
-    if st != LP_OK:
-        raise LPError(st)
-    return out.value
 
 
 def lp_number_static(device, chi_ptr, widths_ptr, nbins, np_, number_ptr, stream=None):

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblp_b200.so")
-SOURCES = ["lp_api.cu", "lp_particles.cu", "lp_spectral.cu", "lp_sort.cu", "lp_shock.cu", "lp_compact.cu", "lp_migrate.cu", "lp_moving.cu", "lp_measure.cu", "lp_static.cu"]
+SOURCES = ["lp_api.cu", "lp_particles.cu", "lp_spectral.cu", "lp_sort.cu", "lp_shock.cu", "lp_compact.cu", "lp_migrate.cu", "lp_moving.cu", "lp_static.cu"]
 HEADERS = ["lp_internal.h", "lp_device.cuh", os.path.join("..", "..", "include", "lp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
