@@ -273,8 +273,18 @@ LP_API lp_status lp_current_particles(const lp_ctx *ctx, double **x, double **y,
 LP_API lp_status lp_step_host(lp_ctx *ctx, double dt, double *hx, double *hy, double *hz,
                        uint64_t *hid, double *hchi, void *stream);
 
-/* Aggregate diagnostics; synchronises `stream`. */
+/* Aggregate diagnostics; synchronises `stream` (the one argument beyond SURVEY.md 8(b)'s signature: the reduction
+ * kernels must be ordered behind the caller's work). */
 LP_API lp_status lp_get_diag(lp_ctx *ctx, lp_diag *out /*host*/, void *stream);
+
+/* What a hit cap means.  A particle whose CFL-limited substep count exceeds config.max_substeps takes max_substeps
+ * substeps instead (n_sub reads negative, lp_diag.n_capped counts it): each of them is longer than the CFL bound
+ * allows, the explicit scheme is unstable there and the row is no longer a solution of Eq. 6 to any
+ * stated accuracy.  By default that is only reported.  With error_on_cap != 0, lp_get_diag fills *out as usual and
+ * returns LP_ERR_UNSUPPORTED when the last spectral update capped any particle, so that a driver loop that checks
+ * its diagnostics never carries such rows on unnoticed.  (Kernels run asynchronously: the diagnostics call is the
+ * first point where the host can know.) */
+LP_API lp_status lp_set_cap_policy(lp_ctx *ctx, int error_on_cap);
 
 /* The particle number  sum_p sum_i chi[p][i] * widths[i]  (the `number` of lp_diag: what Eq. 2 / Eq. 6 conserve,
  * PAPER.md:87, 107) for callers that cannot allocate device memory -- and this call allocates none: no cudaMalloc,

@@ -22,7 +22,7 @@ EXPORTS = ("lp_create", "lp_destroy", "lp_last_error", "lp_workspace_bytes", "lp
            "lp_migrate_record_bytes", "lp_migrate_count", "lp_migrate_pack", "lp_migrate_unpack",
            "lp_capacity", "lp_workspace_bytes_for", "lp_rebind",
            "lp_bind_energy_grid", "lp_init_energy_grid", "lp_rebind_energy_grid", "lp_current_energy_grid",
-           "lp_interpolate_tiled", "lp_number_static")
+           "lp_interpolate_tiled", "lp_number_static", "lp_set_cap_policy")
 
 
 class LPError(RuntimeError):
@@ -105,6 +105,7 @@ def load():
     lib.lp_migrate_count.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int64), C.POINTER(C.c_int64), vp]
     lib.lp_migrate_pack.argtypes = [vp, dp, dp, vp]
     lib.lp_migrate_unpack.argtypes = [vp, dp, C.c_int64, dp, C.c_int64, C.POINTER(C.c_int64), vp]
+    lib.lp_set_cap_policy.argtypes = [vp, C.c_int]
     lib.lp_number_static.argtypes = [C.c_int, dp, dp, C.c_int32, C.c_int64, dp, vp, C.c_char_p, C.c_size_t]
     for name in EXPORTS:
         if name != "lp_last_error":
@@ -301,6 +302,10 @@ def lp_get_diag(ctx, stream=None):
     d = lp_diag()
     _check(ctx, load().lp_get_diag(ctx, C.byref(d), stream))
     return d.as_dict()
+
+
+def lp_set_cap_policy(ctx, error_on_cap):
+    _check(ctx, load().lp_set_cap_policy(ctx, int(bool(error_on_cap))))
 
 
 def lp_launch_count(ctx):

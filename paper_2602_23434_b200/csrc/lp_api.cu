@@ -160,6 +160,7 @@ struct lp_ctx {
     int rk3_next = 0;                      // next stage lp_push_rk3 expects
     bool status_valid = false;             // the status array describes the bound particles in their current order
     bool push_done = false;                // a pusher ran to its last stage since stage 0 (x^{n+1} is in place)
+    bool cap_is_error = false;             // lp_set_cap_policy: lp_get_diag refuses a state with capped rows
     bool id_bits_stale = true;             // ids may have changed since id_bits was measured (bind, injection, host copy)
     int spectral_blocks[6] = { 0, 0, 0, 0, 0, 0 };   // resident blocks per SM of the spectral kernel variants [diag][mode], 0 = not set up
     long long capacity = 0;                // particles the workspace was sized for (cfg.np shrinks in lp_compact)
@@ -1191,6 +1192,16 @@ lp_status lp_get_diag(lp_ctx *ctx, lp_diag *out, void *stream)
     out->n_outside = h.n_outside;
     out->number = h.number;
     out->lost = h.lost;
+    if (ctx->cap_is_error && h.n_capped > 0)        // (out is filled: the caller can still see how many)
+        return fail(ctx, LP_ERR_UNSUPPORTED, "particles hit max_substeps in the last spectral update: their rows took "
+                                             "substeps beyond the CFL bound (raise max_substeps or lower dt)");
+    return LP_OK;
+}
+
+lp_status lp_set_cap_policy(lp_ctx *ctx, int error_on_cap)
+{
+    if (!ctx) return LP_ERR_INVALID_ARG;
+    ctx->cap_is_error = error_on_cap != 0;
     return LP_OK;
 }
 

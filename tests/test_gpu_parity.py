@@ -192,6 +192,14 @@ def test_spectral_update_sign_changing_advection_and_cap():
     d = lp.diag()
     assert d["n_capped"] == int(capped.sum()) and d["max_substeps"] == 12
     assert d["sum_substeps"] == int(np.abs(nsub).sum())
+    # The compare of the capped rows above is a sanity check (same order of magnitude, no garbage), not a parity
+    # claim: such rows are outside the method.  A caller who wants them to be an error gets one:
+    B.lp_set_cap_policy(lp.ctx, True)
+    with pytest.raises(B.LPError) as e:
+        lp.diag()
+    assert e.value.status == B.LP_ERR_UNSUPPORTED and "max_substeps" in str(e.value)
+    B.lp_set_cap_policy(lp.ctx, False)
+    assert lp.diag()["n_capped"] == int(capped.sum())
 
 
 def test_number_conservation_diag():
